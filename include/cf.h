@@ -1,0 +1,174 @@
+/*
+ * cf.h -- C ABI of the B200-native plan-evaluation hot path (libcf_b200.so).
+ *
+ * What it computes: for many candidate deployment plans at once, the per-request-type SLO-hit
+ * counts (hence goodput, "the throughput of type-t requests that meet their latency target",
+ * PAPER.md:139) of arxiv/paper_2512_14098's request-level simulation phase (Algorithm 2 l.13-15,
+ * PAPER.md:252-255; sec. 4.3). One independent discrete simulation runs per
+ * (plan p, arrival rate r, trial k): requests of each type follow their path through the plan's
+ * ordered stages and queue at a c-replica executor pool at every visited stage (Lindley recursion
+ * for c = 1, Kiefer-Wolfowitz free-time multiset for c > 1). The exact integer model -- Philox4x32-10
+ * counters, integer quantile tables, rounding -- is written out in DESIGN.md ("Algorithm", readings
+ * R1..R19); results are bit-exact with the CPU oracle under oracle/.
+ *
+ * Conventions
+ *  - No floating point crosses this ABI. Times are int64 microseconds, services int32 microseconds,
+ *    rates uint32 milli-requests/s, gaps Q16 (65536 == one mean inter-arrival gap).
+ *  - "host" pointers are read during the call only (descriptors, tables, plan lists: small).
+ *    "dev" pointers are CUDA device pointers (e.g. torch.Tensor.data_ptr()); the caller owns all
+ *    memory; nothing persistent is allocated by the library.
+ *  - Every compute call takes a cudaStream_t (as void*), enqueues its work on it and returns
+ *    without synchronising (host-side scheduling happens before the first launch). Scratch comes
+ *    from the caller's `workspace` (dev, >= cf_workspace_bytes(), 256-byte aligned); it must stay
+ *    untouched until the stream work has finished. Distinct streams + distinct workspaces are
+ *    thread-safe; there is no global state.
+ *  - Return value: CF_OK or a negative cf_status. Argument errors are detected on the host before
+ *    anything is enqueued. Conditions that depend on device data (a rate outside [1, 1e9] mrps, or
+ *    arrivals that would exceed 2^62 us, R17) are detected on the device: that
+ *    simulation's outputs are all zero and a sticky CF_ERR_RANGE is recorded in the workspace,
+ *    readable with cf_workspace_status().
+ */
+#ifndef CF_H
+#define CF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  CF_OK = 0,
+  CF_ERR_ARG = -1,   /* null pointer, size out of bounds, bad table id                         */
+  CF_ERR_RANGE = -2, /* overflow guard (services, edge delay, rate, arrival horizon, c, smem)  */
+  CF_ERR_PLAN = -3,  /* c = 0, masks overlap / miss a used component, order violates a DAG edge */
+  CF_ERR_TABLE = -4, /* quantile table decreasing, negative, or of unsupported shape            */
+  CF_ERR_CUDA = -5,  /* a CUDA runtime call failed                                              */
+  CF_ERR_WORKSPACE = -6 /* workspace NULL, misaligned or smaller than cf_workspace_bytes()     */
+} cf_status;
+
+/* Tail-refined integer quantile table (R3; stands for a latency profile "sampled from
+ * profiling results"). levels*2^log2_cells + 1 entries, non-decreasing, >= 0.
+ * Level k < levels-1 covers quantiles [1-2^-k, 1-2^-(k+1)), the last level [1-2^-(levels-1), 1);
+ * each level has 2^log2_cells equal cells; entry (k,m) is the quantile at the left edge of cell m;
+ * the final entry closes the last cell. 1 <= levels <= 32, log2_cells <= 16. q: host. */
+typedef struct {
+  uint32_t levels, log2_cells;
+  const int32_t* q;
+} cf_qtab;
+
+/* Model definition graph + workload. All pointers host. */
+typedef struct {
+  uint32_t n_comp, n_types, n_req, n_trials; /* C<=8, T<=8, 1<=N<=2^24 requests per sim, K trials */
+  const uint8_t* type_mask;    /* [T] bit i: type visits component i; components in topological order */
+  const uint32_t* type_thresh; /* [T] cumulative mix pi_t in Q32, non-decreasing; last entry ignored */
+  const uint16_t* svc_tab;     /* [C*T] id of the service table of (component i, type t) at i*T+t   */
+  const cf_qtab* tabs;         /* [n_tabs] service tables, entries int32 microseconds              */
+  uint32_t n_tabs;
+  cf_qtab arr_tab;             /* unit-mean inter-arrival gap, entries Q16                         */
+  const uint8_t* edges;        /* [2*n_edges] (u,v): component u feeds component v (validation)    */
+  uint32_t n_edges;
+  int64_t edge_delay_us;       /* PAPER.md:322; added between consecutive visited stages; [0,2^31) */
+} cf_graph;
+
+/* P physical plans; plan p is an ORDERED list of n_stages[p] stages, stage s = (bitmask of the
+ * components colocated on that node, replica count c >= 1) (nodes/executors: PAPER.md:127,199-221).
+ * Masks are disjoint within a plan and cover every component some type uses. All pointers host. */
+typedef struct {
+  uint32_t n_plans, max_stages; /* max_stages <= 8 */
+  const uint8_t* n_stages;      /* [P] */
+  const uint8_t* stage_mask;    /* [P*max_stages] */
+  const uint16_t* stage_c;      /* [P*max_stages] */
+} cf_plans;
+
+/* Per-type latency targets L_t and the attainment target used by the rate
+ * bisection (R12): feasible iff hits_t*att_den[t] >= att_num[t]*cnt_t for all t. host. */
+typedef struct {
+  const int64_t* L_us;     /* [T] */
+  const uint32_t* att_num; /* [T] (bisection only; may be NULL for cf_eval_plans) */
+  const uint32_t* att_den; /* [T] */
+} cf_slo;
+
+/* Upper bound of the scratch any call below needs for (graph, plans, R rates per plan). */
+size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R);
+
+/* cf_eval_plans: simulate every (plan p, rate r, trial k), p<P, r<R, k<K.
+ *   rate_mrps    dev [P*R]  arrival rate of (p,r) in milli-requests/s, valid range [1, 1e9]
+ *   seed         Philox key; variant = Philox counter word 3 (decorrelates streams, R4)
+ *   out_counts   dev [P][R][K][T][2] = {cnt_t, hits_t}: requests of type t, and those with
+ *                sojourn D_n - A_n <= L_t (F_{t,d}(L_t) = hits_t/cnt_t)
+ *   out_dep_sum  dev [P][R][K] sum of final departures mod 2^64, or NULL
+ *   out_makespan dev [P][R][K] max final departure (R10), or NULL                               */
+int32_t cf_eval_plans(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps, uint32_t R,
+                      const cf_slo* slo, uint64_t seed, uint32_t variant, uint32_t* out_counts,
+                      uint64_t* out_dep_sum, int64_t* out_makespan, void* workspace,
+                      size_t workspace_bytes, void* stream);
+
+/* cf_goodput_bisect: per plan, n_steps steps of integer bisection on the rate (PAPER.md:340
+ * "the highest request rate that the plan can support"), entirely on the device: lo = 0,
+ * hi = rate_hi_mrps[p] (exclusive); mid = lo + (hi-lo)/2; mid == lo -> no-op; else run the K trials
+ * at mid, pool counts, feasible -> lo = mid else hi = mid (R12, R18).
+ *   rate_hi_mrps     dev [P]
+ *   out_rate_mrps    dev [P]     rate* = final lo
+ *   out_goodput_mrps dev [P][T]  floor(rate* * hits_t / (N*K)), hits pooled at rate* (R10)
+ *   out_counts       dev [P][K][T][2] counts at rate* (zeros if rate* = 0), or NULL               */
+int32_t cf_goodput_bisect(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_hi_mrps,
+                          uint32_t n_steps, const cf_slo* slo, uint64_t seed, uint32_t variant,
+                          uint32_t* out_rate_mrps, uint32_t* out_goodput_mrps, uint32_t* out_counts,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/* Materialised request stream (north_star "request stream materialised in HBM"), C <= 6 only.
+ * Record (32 bytes, 16-byte aligned): { uint64 cu | (type << 56) ; int32 svc[6] } where cu is the
+ * cumulative Q16 gap up to and including the request and svc[i] the sampled service of component i
+ * if the request's type visits i, else 0. Layout [n_variants][K][N]; variant index vi holds Philox
+ * variant variant_lo + vi. cf_stream_bytes = n_variants*K*N*32. */
+size_t cf_stream_bytes(const cf_graph* g, uint32_t n_variants);
+int32_t cf_materialize_stream(const cf_graph* g, uint64_t seed, uint32_t variant_lo,
+                              uint32_t n_variants, void* out_stream /* dev */, void* workspace,
+                              size_t workspace_bytes, void* stream);
+
+/* As cf_eval_plans / cf_goodput_bisect, but requests are read from a materialised stream instead
+ * of being drawn in registers; results are bit-identical to the in-register calls with
+ * variant = variant_lo + plan_variant. plan_variant: host [P] index in [0,n_variants) of the
+ * stream variant plan p reads, or NULL for p % n_variants. */
+int32_t cf_eval_plans_stream(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps,
+                             uint32_t R, const cf_slo* slo, const void* stream_records /* dev */,
+                             uint32_t n_variants, const uint32_t* plan_variant,
+                             uint32_t* out_counts, uint64_t* out_dep_sum, int64_t* out_makespan,
+                             void* workspace, size_t workspace_bytes, void* stream);
+int32_t cf_goodput_bisect_stream(const cf_graph* g, const cf_plans* pl,
+                                 const uint32_t* rate_hi_mrps, uint32_t n_steps, const cf_slo* slo,
+                                 const void* stream_records /* dev */, uint32_t n_variants,
+                                 const uint32_t* plan_variant, uint32_t* out_rate_mrps,
+                                 uint32_t* out_goodput_mrps, uint32_t* out_counts, void* workspace,
+                                 size_t workspace_bytes, void* stream);
+
+/* Parity/debug: per-request trace of one simulation (plan, rate, trial): system arrival A_n,
+ * final departure D_n and type, dev [N] each (any may be NULL). rate_mrps is a host value. */
+int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint32_t rate_mrps,
+                     uint32_t trial, uint64_t seed, uint32_t variant, int64_t* out_arrival,
+                     int64_t* out_departure, uint8_t* out_type, void* workspace,
+                     size_t workspace_bytes, void* stream);
+
+/* Synchronises `stream`, reads the sticky device status of the last call that used `workspace`
+ * and returns it (CF_OK, CF_ERR_RANGE, or CF_ERR_CUDA). */
+int32_t cf_workspace_status(const void* workspace, void* stream);
+
+/* Number of kernels the last call on this workspace's host thread enqueued (bench bookkeeping). */
+uint32_t cf_last_launch_count(void);
+
+/* Micro-benchmark used by bench.py for the ALU roofline denominator: runs `iters` rounds of an
+ * unrolled, independent 32-bit integer instruction mix on every SM and writes the number of
+ * lane-operations executed to *out_ops (host). mix: 0 = IADD3/LOP3 only (ALU pipe), 1 = IMAD only
+ * (FMA pipe), 2 = alternating. Returns the elapsed milliseconds * 1000 (microseconds) in
+ * *out_usec (host), measured with CUDA events on `stream`. Synchronises. */
+int32_t cf_bench_int32_peak(uint32_t mix, uint32_t iters, uint64_t* out_ops, uint64_t* out_usec,
+                            void* stream);
+
+const char* cf_strerror(int32_t status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -124,6 +124,7 @@ int32_t cf_goodput_bisect(const cf_graph* g, const cf_plans* pl, const uint32_t*
  * if the request's type visits i, else 0. Layout [n_variants][K][N]; variant index vi holds Philox
  * variant variant_lo + vi. cf_stream_bytes = n_variants*K*N*32. */
 size_t cf_stream_bytes(const cf_graph* g, uint32_t n_variants);
+size_t cf_materialize_workspace_bytes(const cf_graph* g, uint32_t n_variants); /* scratch of the call below */
 int32_t cf_materialize_stream(const cf_graph* g, uint64_t seed, uint32_t variant_lo,
                               uint32_t n_variants, void* out_stream /* dev */, void* workspace,
                               size_t workspace_bytes, void* stream);

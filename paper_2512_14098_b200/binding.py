@@ -1,0 +1,283 @@
+"""Thin Python binding of libcf_b200.so (include/cf.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI. PyTorch is used for device
+memory and streams, nothing else. There is no CPU fallback: if the shared library is missing the
+import of this module raises, and without a CUDA device every compute call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcf_b200.so")
+
+CF_OK, CF_ERR_ARG, CF_ERR_RANGE, CF_ERR_PLAN, CF_ERR_TABLE, CF_ERR_CUDA, CF_ERR_WORKSPACE = \
+    0, -1, -2, -3, -4, -5, -6
+
+EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_stream_bytes",
+           "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
+           "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status",
+           "cf_last_launch_count", "cf_bench_int32_peak", "cf_strerror"]
+
+
+class CfError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {strerror(status)} ({status})")
+
+
+class cf_qtab(C.Structure):
+    _fields_ = [("levels", C.c_uint32), ("log2_cells", C.c_uint32), ("q", C.POINTER(C.c_int32))]
+
+
+class cf_graph(C.Structure):
+    _fields_ = [("n_comp", C.c_uint32), ("n_types", C.c_uint32), ("n_req", C.c_uint32),
+                ("n_trials", C.c_uint32), ("type_mask", C.POINTER(C.c_uint8)),
+                ("type_thresh", C.POINTER(C.c_uint32)), ("svc_tab", C.POINTER(C.c_uint16)),
+                ("tabs", C.POINTER(cf_qtab)), ("n_tabs", C.c_uint32), ("arr_tab", cf_qtab),
+                ("edges", C.POINTER(C.c_uint8)), ("n_edges", C.c_uint32),
+                ("edge_delay_us", C.c_int64)]
+
+
+class cf_plans(C.Structure):
+    _fields_ = [("n_plans", C.c_uint32), ("max_stages", C.c_uint32),
+                ("n_stages", C.POINTER(C.c_uint8)), ("stage_mask", C.POINTER(C.c_uint8)),
+                ("stage_c", C.POINTER(C.c_uint16))]
+
+
+class cf_slo(C.Structure):
+    _fields_ = [("L_us", C.POINTER(C.c_int64)), ("att_num", C.POINTER(C.c_uint32)),
+                ("att_den", C.POINTER(C.c_uint32))]
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2512_14098_b200.build` "
+                      "(there is no CPU fallback)")
+_lib = C.CDLL(LIB_PATH)
+_lib.cf_workspace_bytes.restype = C.c_size_t
+_lib.cf_stream_bytes.restype = C.c_size_t
+_lib.cf_materialize_workspace_bytes.restype = C.c_size_t
+_lib.cf_strerror.restype = C.c_char_p
+_lib.cf_last_launch_count.restype = C.c_uint32
+for _n in ("cf_eval_plans", "cf_goodput_bisect", "cf_materialize_stream", "cf_eval_plans_stream",
+           "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak"):
+    getattr(_lib, _n).restype = C.c_int32
+
+
+def strerror(status: int) -> str:
+    return _lib.cf_strerror(C.c_int32(status)).decode()
+
+
+def _hp(a: Optional[np.ndarray], ctype):
+    if a is None:
+        return C.cast(None, C.POINTER(ctype))
+    return a.ctypes.data_as(C.POINTER(ctype))
+
+
+def _dp(t: Optional[torch.Tensor]):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_cuda and t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+class Marshalled:
+    """Host structs of a (graph, plans, slo) triple; keeps the numpy buffers alive."""
+
+    def __init__(self, graph, plans=None, slo=None):
+        self.keep = []
+        g = graph
+        tabs = (cf_qtab * len(g.tabs))()
+        for j, t in enumerate(g.tabs):
+            tabs[j] = cf_qtab(t.levels, t.log2_cells, _hp(t.q, C.c_int32))
+        edges = np.ascontiguousarray(g.edges, dtype=np.uint8).reshape(-1)
+        self.keep += [tabs, edges]
+        self.g = cf_graph(g.n_comp, g.n_types, g.n_req, g.n_trials, _hp(g.type_mask, C.c_uint8),
+                          _hp(g.type_thresh, C.c_uint32), _hp(g.svc_tab, C.c_uint16), tabs,
+                          len(g.tabs), cf_qtab(g.arr_tab.levels, g.arr_tab.log2_cells,
+                                               _hp(g.arr_tab.q, C.c_int32)),
+                          _hp(edges if edges.size else None, C.c_uint8), edges.size // 2,
+                          int(g.edge_delay_us))
+        self.pl = None
+        if plans is not None:
+            sm = np.ascontiguousarray(plans.stage_mask).reshape(-1)
+            sc = np.ascontiguousarray(plans.stage_c).reshape(-1)
+            self.keep += [sm, sc]
+            self.pl = cf_plans(plans.n_plans, plans.max_stages, _hp(plans.n_stages, C.c_uint8),
+                               _hp(sm, C.c_uint8), _hp(sc, C.c_uint16))
+        self.slo = None
+        if slo is not None:
+            self.slo = cf_slo(_hp(slo.L_us, C.c_int64), _hp(slo.att_num, C.c_uint32),
+                              _hp(slo.att_den, C.c_uint32))
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise RuntimeError("libcf_b200 needs a CUDA device (no CPU fallback)")
+
+
+def cf_workspace_bytes(graph, plans, R: int) -> int:
+    m = Marshalled(graph, plans)
+    return int(_lib.cf_workspace_bytes(C.byref(m.g), C.byref(m.pl), C.c_uint32(R)))
+
+
+def alloc_workspace(graph, plans, R: int, device="cuda") -> torch.Tensor:
+    return torch.empty(cf_workspace_bytes(graph, plans, R), dtype=torch.uint8, device=device)
+
+
+def _as_dev_u32(x, device) -> torch.Tensor:
+    """uint32 values as an int32-typed CUDA tensor (bit pattern preserved)."""
+    if isinstance(x, torch.Tensor):
+        assert x.dtype in (torch.int32, torch.uint32)
+        return x.contiguous().to(device)
+    a = np.ascontiguousarray(x, dtype=np.uint32)
+    return torch.from_numpy(a.view(np.int32)).to(device)
+
+
+def cf_workspace_status(workspace: torch.Tensor, stream=None) -> int:
+    return int(_lib.cf_workspace_status(_dp(workspace), _stream_ptr(stream)))
+
+
+def cf_last_launch_count() -> int:
+    return int(_lib.cf_last_launch_count())
+
+
+def cf_eval_plans(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, out_counts=None,
+                  out_dep_sum=None, out_makespan=None, workspace=None, stream=None, aux=True,
+                  stream_records=None, n_variants: int = 1, plan_variant=None, check=True):
+    """cf_eval_plans / cf_eval_plans_stream (if stream_records is given). rate_mrps: [P,R] CUDA int32
+    tensor (uint32 bit pattern) or anything numpy can convert. Returns dict of CUDA tensors:
+    counts int32 [P,R,K,T,2], dep_sum int64 [P,R,K] (uint64 bit pattern), makespan int64 [P,R,K]."""
+    _require_cuda()
+    dev = torch.device("cuda")
+    m = Marshalled(graph, plans, slo)
+    rates = _as_dev_u32(rate_mrps, dev).reshape(plans.n_plans, -1)
+    P, R = rates.shape
+    K, T = graph.n_trials, graph.n_types
+    if out_counts is None:
+        out_counts = torch.empty((P, R, K, T, 2), dtype=torch.int32, device=dev)
+    if aux and out_dep_sum is None:
+        out_dep_sum = torch.empty((P, R, K), dtype=torch.int64, device=dev)
+    if aux and out_makespan is None:
+        out_makespan = torch.empty((P, R, K), dtype=torch.int64, device=dev)
+    if workspace is None:
+        workspace = alloc_workspace(graph, plans, R)
+    if stream_records is None:
+        rc = _lib.cf_eval_plans(C.byref(m.g), C.byref(m.pl), _dp(rates), C.c_uint32(R), C.byref(m.slo),
+                                C.c_uint64(seed), C.c_uint32(variant), _dp(out_counts),
+                                _dp(out_dep_sum), _dp(out_makespan), _dp(workspace),
+                                C.c_size_t(workspace.numel()), _stream_ptr(stream))
+    else:
+        pv = None if plan_variant is None else np.ascontiguousarray(plan_variant, dtype=np.uint32)
+        rc = _lib.cf_eval_plans_stream(C.byref(m.g), C.byref(m.pl), _dp(rates), C.c_uint32(R),
+                                       C.byref(m.slo), _dp(stream_records), C.c_uint32(n_variants),
+                                       _hp(pv, C.c_uint32), _dp(out_counts), _dp(out_dep_sum),
+                                       _dp(out_makespan), _dp(workspace),
+                                       C.c_size_t(workspace.numel()), _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_eval_plans")
+    return dict(counts=out_counts, dep_sum=out_dep_sum, makespan=out_makespan, workspace=workspace,
+                rc=int(rc))
+
+
+def cf_goodput_bisect(graph, plans, rate_hi_mrps, n_steps: int, slo, seed: int, variant: int = 0, *,
+                      workspace=None, stream=None, stream_records=None, n_variants: int = 1,
+                      plan_variant=None, want_counts=True, check=True):
+    """cf_goodput_bisect / cf_goodput_bisect_stream. Returns dict of CUDA tensors: rate_mrps int32 [P],
+    goodput_mrps int32 [P,T], counts int32 [P,K,T,2]."""
+    _require_cuda()
+    dev = torch.device("cuda")
+    m = Marshalled(graph, plans, slo)
+    hi = _as_dev_u32(rate_hi_mrps, dev).reshape(-1)
+    P, K, T = plans.n_plans, graph.n_trials, graph.n_types
+    assert hi.numel() == P
+    rate = torch.empty(P, dtype=torch.int32, device=dev)
+    good = torch.empty((P, T), dtype=torch.int32, device=dev)
+    counts = torch.empty((P, K, T, 2), dtype=torch.int32, device=dev) if want_counts else None
+    if workspace is None:
+        workspace = alloc_workspace(graph, plans, 1)
+    if stream_records is None:
+        rc = _lib.cf_goodput_bisect(C.byref(m.g), C.byref(m.pl), _dp(hi), C.c_uint32(n_steps),
+                                    C.byref(m.slo), C.c_uint64(seed), C.c_uint32(variant), _dp(rate),
+                                    _dp(good), _dp(counts), _dp(workspace),
+                                    C.c_size_t(workspace.numel()), _stream_ptr(stream))
+    else:
+        pv = None if plan_variant is None else np.ascontiguousarray(plan_variant, dtype=np.uint32)
+        rc = _lib.cf_goodput_bisect_stream(C.byref(m.g), C.byref(m.pl), _dp(hi), C.c_uint32(n_steps),
+                                           C.byref(m.slo), _dp(stream_records), C.c_uint32(n_variants),
+                                           _hp(pv, C.c_uint32), _dp(rate), _dp(good), _dp(counts),
+                                           _dp(workspace), C.c_size_t(workspace.numel()),
+                                           _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_goodput_bisect")
+    return dict(rate_mrps=rate, goodput_mrps=good, counts=counts, workspace=workspace, rc=int(rc))
+
+
+def cf_stream_bytes(graph, n_variants: int) -> int:
+    m = Marshalled(graph)
+    return int(_lib.cf_stream_bytes(C.byref(m.g), C.c_uint32(n_variants)))
+
+
+def cf_materialize_stream(graph, seed: int, variant_lo: int, n_variants: int, *, out=None,
+                          stream=None, check=True):
+    """Returns a CUDA uint8 tensor [n_variants, K, N, 32] of stream records."""
+    _require_cuda()
+    m = Marshalled(graph)
+    if out is None:
+        out = torch.empty((n_variants, graph.n_trials, graph.n_req, 32), dtype=torch.uint8, device="cuda")
+    wsb = int(_lib.cf_materialize_workspace_bytes(C.byref(m.g), C.c_uint32(n_variants)))
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    rc = _lib.cf_materialize_stream(C.byref(m.g), C.c_uint64(seed), C.c_uint32(variant_lo),
+                                    C.c_uint32(n_variants), _dp(out), _dp(ws), C.c_size_t(wsb),
+                                    _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_materialize_stream")
+    torch.cuda.current_stream().synchronize() if stream is None else stream.synchronize()  # ws lifetime
+    return out
+
+
+def cf_trace_sim(graph, plans, plan: int, rate_mrps: int, trial: int, seed: int, variant: int = 0, *,
+                 stream=None, check=True):
+    _require_cuda()
+    m = Marshalled(graph, plans)
+    N = graph.n_req
+    arr = torch.empty(N, dtype=torch.int64, device="cuda")
+    dep = torch.empty(N, dtype=torch.int64, device="cuda")
+    typ = torch.empty(N, dtype=torch.uint8, device="cuda")
+    ws = alloc_workspace(graph, plans, 1)
+    rc = _lib.cf_trace_sim(C.byref(m.g), C.byref(m.pl), C.c_uint32(plan), C.c_uint32(rate_mrps),
+                           C.c_uint32(trial), C.c_uint64(seed), C.c_uint32(variant), _dp(arr), _dp(dep),
+                           _dp(typ), _dp(ws), C.c_size_t(ws.numel()), _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_trace_sim")
+    status = cf_workspace_status(ws, stream)
+    return dict(arrival=arr, departure=dep, type=typ, rc=int(rc), status=status)
+
+
+def cf_bench_int32_peak(mix: int, iters: int = 2000, stream=None):
+    """Returns (lane_ops, microseconds) of the integer-issue micro-benchmark."""
+    _require_cuda()
+    ops, usec = C.c_uint64(0), C.c_uint64(0)
+    rc = _lib.cf_bench_int32_peak(C.c_uint32(mix), C.c_uint32(iters), C.byref(ops), C.byref(usec),
+                                  _stream_ptr(stream))
+    if rc != CF_OK:
+        raise CfError(rc, "cf_bench_int32_peak")
+    return int(ops.value), int(usec.value)
+
+
+def to_numpy_u32(t: torch.Tensor) -> np.ndarray:
+    return t.detach().cpu().numpy().view(np.uint32)
+
+
+def to_numpy_u64(t: torch.Tensor) -> np.ndarray:
+    return t.detach().cpu().numpy().view(np.uint64)

@@ -1,0 +1,846 @@
+// cf_api.cu -- host side of libcf_b200: the C ABI of include/cf.h.
+//
+// Validation, scheduling (grouping simulations that share a request stream and a topology into
+// warps and CTAs), workspace layout and kernel launches. All compute runs in the kernels of
+// cf_device.cuh / this file; there is no CPU fallback: without a CUDA device every compute call
+// returns CF_ERR_CUDA.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <numeric>
+#include <vector>
+
+#include "../../include/cf.h"
+#include "cf_device.cuh"
+
+using namespace cfk;
+
+namespace {
+
+thread_local uint32_t g_launch_count = 0;
+
+constexpr size_t kAlign = 256;
+constexpr uint32_t kMaxSmem = 227u * 1024u;
+size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------------------------
+// validation (host logic; mirrors the contract in cf.h, written independently of the oracle)
+// ------------------------------------------------------------------------------------------------
+size_t tab_entries(const cf_qtab& t) { return ((size_t)t.levels << t.log2_cells) + 1; }
+
+int32_t check_tab(const cf_qtab& t) {
+  if (!t.q || t.levels < 1 || t.levels > 32 || t.log2_cells > 16) return CF_ERR_TABLE;
+  const size_t n = tab_entries(t);
+  int32_t prev = 0;
+  for (size_t i = 0; i < n; ++i) {
+    if (t.q[i] < prev) return CF_ERR_TABLE;  // also rejects a negative first entry
+    prev = t.q[i];
+  }
+  return CF_OK;
+}
+
+int32_t check_graph(const cf_graph* g) {
+  if (!g) return CF_ERR_ARG;
+  if (g->n_comp < 1 || g->n_comp > 8 || g->n_types < 1 || g->n_types > 8) return CF_ERR_ARG;
+  if (g->n_req < 1 || g->n_req > (1u << 24) || g->n_trials < 1 || g->n_trials > 65535) return CF_ERR_ARG;
+  if (!g->type_mask || !g->type_thresh || !g->svc_tab || !g->tabs || g->n_tabs < 1) return CF_ERR_ARG;
+  if (g->n_edges && !g->edges) return CF_ERR_ARG;
+  const uint32_t C = g->n_comp, T = g->n_types;
+  for (uint32_t t = 0; t < T; ++t) {
+    if (g->type_mask[t] >> C) return CF_ERR_ARG;
+    if (t && g->type_thresh[t] < g->type_thresh[t - 1]) return CF_ERR_ARG;
+  }
+  for (uint32_t e = 0; e < 2 * g->n_edges; ++e)
+    if (g->edges[e] >= C) return CF_ERR_ARG;
+  for (uint32_t i = 0; i < C; ++i)
+    for (uint32_t t = 0; t < T; ++t)
+      if (((g->type_mask[t] >> i) & 1) && g->svc_tab[i * T + t] >= g->n_tabs) return CF_ERR_ARG;
+  for (uint32_t j = 0; j < g->n_tabs; ++j)
+    if (int32_t rc = check_tab(g->tabs[j])) return rc;
+  if (int32_t rc = check_tab(g->arr_tab)) return rc;
+  if (g->edge_delay_us < 0 || g->edge_delay_us >= (1ll << 31)) return CF_ERR_RANGE;
+  // DESIGN.md R17: a request's total service over all its components must fit int32
+  int64_t worst = 0;
+  for (uint32_t i = 0; i < C; ++i) {
+    int64_t mx = 0;
+    for (uint32_t t = 0; t < T; ++t)
+      if ((g->type_mask[t] >> i) & 1) {
+        const cf_qtab& tb = g->tabs[g->svc_tab[i * T + t]];
+        mx = std::max<int64_t>(mx, tb.q[tab_entries(tb) - 1]);
+      }
+    worst += mx;
+  }
+  if (worst > INT32_MAX) return CF_ERR_RANGE;
+  return CF_OK;
+}
+
+int32_t check_plans(const cf_graph* g, const cf_plans* pl) {
+  if (!pl) return CF_ERR_ARG;
+  if (pl->n_plans < 1 || pl->max_stages < 1 || pl->max_stages > 8) return CF_ERR_ARG;
+  if (!pl->n_stages || !pl->stage_mask || !pl->stage_c) return CF_ERR_ARG;
+  uint32_t used = 0;
+  for (uint32_t t = 0; t < g->n_types; ++t) used |= g->type_mask[t];
+  for (uint32_t p = 0; p < pl->n_plans; ++p) {
+    const uint32_t V = pl->n_stages[p];
+    if (V < 1 || V > pl->max_stages) return CF_ERR_PLAN;
+    uint32_t seen = 0;
+    int where[8] = {-1, -1, -1, -1, -1, -1, -1, -1};
+    for (uint32_t s = 0; s < V; ++s) {
+      const uint32_t m = pl->stage_mask[p * pl->max_stages + s];
+      if (!m || (m >> g->n_comp) || (m & seen)) return CF_ERR_PLAN;
+      if (pl->stage_c[p * pl->max_stages + s] < 1) return CF_ERR_PLAN;
+      seen |= m;
+      for (uint32_t i = 0; i < g->n_comp; ++i)
+        if ((m >> i) & 1) where[i] = (int)s;
+    }
+    if (used & ~seen) return CF_ERR_PLAN;
+    for (uint32_t e = 0; e < g->n_edges; ++e) {
+      const int a = where[g->edges[2 * e]], b = where[g->edges[2 * e + 1]];
+      if (a >= 0 && b >= 0 && a > b) return CF_ERR_PLAN;
+    }
+  }
+  return CF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// schedule
+// ------------------------------------------------------------------------------------------------
+struct Launch {
+  uint32_t cta_begin, n_ctas, smem_bytes;
+};
+
+struct Schedule {
+  std::vector<TopoDesc> topos;
+  std::vector<SimDesc> sims;
+  std::vector<WarpDesc> warps;
+  std::vector<CtaDesc> ctas;
+  std::vector<Launch> launches;
+  std::vector<uint16_t> plan_c;  // [P*8]
+  int vmax = 2;                  // template choice
+  int cmax = 6;
+};
+
+uint32_t heap_rows(uint32_t c) { return c >= 2 ? c : 0; }  // nodes 2..c+1
+
+const uint32_t kSmemClasses[] = {16u << 10, 24u << 10, 32u << 10, 48u << 10, 64u << 10,
+                                 96u << 10, 128u << 10, kMaxSmem};
+
+uint32_t fixed_smem(int vmax, int cmax) {
+  if (cmax <= 6) {
+    if (vmax <= 2) return SmemLayout<2, 6>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout<6, 6>::fixed_bytes;
+    return SmemLayout<8, 6>::fixed_bytes;
+  }
+  return SmemLayout<8, 8>::fixed_bytes;
+}
+
+// plan_sel: which plans take part (all if null); plan_variant: stream variant per plan (0 if null)
+int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
+                       const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
+                       Schedule* out) {
+  const uint32_t P = pl->n_plans, MS = pl->max_stages;
+  Schedule& sc = *out;
+  sc.plan_c.assign((size_t)P * 8, 1);
+  uint32_t maxV = 1;
+  std::map<std::vector<uint8_t>, uint32_t> topo_id;
+  std::vector<uint32_t> plan_topo(P);
+  for (uint32_t p = 0; p < P; ++p) {
+    const uint32_t V = pl->n_stages[p];
+    maxV = std::max(maxV, V);
+    std::vector<uint8_t> key(pl->stage_mask + (size_t)p * MS, pl->stage_mask + (size_t)p * MS + V);
+    auto it = topo_id.find(key);
+    if (it == topo_id.end()) {
+      TopoDesc td;
+      std::memset(&td, 0, sizeof(td));
+      td.n_stages = (uint8_t)V;
+      for (uint32_t s = 0; s < V; ++s) td.mask[s] = key[s];
+      it = topo_id.emplace(key, (uint32_t)sc.topos.size()).first;
+      sc.topos.push_back(td);
+    }
+    plan_topo[p] = it->second;
+    for (uint32_t s = 0; s < V; ++s) sc.plan_c[(size_t)p * 8 + s] = pl->stage_c[(size_t)p * MS + s];
+  }
+  sc.cmax = g->n_comp <= 6 ? 6 : 8;
+  sc.vmax = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 6 ? 6 : 8));
+  const uint32_t fixed = fixed_smem(sc.vmax, sc.cmax);
+
+  // order plans by (variant, topology, replica vector) so that warps are homogeneous
+  std::vector<uint32_t> order;
+  if (only_plan) order.push_back(*only_plan);
+  else { order.resize(P); std::iota(order.begin(), order.end(), 0u); }
+  auto variant_of = [&](uint32_t p) -> uint32_t {
+    if (n_variants <= 1) return 0u;
+    return plan_variant ? plan_variant[p] : p % n_variants;
+  };
+  for (uint32_t p : order)
+    if (variant_of(p) >= std::max(1u, n_variants)) return CF_ERR_ARG;
+  std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) {
+    const uint32_t va = variant_of(a), vb = variant_of(b);
+    if (va != vb) return va < vb;
+    if (plan_topo[a] != plan_topo[b]) return plan_topo[a] < plan_topo[b];
+    // heavier heaps first within a topology, then lexicographic replica vector
+    return std::lexicographical_compare(sc.plan_c.begin() + (size_t)b * 8, sc.plan_c.begin() + (size_t)b * 8 + 8,
+                                        sc.plan_c.begin() + (size_t)a * 8, sc.plan_c.begin() + (size_t)a * 8 + 8);
+  });
+
+  // simulations -> warps (same variant and topology, <= 32 lanes)
+  std::vector<uint32_t> warp_variant;
+  std::vector<uint32_t> warp_heap_bytes;
+  size_t i = 0;
+  while (i < order.size()) {
+    size_t j = i;
+    while (j < order.size() && variant_of(order[j]) == variant_of(order[i]) &&
+           plan_topo[order[j]] == plan_topo[order[i]])
+      ++j;
+    // group [i, j): emit sims plan-major, rate-minor
+    const size_t sim0 = sc.sims.size();
+    for (size_t q = i; q < j; ++q)
+      for (uint32_t r = 0; r < R; ++r) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
+    const size_t n_group = sc.sims.size() - sim0;
+    const TopoDesc& td = sc.topos[plan_topo[order[i]]];
+    for (size_t w0 = 0; w0 < n_group; w0 += 32) {
+      WarpDesc wd;
+      std::memset(&wd, 0, sizeof(wd));
+      wd.sim_begin = (uint32_t)(sim0 + w0);
+      wd.n_lanes = (uint32_t)std::min<size_t>(32, n_group - w0);
+      wd.topo = plan_topo[order[i]];
+      uint32_t off = 0;
+      for (uint32_t s = 0; s < td.n_stages; ++s) {
+        uint32_t rows = 0;
+        for (uint32_t l = 0; l < wd.n_lanes; ++l)
+          rows = std::max(rows, heap_rows(sc.plan_c[(size_t)sc.sims[wd.sim_begin + l].plan * 8 + s]));
+        wd.heap_off[s] = off;
+        off += rows * 256u;
+      }
+      if (fixed + off > kMaxSmem) return CF_ERR_RANGE;  // replica counts too large for one SM
+      sc.warps.push_back(wd);
+      warp_variant.push_back(variant_of(order[i]));
+      warp_heap_bytes.push_back(off);
+    }
+    i = j;
+  }
+
+  // warps -> CTAs (same variant, <= kWarpsPerCta warps, shared memory within the limit)
+  std::vector<CtaDesc> ctas;
+  size_t w = 0;
+  while (w < sc.warps.size()) {
+    CtaDesc cd;
+    cd.warp_begin = (uint32_t)w;
+    cd.n_warps = 0;
+    cd.variant = warp_variant[w];
+    cd.heap_bytes = 0;
+    // keep CTAs at <= 64 KiB where possible so several fit on an SM
+    const uint32_t soft = std::max<uint32_t>(64u << 10, fixed + warp_heap_bytes[w]);
+    while (w < sc.warps.size() && cd.n_warps < (uint32_t)kWarpsPerCta && warp_variant[w] == cd.variant &&
+           fixed + cd.heap_bytes + warp_heap_bytes[w] <= soft) {
+      // heap offsets become CTA-relative
+      for (int s = 0; s < 8; ++s) sc.warps[w].heap_off[s] += cd.heap_bytes;
+      cd.heap_bytes += warp_heap_bytes[w];
+      ++cd.n_warps;
+      ++w;
+    }
+    ctas.push_back(cd);
+  }
+  // launch classes by shared-memory size
+  auto cls = [&](const CtaDesc& c) {
+    const uint32_t need = fixed + c.heap_bytes;
+    for (uint32_t k : kSmemClasses)
+      if (need <= k) return k;
+    return kMaxSmem;
+  };
+  std::stable_sort(ctas.begin(), ctas.end(), [&](const CtaDesc& a, const CtaDesc& b) { return cls(a) > cls(b); });
+  sc.ctas = ctas;
+  for (size_t c = 0; c < ctas.size();) {
+    size_t e = c;
+    while (e < ctas.size() && cls(ctas[e]) == cls(ctas[c])) ++e;
+    sc.launches.push_back(Launch{(uint32_t)c, (uint32_t)(e - c), cls(ctas[c])});
+    c = e;
+  }
+  return CF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// workspace blob
+// ------------------------------------------------------------------------------------------------
+struct Blob {
+  std::vector<uint8_t> bytes;
+  size_t add(const void* src, size_t n) {
+    const size_t off = align_up(bytes.size());
+    bytes.resize(off + n);
+    if (src && n) std::memcpy(bytes.data() + off, src, n);
+    return off;
+  }
+  size_t reserve(size_t n) {  // zero-filled
+    const size_t off = align_up(bytes.size());
+    bytes.resize(off + n, 0);
+    return off;
+  }
+};
+
+size_t pool_entries(const cf_graph* g) {
+  size_t n = tab_entries(g->arr_tab);
+  for (uint32_t j = 0; j < g->n_tabs; ++j) n += tab_entries(g->tabs[j]);
+  return n;
+}
+
+// fills the graph part of KParams and appends the table pool to the blob; returns pool offset
+size_t fill_graph_params(const cf_graph* g, const cf_slo* slo, uint64_t seed, Blob* blob, KParams* kp) {
+  std::memset(kp, 0, sizeof(*kp));
+  kp->C = g->n_comp; kp->T = g->n_types; kp->N = g->n_req; kp->K = g->n_trials;
+  std::vector<int32_t> pool;
+  std::vector<uint32_t> tab_off(g->n_tabs);
+  for (uint32_t j = 0; j < g->n_tabs; ++j) {
+    tab_off[j] = (uint32_t)pool.size();
+    pool.insert(pool.end(), g->tabs[j].q, g->tabs[j].q + tab_entries(g->tabs[j]));
+  }
+  kp->arr_tab = DevTab{(uint32_t)pool.size(), g->arr_tab.levels, g->arr_tab.log2_cells, 0};
+  pool.insert(pool.end(), g->arr_tab.q, g->arr_tab.q + tab_entries(g->arr_tab));
+  for (uint32_t t = 0; t < 8; ++t) {
+    kp->type_thresh[t] = t < g->n_types ? g->type_thresh[t] : 0xffffffffu;
+    kp->type_mask[t] = t < g->n_types ? g->type_mask[t] : 0;
+    kp->L_us[t] = (slo && slo->L_us && t < g->n_types) ? slo->L_us[t] : 0;
+  }
+  for (uint32_t i = 0; i < g->n_comp; ++i)
+    for (uint32_t t = 0; t < g->n_types; ++t)
+      if ((g->type_mask[t] >> i) & 1) {
+        const uint32_t id = g->svc_tab[i * g->n_types + t];
+        kp->svc_tab[i * 8 + t] = DevTab{tab_off[id], g->tabs[id].levels, g->tabs[id].log2_cells, 0};
+      }
+  kp->edge_delay = g->edge_delay_us;
+  kp->seed_lo = (uint32_t)seed;
+  kp->seed_hi = (uint32_t)(seed >> 32);
+  return blob->add(pool.data(), pool.size() * sizeof(int32_t));
+}
+
+struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c; };
+
+SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
+  SchedOffsets o;
+  o.topos = blob->add(sc.topos.data(), sc.topos.size() * sizeof(TopoDesc));
+  o.sims = blob->add(sc.sims.data(), sc.sims.size() * sizeof(SimDesc));
+  o.warps = blob->add(sc.warps.data(), sc.warps.size() * sizeof(WarpDesc));
+  o.ctas = blob->add(sc.ctas.data(), sc.ctas.size() * sizeof(CtaDesc));
+  o.plan_c = blob->add(sc.plan_c.data(), sc.plan_c.size() * sizeof(uint16_t));
+  return o;
+}
+
+void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool_off) {
+  kp->qpool = reinterpret_cast<const int32_t*>(ws + pool_off);
+  kp->topos = reinterpret_cast<const TopoDesc*>(ws + o.topos);
+  kp->sims = reinterpret_cast<const SimDesc*>(ws + o.sims);
+  kp->warps = reinterpret_cast<const WarpDesc*>(ws + o.warps);
+  kp->ctas = reinterpret_cast<const CtaDesc*>(ws + o.ctas);
+  kp->plan_c = reinterpret_cast<const uint16_t*>(ws + o.plan_c);
+  kp->status = reinterpret_cast<int32_t*>(ws);
+}
+
+// ------------------------------------------------------------------------------------------------
+// launches
+// ------------------------------------------------------------------------------------------------
+template <int VMAX, int CMAX, bool HAS_DELAY>
+cudaError_t launch_one(const KParams& kp, const Launch& L, uint32_t n_trials, cudaStream_t st) {
+  auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+  if (e != cudaSuccess) return e;
+  // grid.y is limited to 65535: n_trials <= 65535 is validated
+  kern<<<dim3(L.n_ctas, n_trials), kThreads, L.smem_bytes, st>>>(kp, L.cta_begin);
+  ++g_launch_count;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_sims(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  const bool d = kp.edge_delay != 0;
+  for (const Launch& L : sc.launches) {
+    cudaError_t e;
+    if (sc.cmax == 8) e = d ? launch_one<8, 8, true>(kp, L, n_trials, st) : launch_one<8, 8, false>(kp, L, n_trials, st);
+    else if (sc.vmax == 2) e = d ? launch_one<2, 6, true>(kp, L, n_trials, st) : launch_one<2, 6, false>(kp, L, n_trials, st);
+    else if (sc.vmax == 6) e = d ? launch_one<6, 6, true>(kp, L, n_trials, st) : launch_one<6, 6, false>(kp, L, n_trials, st);
+    else e = d ? launch_one<8, 6, true>(kp, L, n_trials, st) : launch_one<8, 6, false>(kp, L, n_trials, st);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+int32_t check_workspace(void* ws, size_t have, size_t need) {
+  if (!ws || (reinterpret_cast<uintptr_t>(ws) & (kAlign - 1)) || have < need) return CF_ERR_WORKSPACE;
+  return CF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// bisection kernels (a9): all bracket state lives in the workspace, no host round trips
+// ------------------------------------------------------------------------------------------------
+struct BisectState {
+  uint32_t* lo; uint32_t* hi; uint32_t* mid;  // [P]; mid == 0 <=> this step is a no-op for the plan
+  uint32_t* probe;                            // [P][K][T][2] counts of the current probe
+  uint32_t* at_lo;                            // [P][K][T][2] counts remembered for lo
+};
+
+__global__ void bisect_init_kernel(BisectState bs, const uint32_t* rate_hi, uint32_t P, uint32_t per_plan) {
+  const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const uint32_t lo = 0, hi = rate_hi[p];
+  const uint32_t mid = lo + (hi - lo) / 2;
+  bs.lo[p] = lo;
+  bs.hi[p] = hi;
+  bs.mid[p] = (mid == lo) ? 0u : mid;
+  for (uint32_t i = 0; i < per_plan; ++i) bs.at_lo[(size_t)p * per_plan + i] = 0;
+}
+
+// one thread per plan: pool the probe counts over trials, test feasibility, move the bracket
+__global__ void bisect_update_kernel(BisectState bs, uint32_t P, uint32_t K, uint32_t T,
+                                     const uint32_t* att_num, const uint32_t* att_den,
+                                     int32_t* status) {
+  const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  uint32_t lo = bs.lo[p], hi = bs.hi[p];
+  const uint32_t mid = bs.mid[p];
+  if (mid != 0) {
+    const uint32_t* pc = bs.probe + (size_t)p * K * T * 2;
+    bool feasible = true;
+    for (uint32_t k = 0; k < K; ++k) {  // DESIGN.md R18: an out-of-range probe (zeroed) is infeasible
+      uint64_t n = 0;
+      for (uint32_t t = 0; t < T; ++t) n += pc[(k * T + t) * 2];
+      if (n == 0) feasible = false;
+    }
+    for (uint32_t t = 0; t < T; ++t) {
+      uint64_t cnt = 0, hits = 0;
+      for (uint32_t k = 0; k < K; ++k) { cnt += pc[(k * T + t) * 2]; hits += pc[(k * T + t) * 2 + 1]; }
+      if (cnt > 0 && hits * (uint64_t)att_den[t] < (uint64_t)att_num[t] * cnt) feasible = false;
+    }
+    if (feasible) {
+      lo = mid;
+      uint32_t* al = bs.at_lo + (size_t)p * K * T * 2;
+      for (uint32_t i = 0; i < K * T * 2; ++i) al[i] = pc[i];
+    } else {
+      hi = mid;
+    }
+    bs.lo[p] = lo;
+    bs.hi[p] = hi;
+  }
+  const uint32_t nm = lo + (hi - lo) / 2;
+  bs.mid[p] = (nm == lo) ? 0u : nm;
+}
+
+__global__ void bisect_final_kernel(BisectState bs, uint32_t P, uint32_t K, uint32_t T, uint32_t N,
+                                    uint32_t* out_rate, uint32_t* out_goodput, uint32_t* out_counts) {
+  const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const uint32_t lo = bs.lo[p];
+  out_rate[p] = lo;
+  const uint32_t* al = bs.at_lo + (size_t)p * K * T * 2;
+  for (uint32_t t = 0; t < T; ++t) {
+    uint64_t hits = 0;
+    for (uint32_t k = 0; k < K; ++k) hits += al[(k * T + t) * 2 + 1];
+    out_goodput[p * T + t] = (uint32_t)(((uint64_t)lo * hits) / ((uint64_t)N * K));
+  }
+  if (out_counts)
+    for (uint32_t i = 0; i < K * T * 2; ++i) out_counts[(size_t)p * K * T * 2 + i] = al[i];
+}
+
+// ------------------------------------------------------------------------------------------------
+// stream materialisation (a10 producer): one warp per 32-request chunk, then a per-(variant,trial)
+// pass that turns chunk-relative cumulative gaps into absolute ones.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+materialize_chunks_kernel(const __grid_constant__ KParams prm, uint32_t variant_lo, uint4* out,
+                          uint64_t* chunk_totals, uint32_t chunks_per_sim) {
+  __shared__ uint32_t cnt_dummy[8];
+  const int lane = threadIdx.x & 31;
+  const uint32_t chunk = blockIdx.x * 4 + (threadIdx.x >> 5);
+  const uint32_t trial = blockIdx.y, vi = blockIdx.z;
+  if (chunk >= chunks_per_sim) return;
+  const size_t sim = (size_t)vi * prm.K + trial;
+  // records of one request are 2 x uint4; lanes beyond N write nothing
+  uint4 tmp_base[1];
+  (void)tmp_base;
+  uint4* dst = out + (sim * prm.N + (size_t)chunk * 32) * 2;
+  // produce into registers via a small shared staging area to reuse the producer
+  __shared__ __align__(16) uint4 stage[4][32 * 2];
+  produce_chunk_philox<6>(prm, chunk * 32, trial, variant_lo + vi, stage[threadIdx.x >> 5],
+                          chunk_totals + sim * chunks_per_sim + chunk, cnt_dummy, lane);
+  __syncwarp();
+  if (chunk * 32 + lane < prm.N) {
+    dst[lane * 2 + 0] = stage[threadIdx.x >> 5][lane * 2 + 0];
+    dst[lane * 2 + 1] = stage[threadIdx.x >> 5][lane * 2 + 1];
+  }
+}
+
+// one CTA per (variant, trial): exclusive scan of the chunk totals, then add to every record
+__global__ void __launch_bounds__(256)
+materialize_fixup_kernel(uint4* out, uint64_t* chunk_totals, uint32_t N, uint32_t chunks_per_sim) {
+  const size_t sim = blockIdx.x;
+  uint64_t* tot = chunk_totals + sim * chunks_per_sim;
+  __shared__ uint64_t carry;
+  __shared__ uint64_t warp_sum[8];
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // pass 1: in-place exclusive prefix of chunk totals (blocks of 256 chunks)
+  for (uint32_t base = 0; base < chunks_per_sim; base += 256) {
+    const uint32_t c = base + threadIdx.x;
+    const uint64_t v = c < chunks_per_sim ? tot[c] : 0;
+    const uint64_t inc = warp_inclusive_sum(v, lane);
+    if (lane == 31) warp_sum[warp] = inc;
+    __syncthreads();
+    uint64_t off = carry;
+    for (int w = 0; w < warp; ++w) off += warp_sum[w];
+    if (c < chunks_per_sim) tot[c] = off + inc - v;
+    __syncthreads();
+    if (threadIdx.x == 255) carry = off + inc;
+    __syncthreads();
+  }
+  // pass 2: add the chunk base to the cu field of every record head
+  uint4* rec = out + sim * (size_t)N * 2;
+  for (uint32_t n = threadIdx.x; n < N; n += 256) {
+    uint4 h = rec[(size_t)n * 2];
+    const uint64_t t = h.y >> 24;
+    uint64_t cu = (((uint64_t)(h.y & 0x00ffffffu)) << 32 | h.x) + tot[n >> 5];
+    h.x = (uint32_t)cu;
+    h.y = (uint32_t)(cu >> 32) | (uint32_t)(t << 24);
+    rec[(size_t)n * 2] = h;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// INT32 peak micro-benchmark (bench.py's ALU roofline denominator)
+// ------------------------------------------------------------------------------------------------
+template <int MIX>
+__global__ void __launch_bounds__(256) int32_peak_kernel(uint32_t iters, uint32_t* sink) {
+  uint32_t a[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = threadIdx.x * 2654435761u + i * 40503u + blockIdx.x;
+  const uint32_t k1 = 0x9E3779B9u + blockIdx.x, k2 = 0x85EBCA6Bu + threadIdx.x;
+  for (uint32_t it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        if (MIX == 0) {                       // ALU pipe: LOP3 / IADD3 alternating
+          a[i] = (u & 1) ? (a[i] ^ k1 ^ a[(i + 1) & 7]) : (a[i] + k2 + a[(i + 3) & 7]);
+        } else if (MIX == 1) {                // FMA pipe: IMAD
+          a[i] = a[i] * k1 + a[(i + 1) & 7];
+        } else {                              // alternate the two pipes
+          a[i] = (i & 1) ? (a[i] * k1 + k2) : (a[i] ^ k1 ^ a[(i + 2) & 7]);
+        }
+      }
+    }
+  }
+  uint32_t r = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) r ^= a[i];
+  if (r == 0x12345678u) sink[0] = r;  // keeps the loop alive
+}
+
+int32_t cuda_rc(cudaError_t e) {
+  if (e == cudaSuccess) return CF_OK;
+  std::fprintf(stderr, "libcf_b200: CUDA error: %s\n", cudaGetErrorString(e));
+  return CF_ERR_CUDA;
+}
+
+// shared implementation of cf_eval_plans / cf_eval_plans_stream / cf_trace_sim
+struct EvalArgs {
+  const cf_graph* g; const cf_plans* pl; const uint32_t* rates_dev; uint32_t R; const cf_slo* slo;
+  uint64_t seed; uint32_t variant; const void* stream_records; uint32_t n_variants;
+  const uint32_t* plan_variant; uint32_t* out_counts; uint64_t* out_dep_sum; int64_t* out_makespan;
+  void* ws; size_t ws_bytes; cudaStream_t st;
+};
+
+int32_t eval_impl(const EvalArgs& a) {
+  g_launch_count = 0;
+  if (int32_t rc = check_graph(a.g)) return rc;
+  if (int32_t rc = check_plans(a.g, a.pl)) return rc;
+  if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
+  if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
+  Schedule sc;
+  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, &sc))
+    return rc;
+  Blob blob;
+  blob.reserve(kAlign);  // status block
+  KParams kp;
+  const size_t pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &kp);
+  const SchedOffsets so = add_schedule(sc, &blob);
+  if (blob.bytes.size() > a.ws_bytes) return CF_ERR_WORKSPACE;
+  uint8_t* ws = static_cast<uint8_t*>(a.ws);
+  if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, a.st)))
+    return rc;
+  point_schedule(&kp, ws, so, pool_off);
+  kp.stream = static_cast<const uint4*>(a.stream_records);
+  kp.variant_lo = a.stream_records ? 0 : a.variant;
+  kp.rates = a.rates_dev;
+  kp.out_counts = a.out_counts;
+  kp.out_dep_sum = a.out_dep_sum;
+  kp.out_makespan = a.out_makespan;
+  return cuda_rc(launch_sims(kp, sc, a.g->n_trials, a.st));
+}
+
+struct BisectArgs {
+  const cf_graph* g; const cf_plans* pl; const uint32_t* rate_hi_dev; uint32_t n_steps; const cf_slo* slo;
+  uint64_t seed; uint32_t variant; const void* stream_records; uint32_t n_variants;
+  const uint32_t* plan_variant; uint32_t* out_rate; uint32_t* out_goodput; uint32_t* out_counts;
+  void* ws; size_t ws_bytes; cudaStream_t st;
+};
+
+int32_t bisect_impl(const BisectArgs& a) {
+  g_launch_count = 0;
+  if (int32_t rc = check_graph(a.g)) return rc;
+  if (int32_t rc = check_plans(a.g, a.pl)) return rc;
+  if (!a.rate_hi_dev || !a.slo || !a.slo->L_us || !a.slo->att_num || !a.slo->att_den || !a.out_rate || !a.out_goodput)
+    return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
+  if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
+  const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
+  Schedule sc;
+  if (int32_t rc = build_schedule(a.g, a.pl, 1, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, &sc))
+    return rc;
+  Blob blob;
+  blob.reserve(kAlign);
+  KParams kp;
+  const size_t pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &kp);
+  const SchedOffsets so = add_schedule(sc, &blob);
+  const size_t att_off = blob.add(a.slo->att_num, T * 4);
+  const size_t den_off = blob.add(a.slo->att_den, T * 4);
+  const size_t per_plan = (size_t)K * T * 2;
+  const size_t lo_off = blob.reserve((size_t)P * 4), hi_off = blob.reserve((size_t)P * 4),
+               mid_off = blob.reserve((size_t)P * 4);
+  const size_t blob_bytes = blob.bytes.size();
+  const size_t probe_off = align_up(blob_bytes), at_lo_off = align_up(probe_off + P * per_plan * 4);
+  if (at_lo_off + P * per_plan * 4 > a.ws_bytes) return CF_ERR_WORKSPACE;
+  uint8_t* ws = static_cast<uint8_t*>(a.ws);
+  if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob_bytes, cudaMemcpyHostToDevice, a.st)))
+    return rc;
+  point_schedule(&kp, ws, so, pool_off);
+  BisectState bs;
+  bs.lo = reinterpret_cast<uint32_t*>(ws + lo_off);
+  bs.hi = reinterpret_cast<uint32_t*>(ws + hi_off);
+  bs.mid = reinterpret_cast<uint32_t*>(ws + mid_off);
+  bs.probe = reinterpret_cast<uint32_t*>(ws + probe_off);
+  bs.at_lo = reinterpret_cast<uint32_t*>(ws + at_lo_off);
+  kp.stream = static_cast<const uint4*>(a.stream_records);
+  kp.variant_lo = a.stream_records ? 0 : a.variant;
+  kp.bisect_mode = 1;
+  kp.rates = bs.mid;
+  kp.out_counts = bs.probe;
+  const uint32_t nb = (P + 127) / 128;
+  bisect_init_kernel<<<nb, 128, 0, a.st>>>(bs, a.rate_hi_dev, P, (uint32_t)per_plan);
+  ++g_launch_count;
+  for (uint32_t step = 0; step < a.n_steps; ++step) {
+    if (int32_t rc = cuda_rc(launch_sims(kp, sc, K, a.st))) return rc;
+    bisect_update_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, reinterpret_cast<const uint32_t*>(ws + att_off),
+                                               reinterpret_cast<const uint32_t*>(ws + den_off), kp.status);
+    ++g_launch_count;
+  }
+  bisect_final_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, a.g->n_req, a.out_rate, a.out_goodput, a.out_counts);
+  ++g_launch_count;
+  return cuda_rc(cudaGetLastError());
+}
+
+}  // namespace
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+extern "C" {
+
+size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
+  if (!g || !pl || !g->tabs) return 0;
+  const size_t P = pl->n_plans, K = g->n_trials, T = g->n_types;
+  if (R < 1) R = 1;
+  size_t n = kAlign;                                        // status
+  n += align_up(pool_entries(g) * 4);
+  n += align_up(P * sizeof(TopoDesc));
+  n += align_up(P * R * sizeof(SimDesc));
+  const size_t max_warps = P * R / 32 + P + 1;
+  n += align_up(max_warps * sizeof(WarpDesc));
+  n += align_up(max_warps * sizeof(CtaDesc));
+  n += align_up(P * 8 * 2);
+  n += 2 * kAlign + 3 * align_up(P * 4);                    // bisection: att, lo/hi/mid
+  n += 2 * align_up(P * K * T * 2 * 4) + kAlign;            // probe + at_lo counts
+  n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch
+  const size_t chunks = ((size_t)g->n_req + 31) / 32;
+  (void)chunks;
+  return n + 4 * kAlign;
+}
+
+int32_t cf_eval_plans(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps, uint32_t R,
+                      const cf_slo* slo, uint64_t seed, uint32_t variant, uint32_t* out_counts,
+                      uint64_t* out_dep_sum, int64_t* out_makespan, void* workspace,
+                      size_t workspace_bytes, void* stream) {
+  EvalArgs a{g, pl, rate_mrps, R, slo, seed, variant, nullptr, 1, nullptr, out_counts, out_dep_sum,
+             out_makespan, workspace, workspace_bytes, static_cast<cudaStream_t>(stream)};
+  return eval_impl(a);
+}
+
+int32_t cf_eval_plans_stream(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps,
+                             uint32_t R, const cf_slo* slo, const void* stream_records,
+                             uint32_t n_variants, const uint32_t* plan_variant,
+                             uint32_t* out_counts, uint64_t* out_dep_sum, int64_t* out_makespan,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+  if (!stream_records) return CF_ERR_ARG;
+  EvalArgs a{g, pl, rate_mrps, R, slo, 0, 0, stream_records, n_variants, plan_variant, out_counts,
+             out_dep_sum, out_makespan, workspace, workspace_bytes, static_cast<cudaStream_t>(stream)};
+  return eval_impl(a);
+}
+
+int32_t cf_goodput_bisect(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_hi_mrps,
+                          uint32_t n_steps, const cf_slo* slo, uint64_t seed, uint32_t variant,
+                          uint32_t* out_rate_mrps, uint32_t* out_goodput_mrps, uint32_t* out_counts,
+                          void* workspace, size_t workspace_bytes, void* stream) {
+  BisectArgs a{g, pl, rate_hi_mrps, n_steps, slo, seed, variant, nullptr, 1, nullptr, out_rate_mrps,
+               out_goodput_mrps, out_counts, workspace, workspace_bytes, static_cast<cudaStream_t>(stream)};
+  return bisect_impl(a);
+}
+
+int32_t cf_goodput_bisect_stream(const cf_graph* g, const cf_plans* pl,
+                                 const uint32_t* rate_hi_mrps, uint32_t n_steps, const cf_slo* slo,
+                                 const void* stream_records, uint32_t n_variants,
+                                 const uint32_t* plan_variant, uint32_t* out_rate_mrps,
+                                 uint32_t* out_goodput_mrps, uint32_t* out_counts, void* workspace,
+                                 size_t workspace_bytes, void* stream) {
+  if (!stream_records) return CF_ERR_ARG;
+  BisectArgs a{g, pl, rate_hi_mrps, n_steps, slo, 0, 0, stream_records, n_variants, plan_variant,
+               out_rate_mrps, out_goodput_mrps, out_counts, workspace, workspace_bytes,
+               static_cast<cudaStream_t>(stream)};
+  return bisect_impl(a);
+}
+
+size_t cf_stream_bytes(const cf_graph* g, uint32_t n_variants) {
+  if (!g) return 0;
+  return (size_t)n_variants * g->n_trials * g->n_req * 32;
+}
+
+size_t cf_materialize_workspace_bytes(const cf_graph* g, uint32_t n_variants) {
+  if (!g || !g->tabs) return 0;
+  const size_t chunks = ((size_t)g->n_req + 31) / 32;
+  return 2 * kAlign + align_up(pool_entries(g) * 4) + align_up((size_t)n_variants * g->n_trials * chunks * 8);
+}
+
+int32_t cf_materialize_stream(const cf_graph* g, uint64_t seed, uint32_t variant_lo,
+                              uint32_t n_variants, void* out_stream, void* workspace,
+                              size_t workspace_bytes, void* stream) {
+  g_launch_count = 0;
+  if (int32_t rc = check_graph(g)) return rc;
+  if (g->n_comp > 6 || n_variants < 1 || n_variants > 65535 || !out_stream) return CF_ERR_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const uint32_t chunks = (g->n_req + 31) / 32;
+  Blob blob;
+  blob.reserve(kAlign);
+  KParams kp;
+  const size_t pool_off = fill_graph_params(g, nullptr, seed, &blob, &kp);
+  const size_t tot_off = align_up(blob.bytes.size());
+  const size_t need = tot_off + (size_t)n_variants * g->n_trials * chunks * 8;
+  if (int32_t rc = check_workspace(workspace, workspace_bytes, need)) return rc;
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st)))
+    return rc;
+  kp.qpool = reinterpret_cast<const int32_t*>(ws + pool_off);
+  kp.status = reinterpret_cast<int32_t*>(ws);
+  uint64_t* totals = reinterpret_cast<uint64_t*>(ws + tot_off);
+  materialize_chunks_kernel<<<dim3((chunks + 3) / 4, g->n_trials, n_variants), 128, 0, st>>>(
+      kp, variant_lo, static_cast<uint4*>(out_stream), totals, chunks);
+  ++g_launch_count;
+  materialize_fixup_kernel<<<n_variants * g->n_trials, 256, 0, st>>>(static_cast<uint4*>(out_stream), totals,
+                                                                      g->n_req, chunks);
+  ++g_launch_count;
+  return cuda_rc(cudaGetLastError());
+}
+
+int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint32_t rate_mrps,
+                     uint32_t trial, uint64_t seed, uint32_t variant, int64_t* out_arrival,
+                     int64_t* out_departure, uint8_t* out_type, void* workspace,
+                     size_t workspace_bytes, void* stream) {
+  g_launch_count = 0;
+  if (int32_t rc = check_graph(g)) return rc;
+  if (int32_t rc = check_plans(g, pl)) return rc;
+  if (plan >= pl->n_plans || trial >= g->n_trials) return CF_ERR_ARG;
+  if (int32_t rc = check_workspace(workspace, workspace_bytes, cf_workspace_bytes(g, pl, 1))) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  Schedule sc;
+  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, &sc)) return rc;
+  // the single simulation reads rate slot `plan` (pr = plan*1 + 0): upload a full-length rate array
+  Blob blob;
+  blob.reserve(kAlign);
+  KParams kp;
+  int64_t zeros[8] = {0};
+  cf_slo slo{zeros, nullptr, nullptr};
+  const size_t pool_off = fill_graph_params(g, &slo, seed, &blob, &kp);
+  const SchedOffsets so = add_schedule(sc, &blob);
+  std::vector<uint32_t> rates(pl->n_plans, rate_mrps);
+  const size_t rate_off = blob.add(rates.data(), rates.size() * 4);
+  const size_t scratch_off = blob.reserve((size_t)pl->n_plans * g->n_trials * g->n_types * 2 * 4);
+  if (blob.bytes.size() > workspace_bytes) return CF_ERR_WORKSPACE;
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st)))
+    return rc;
+  point_schedule(&kp, ws, so, pool_off);
+  kp.variant_lo = variant;
+  kp.rates = reinterpret_cast<const uint32_t*>(ws + rate_off);
+  kp.out_counts = reinterpret_cast<uint32_t*>(ws + scratch_off);
+  kp.tr_arrival = out_arrival;
+  kp.tr_departure = out_departure;
+  kp.tr_type = out_type;
+  kp.trial_base = trial;
+  return cuda_rc(launch_sims(kp, sc, 1, st));
+}
+
+int32_t cf_workspace_status(const void* workspace, void* stream) {
+  if (!workspace) return CF_ERR_WORKSPACE;
+  int32_t st = 0;
+  cudaError_t e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+  if (e == cudaSuccess) e = cudaMemcpy(&st, workspace, sizeof(st), cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) return cuda_rc(e);
+  return st;
+}
+
+uint32_t cf_last_launch_count(void) { return g_launch_count; }
+
+int32_t cf_bench_int32_peak(uint32_t mix, uint32_t iters, uint64_t* out_ops, uint64_t* out_usec,
+                            void* stream) {
+  if (!out_ops || !out_usec || mix > 2 || iters < 1) return CF_ERR_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return CF_ERR_CUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return CF_ERR_CUDA;
+  uint32_t* sink = nullptr;
+  if (cudaMalloc(&sink, 4) != cudaSuccess) return CF_ERR_CUDA;
+  const uint32_t blocks = (uint32_t)sms * 8, threads = 256;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  auto run = [&](uint32_t it) {
+    if (mix == 0) int32_peak_kernel<0><<<blocks, threads, 0, st>>>(it, sink);
+    else if (mix == 1) int32_peak_kernel<1><<<blocks, threads, 0, st>>>(it, sink);
+    else int32_peak_kernel<2><<<blocks, threads, 0, st>>>(it, sink);
+  };
+  run(iters / 8 + 1);  // warm-up
+  cudaEventRecord(e0, st);
+  run(iters);
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (e != cudaSuccess) return cuda_rc(e);
+  // 64 integer instructions per inner iteration per thread (8 x 8), one lane-op each
+  *out_ops = (uint64_t)blocks * threads * (uint64_t)iters * 64ull;
+  *out_usec = (uint64_t)(ms * 1000.0);
+  return CF_OK;
+}
+
+const char* cf_strerror(int32_t status) {
+  switch (status) {
+    case CF_OK: return "ok";
+    case CF_ERR_ARG: return "invalid argument";
+    case CF_ERR_RANGE: return "value out of the supported range";
+    case CF_ERR_PLAN: return "invalid plan";
+    case CF_ERR_TABLE: return "invalid quantile table";
+    case CF_ERR_CUDA: return "CUDA runtime error";
+    case CF_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"

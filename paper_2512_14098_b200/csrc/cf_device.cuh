@@ -1,0 +1,463 @@
+// cf_device.cuh -- device code of libcf_b200 (sm_100a). See DESIGN.md "Kernels".
+//
+// Mapping:
+//   * one THREAD per simulation (plan, rate, trial); a CTA holds simulations that share the trial
+//     and the Philox variant, hence (common random numbers, R4) the same request stream;
+//   * the CTA draws that stream ONCE per tile (a1 Philox4x32-10, a2 table lookup, a3 type + gap
+//     prefix sum) into shared memory -- or copies it from the materialised HBM stream (a10) -- and
+//     every thread then walks the tile sequentially;
+//   * each warp holds simulations of one plan topology; it turns 32 component-level records into
+//     stage-level records (a4) once per chunk, so the per-request loop sees only {cu, type, S[s]};
+//   * a5/a6: the free-time multiset of a c-replica stage is a binary min-heap of int64 per thread,
+//     root in a register, nodes 2..c+1 in shared memory interleaved by lane (bank = lane, no
+//     conflicts); c = 1 degenerates to the Lindley recursion with no memory traffic;
+//   * a7 hand-off is the running x; a8 counters are packed per-type byte fields flushed per chunk.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace cfk {
+
+constexpr int kWarpsPerCta = 4;
+constexpr int kThreads = kWarpsPerCta * 32;
+constexpr int kTile = 128;              // requests per CTA tile
+constexpr int kChunks = kTile / 32;     // 32-request chunks per tile
+constexpr int64_t kInf = INT64_MAX;
+
+struct DevTab {
+  uint32_t off;  // index of entry 0 in the int32 pool
+  uint32_t levels, log2_cells, pad;
+};
+
+struct TopoDesc {  // one plan topology = ordered stage masks
+  uint8_t n_stages;
+  uint8_t mask[8];
+  uint8_t pad[7];
+};
+
+struct SimDesc {
+  uint32_t plan;  // plan index (for replica counts)
+  uint32_t pr;    // p*R + r : index into the rate array; output slot is pr*K + k
+};
+
+struct WarpDesc {
+  uint32_t sim_begin, n_lanes, topo, pad;
+  uint32_t heap_off[8];  // byte offset of this warp's stage-s heap region in the CTA heap arena
+};
+
+struct CtaDesc {
+  uint32_t warp_begin, n_warps, variant, heap_bytes;
+};
+
+struct KParams {
+  uint32_t C, T, N, K;
+  uint32_t type_thresh[8];
+  uint8_t type_mask[8];
+  DevTab svc_tab[64];  // [i*8 + t]
+  DevTab arr_tab;
+  const int32_t* qpool;
+  int64_t L_us[8];
+  int64_t edge_delay;
+  uint32_t seed_lo, seed_hi;
+  // request source: in-register Philox (stream == nullptr, Philox variant = variant_lo + cta.variant)
+  // or materialised records [variant][K][N] x 32 B
+  const uint4* stream;
+  uint32_t variant_lo;
+  uint32_t bisect_mode;  // rate 0 means "skip this simulation" instead of a range error
+  uint32_t trial_base;   // trial = trial_base + blockIdx.y (cf_trace_sim runs one trial)
+  // schedule
+  const CtaDesc* ctas;
+  const WarpDesc* warps;
+  const SimDesc* sims;
+  const TopoDesc* topos;
+  const uint16_t* plan_c;  // [P*8]
+  const uint32_t* rates;   // [P*R]
+  // outputs
+  uint32_t* out_counts;    // [PR][K][T][2]
+  uint64_t* out_dep_sum;   // [PR][K] or null
+  int64_t* out_makespan;   // [PR][K] or null
+  int32_t* status;         // sticky device status
+  int64_t* tr_arrival;     // trace (single simulation) or null
+  int64_t* tr_departure;
+  uint8_t* tr_type;
+};
+
+// ------------------------------------------------------------------------------------------------
+// a1: Philox4x32-10 (Salmon et al. SC'11), counter (n, trial, block, variant), key = seed
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+    c0 = n0;
+    c2 = n2;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2: integer sample from a tail-refined quantile table (R3)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int32_t qtab_sample(const int32_t* __restrict__ pool, const DevTab tb,
+                                               uint32_t u) {
+  const uint32_t L1 = tb.levels - 1, B = tb.log2_cells;
+  const uint32_t k = min((uint32_t)__clz((int)~u), L1);  // leading ones, capped at the last level
+  const uint32_t drop = (k < L1) ? k + 1 : L1;           // <= 31 because levels <= 32
+  const uint32_t r = u << drop;
+  const uint32_t m = (r >> 1) >> (31 - B);               // top B bits (B may be 0)
+  const uint32_t f = (r >> (16 - B)) & 0xffffu;
+  const int32_t* q = pool + tb.off + (k << B) + m;
+  const int32_t q0 = __ldg(q), q1 = __ldg(q + 1);
+  return q0 + (int32_t)(((int64_t)(q1 - q0) * (int64_t)f) >> 16);
+}
+
+__device__ __forceinline__ uint64_t warp_inclusive_sum(uint64_t v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint64_t o = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += o;
+  }
+  return v;
+}
+
+// Component-level record of one request in shared memory (and, for C <= 6, in the HBM stream):
+//   w0.x,w0.y = cu (56 bit) | type << 56 ; w0.z,w0.w,w1.* = svc[0..5] ; (C > 6: w2.x,w2.y = svc[6..7])
+// In-register mode cu is relative to the start of the 32-request chunk; the consumer adds the base.
+template <int CMAX>
+struct CompRec {
+  static constexpr int kWords = (CMAX <= 6) ? 2 : 3;  // uint4 words
+};
+
+// Stage-level record a warp builds for its topology: cu (absolute) | type<<56, then S[s] per stage
+// (-1 = stage not visited by this request's type).
+template <int VMAX>
+struct StageRec {
+  static constexpr int kWords = (VMAX <= 2) ? 1 : (VMAX <= 6 ? 2 : 3);
+};
+
+// ------------------------------------------------------------------------------------------------
+// Producer: chunk `chunk` (32 requests starting at n0) of the tile, one request per lane.
+// ------------------------------------------------------------------------------------------------
+template <int CMAX>
+__device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_t n0, uint32_t trial,
+                                                     uint32_t variant, uint4* tile_chunk,
+                                                     uint64_t* chunk_total, uint32_t* cnt_s,
+                                                     int lane) {
+  const uint32_t n = n0 + lane;
+  const bool valid = n < prm.N;
+  uint32_t gap = 0, t = 0;
+  int32_t svc[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) svc[i] = 0;
+  if (valid) {
+    const uint4 b0 = philox4x32_10(n, trial, 0, variant, prm.seed_lo, prm.seed_hi);
+    gap = (uint32_t)qtab_sample(prm.qpool, prm.arr_tab, b0.x);
+    t = prm.T - 1;
+    for (int tt = (int)prm.T - 2; tt >= 0; --tt)
+      if (b0.y < prm.type_thresh[tt]) t = tt;  // first tt with u < thresh[tt]
+    const uint32_t tm = prm.type_mask[t];
+    if (tm & 0x0fu) {
+      const uint4 b1 = philox4x32_10(n, trial, 1, variant, prm.seed_lo, prm.seed_hi);
+      if (tm & 1u) svc[0] = qtab_sample(prm.qpool, prm.svc_tab[0 * 8 + t], b1.x);
+      if (tm & 2u) svc[1] = qtab_sample(prm.qpool, prm.svc_tab[1 * 8 + t], b1.y);
+      if (tm & 4u) svc[2] = qtab_sample(prm.qpool, prm.svc_tab[2 * 8 + t], b1.z);
+      if (tm & 8u) svc[3] = qtab_sample(prm.qpool, prm.svc_tab[3 * 8 + t], b1.w);
+    }
+    if (tm & 0xf0u) {
+      const uint4 b2 = philox4x32_10(n, trial, 2, variant, prm.seed_lo, prm.seed_hi);
+      if (tm & 16u) svc[4] = qtab_sample(prm.qpool, prm.svc_tab[4 * 8 + t], b2.x);
+      if (tm & 32u) svc[5] = qtab_sample(prm.qpool, prm.svc_tab[5 * 8 + t], b2.y);
+      if (CMAX > 6) {
+        if (tm & 64u) svc[6] = qtab_sample(prm.qpool, prm.svc_tab[6 * 8 + t], b2.z);
+        if (tm & 128u) svc[7] = qtab_sample(prm.qpool, prm.svc_tab[7 * 8 + t], b2.w);
+      }
+    }
+    atomicAdd(&cnt_s[t], 1u);
+  }
+  const uint64_t cu = warp_inclusive_sum((uint64_t)gap, lane);  // relative to the chunk start
+  if (lane == 31) *chunk_total = cu;
+  uint4* dst = tile_chunk + lane * CompRec<CMAX>::kWords;
+  dst[0] = make_uint4((uint32_t)cu, (uint32_t)(cu >> 32) | (t << 24), (uint32_t)svc[0], (uint32_t)svc[1]);
+  dst[1] = make_uint4((uint32_t)svc[2], (uint32_t)svc[3], (uint32_t)svc[4], (uint32_t)svc[5]);
+  if (CMAX > 6) dst[2] = make_uint4((uint32_t)svc[6], (uint32_t)svc[7], 0u, 0u);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Min-heap replace-min (a6). root = current minimum (register); nodes 2..c live in shared memory at
+// heap + (j-2)*256 (256 B = 32 lanes x 8 B per node row), node c+1 holds +inf.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int64_t lds64(const uint8_t* smem, uint32_t off) {
+  return *reinterpret_cast<const int64_t*>(smem + off);
+}
+__device__ __forceinline__ void sts64(uint8_t* smem, uint32_t off, int64_t v) {
+  *reinterpret_cast<int64_t*>(smem + off) = v;
+}
+
+__device__ __forceinline__ void heap_replace_min(uint8_t* smem, int64_t& root, uint32_t hb,
+                                                 uint32_t c, int64_t x) {
+  if (c < 2) {
+    root = x;
+    return;
+  }
+  int64_t a = lds64(smem, hb), b = lds64(smem, hb + 256);
+  bool bl = b < a;
+  int64_t m = bl ? b : a;
+  if (x <= m) {
+    root = x;
+    return;
+  }
+  root = m;
+  uint32_t i = 2u + (bl ? 1u : 0u);  // the hole
+  while (true) {
+    const uint32_t child = 2u * i;
+    if (child > c) break;
+    const uint32_t pa = hb + (child - 2u) * 256u;
+    a = lds64(smem, pa);
+    b = lds64(smem, pa + 256u);
+    bl = b < a;
+    m = bl ? b : a;
+    if (x <= m) break;
+    sts64(smem, hb + (i - 2u) * 256u, m);
+    i = child + (bl ? 1u : 0u);
+  }
+  sts64(smem, hb + (i - 2u) * 256u, x);
+}
+
+// ------------------------------------------------------------------------------------------------
+// The simulation kernel. grid = (CTAs of this launch, K trials); block = kThreads.
+// Dynamic shared memory: [tiles 2 x kTile x CompRec][chunk totals][cnt][L][warp stage buffers][heaps]
+// ------------------------------------------------------------------------------------------------
+template <int VMAX, int CMAX>
+struct SmemLayout {
+  static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
+  static constexpr uint32_t kStageRecBytes = StageRec<VMAX>::kWords * 16;
+  static constexpr uint32_t tiles = 0;
+  static constexpr uint32_t totals = tiles + 2 * kTile * kCompRecBytes;
+  static constexpr uint32_t cnt = totals + 2 * kChunks * 8;
+  static constexpr uint32_t lus = cnt + 8 * 4;
+  static constexpr uint32_t wbuf = lus + 8 * 8;
+  static constexpr uint32_t heaps = wbuf + kWarpsPerCta * 32 * kStageRecBytes;
+  static constexpr uint32_t fixed_bytes = heaps;
+};
+
+template <int VMAX, int CMAX, bool HAS_DELAY>
+__global__ void __launch_bounds__(kThreads)
+cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
+  using SL = SmemLayout<VMAX, CMAX>;
+  extern __shared__ __align__(16) uint8_t smem[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t trial = prm.trial_base + blockIdx.y;
+  const CtaDesc cta = prm.ctas[cta_base + blockIdx.x];
+  const uint32_t variant = prm.variant_lo + cta.variant;
+
+  uint4* tiles = reinterpret_cast<uint4*>(smem + SL::tiles);
+  uint64_t* totals = reinterpret_cast<uint64_t*>(smem + SL::totals);
+  uint32_t* cnt_s = reinterpret_cast<uint32_t*>(smem + SL::cnt);
+  int64_t* L_s = reinterpret_cast<int64_t*>(smem + SL::lus);
+  uint4* wbuf = reinterpret_cast<uint4*>(smem + SL::wbuf) + warp * 32 * StageRec<VMAX>::kWords;
+
+  if (tid < 8) {
+    cnt_s[tid] = 0;
+    L_s[tid] = prm.L_us[tid];
+  }
+
+  // ---- per-lane simulation state -------------------------------------------------------------
+  const bool warp_active = warp < (int)cta.n_warps;
+  WarpDesc wd;
+  TopoDesc topo;
+  uint32_t period = 1, pr = 0, sim_c[VMAX], hb[VMAX];
+  bool lane_live = false, rate_bad = false, skip = false;
+  int64_t root[VMAX];
+#pragma unroll
+  for (int s = 0; s < VMAX; ++s) { root[s] = 0; sim_c[s] = 1; hb[s] = 0; }
+  if (warp_active) {
+    wd = prm.warps[cta.warp_begin + warp];
+    topo = prm.topos[wd.topo];
+    lane_live = lane < (int)wd.n_lanes;
+    const SimDesc sd = prm.sims[wd.sim_begin + (lane_live ? lane : 0)];  // idle lanes mirror lane 0
+    pr = sd.pr;
+    const uint32_t rate = prm.rates[pr];
+    if (rate < 1u || rate > 1000000000u) {
+      if (prm.bisect_mode && rate == 0u) skip = true; else rate_bad = true;
+    } else {
+      period = (1000000000u + rate / 2u) / rate;
+    }
+#pragma unroll
+    for (int s = 0; s < VMAX; ++s) {
+      if (s < topo.n_stages) {
+        sim_c[s] = prm.plan_c[sd.plan * 8 + s];
+        hb[s] = SL::heaps + wd.heap_off[s] + lane * 8;
+        for (uint32_t j = 2; j <= sim_c[s]; ++j) sts64(smem, hb[s] + (j - 2u) * 256u, 0);
+        if (sim_c[s] >= 2) sts64(smem, hb[s] + (sim_c[s] - 1u) * 256u, kInf);  // node c+1
+      }
+    }
+  }
+  uint32_t hits[8];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) hits[t] = 0;
+  uint64_t dep_sum = 0, cu_base = 0, last_cu = 0;
+  int64_t makespan = 0;
+  const int64_t delay = prm.edge_delay;
+  const bool tracing = prm.tr_arrival != nullptr || prm.tr_departure != nullptr || prm.tr_type != nullptr;
+
+  // ---- producer for one tile -----------------------------------------------------------------
+  const uint32_t n_tiles = (prm.N + kTile - 1) / kTile;
+  auto produce = [&](uint32_t tile_idx) {
+    const uint32_t buf = tile_idx & 1u;
+    uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
+    const uint32_t n0 = tile_idx * kTile;
+    if (prm.stream == nullptr) {
+      for (int ch = warp; ch < kChunks; ch += kWarpsPerCta)
+        produce_chunk_philox<CMAX>(prm, n0 + ch * 32, trial, variant,
+                                   tb + ch * 32 * CompRec<CMAX>::kWords, totals + buf * kChunks + ch,
+                                   cnt_s, lane);
+    } else {
+      // a10: copy kTile 32-byte records (2 x uint4 each) from the materialised stream; cu is absolute
+      const uint4* src = prm.stream + ((size_t)(cta.variant * prm.K + trial) * prm.N + n0) * 2;
+      const uint32_t n_words = min((uint32_t)kTile, prm.N - n0) * 2u;
+      for (uint32_t w = tid; w < n_words; w += kThreads) {
+        const uint4 v = __ldg(src + w);
+        tb[w] = v;
+        if ((w & 1u) == 0u) atomicAdd(&cnt_s[v.y >> 24], 1u);
+      }
+      if (tid < kChunks) totals[buf * kChunks + tid] = 0;
+    }
+  };
+
+  __syncthreads();
+  produce(0);
+  __syncthreads();
+
+  for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
+    if (tile_idx + 1 < n_tiles) produce(tile_idx + 1);
+    if (warp_active) {
+      const uint32_t buf = tile_idx & 1u;
+      const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
+      const uint32_t n0 = tile_idx * kTile;
+#pragma unroll 1
+      for (int ch = 0; ch < kChunks; ++ch) {
+        const uint32_t nc0 = n0 + ch * 32;
+        if (nc0 >= prm.N) break;
+        // ---- a4: component-level -> stage-level records for this warp's topology -------------
+        {
+          const uint4* src = tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
+          const uint4 w0 = src[0], w1 = src[1];
+          int32_t svc[8];
+          svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x;
+          svc[3] = (int32_t)w1.y; svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w;
+          svc[6] = 0; svc[7] = 0;
+          if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
+          const uint32_t t = w0.y >> 24;
+          const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;
+          const uint32_t tm = prm.type_mask[t];
+          int32_t S[VMAX];
+#pragma unroll
+          for (int s = 0; s < VMAX; ++s) {
+            const uint32_t sm = (s < topo.n_stages) ? topo.mask[s] : 0u;
+            int32_t acc = 0;
+#pragma unroll
+            for (int i = 0; i < CMAX; ++i) acc += ((sm >> i) & 1u) ? svc[i] : 0;
+            S[s] = (sm & tm) ? acc : -1;
+          }
+          uint4* dst = wbuf + lane * StageRec<VMAX>::kWords;
+          const uint32_t hi = (uint32_t)(cu >> 32) | (t << 24);
+          if (VMAX <= 2) {
+            dst[0] = make_uint4((uint32_t)cu, hi, (uint32_t)S[0], (uint32_t)S[VMAX > 1 ? 1 : 0]);
+          } else {
+            dst[0] = make_uint4((uint32_t)cu, hi, (uint32_t)S[0], (uint32_t)S[1]);
+            dst[1] = make_uint4((uint32_t)S[2], (uint32_t)S[VMAX > 3 ? 3 : 0], (uint32_t)S[VMAX > 4 ? 4 : 0],
+                                (uint32_t)S[VMAX > 5 ? 5 : 0]);
+            if (VMAX > 6) dst[2] = make_uint4((uint32_t)S[VMAX > 6 ? 6 : 0], (uint32_t)S[VMAX > 7 ? 7 : 0], 0u, 0u);
+          }
+        }
+        __syncwarp();
+        // ---- the per-request loop: every lane runs its own simulation over the same 32 requests
+        const int n_here = (int)min(32u, prm.N - nc0);
+        uint64_t hp = 0;  // per-type hit counters of this chunk, one byte each
+#pragma unroll 1
+        for (int r = 0; r < n_here; ++r) {
+          const uint4* rp = wbuf + r * StageRec<VMAX>::kWords;
+          const uint4 w0 = rp[0];
+          int32_t S[VMAX];
+          S[0] = (int32_t)w0.z;
+          if (VMAX > 1) S[1] = (int32_t)w0.w;
+          if (VMAX > 2) {
+            const uint4 w1 = rp[1];
+            S[2] = (int32_t)w1.x;
+            if (VMAX > 3) S[3] = (int32_t)w1.y;
+            if (VMAX > 4) S[4] = (int32_t)w1.z;
+            if (VMAX > 5) S[5] = (int32_t)w1.w;
+          }
+          if (VMAX > 6) {
+            const uint4 w2 = rp[2];
+            S[6] = (int32_t)w2.x;
+            if (VMAX > 7) S[7] = (int32_t)w2.y;
+          }
+          const uint32_t t = w0.y >> 24;
+          const uint64_t cu = ((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x;
+          // a3: A = (CU * period + 2^15) >> 16
+          const int64_t A = (int64_t)((cu * (uint64_t)period + 32768ull) >> 16);
+          int64_t x = A;
+          bool first = true;
+#pragma unroll
+          for (int s = 0; s < VMAX; ++s) {
+            if (S[s] >= 0) {
+              if (HAS_DELAY) { if (!first) x += delay; first = false; }
+              const int64_t f = root[s];
+              x = (x > f ? x : f) + (int64_t)S[s];  // a5/a6: start at max(arrival, earliest free)
+              heap_replace_min(smem, root[s], hb[s], sim_c[s], x);
+            }
+          }
+          // a8
+          const bool hit = (x - A) <= L_s[t];
+          hp += (uint64_t)(hit ? 1u : 0u) << (t * 8u);
+          dep_sum += (uint64_t)x;
+          makespan = x > makespan ? x : makespan;
+          last_cu = cu;
+          if (tracing && warp == 0 && lane == 0) {
+            const uint32_t n = nc0 + r;
+            if (prm.tr_arrival) prm.tr_arrival[n] = A;
+            if (prm.tr_departure) prm.tr_departure[n] = x;
+            if (prm.tr_type) prm.tr_type[n] = (uint8_t)t;
+          }
+        }
+#pragma unroll
+        for (int t = 0; t < 8; ++t) hits[t] += (uint32_t)(hp >> (8 * t)) & 0xffu;
+        __syncwarp();
+        cu_base += totals[buf * kChunks + ch];
+      }
+    }
+    __syncthreads();
+  }
+
+  // ---- outputs ---------------------------------------------------------------------------------
+  if (warp_active && lane_live) {
+    // DESIGN.md R17: the arrival horizon CU_N * period + 2^15 must stay below 2^62
+    bool bad = rate_bad;
+    if (!bad && !skip) {
+      const uint64_t hi = __umul64hi(last_cu, (uint64_t)period);
+      const uint64_t lo = last_cu * (uint64_t)period;
+      if (hi != 0 || lo >= (1ull << 62) - 32768ull) bad = true;
+    }
+    if (bad) atomicMin(prm.status, -2);
+    const bool zero = bad || skip;
+    const size_t slot = (size_t)pr * prm.K + trial;
+    uint32_t* oc = prm.out_counts + slot * prm.T * 2;
+    for (uint32_t t = 0; t < prm.T; ++t) {
+      oc[2 * t + 0] = zero ? 0u : cnt_s[t];
+      oc[2 * t + 1] = zero ? 0u : hits[t];
+    }
+    if (prm.out_dep_sum) prm.out_dep_sum[slot] = zero ? 0ull : dep_sum;
+    if (prm.out_makespan) prm.out_makespan[slot] = zero ? 0ll : makespan;
+  }
+}
+
+}  // namespace cfk

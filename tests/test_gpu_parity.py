@@ -1,0 +1,262 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit.
+
+All arithmetic is integer, so the bar is exact equality of SLO-hit counts, departure checksums,
+makespans, traced departures, stream records, bisected rates and goodput (north_star)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2512_14098_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+NT = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def cf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2512_14098_b200 import binding
+    return binding
+
+
+def check_eval(cf, orc, w, graph=None, plans=None, rates=None, variant=0, **kw):
+    g = graph or w.graph
+    pl = plans or w.plans
+    rates = w.rate_mrps if rates is None else rates
+    got = cf.cf_eval_plans(g, pl, rates, w.slo, w.seed, variant, **kw)
+    status = cf.cf_workspace_status(got["workspace"])
+    want = orc.eval_plans(g, pl, rates, w.slo, w.seed, variant, n_threads=NT)
+    assert status == want["rc"]
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+    np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+    return got, want
+
+
+# ---------------------------------------------------------------------------------------------
+# the five configs at reduced sizes (several tiles + ragged tail), every sim compared
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mean_us", W.CONFIG0_SERVICE_MEANS_US)
+def test_cfg0_mm1_full_size(cf, orc, mean_us):
+    w = W.config0_mm1(mean_us)  # full BASELINE size: 10,000 requests x 4 trials x 8 rates
+    check_eval(cf, orc, w)
+    b = cf.cf_goodput_bisect(w.graph, w.plans, w.rate_hi_mrps, w.n_steps, w.slo, w.seed)
+    bo = orc.goodput_bisect(w.graph, w.plans, w.rate_hi_mrps, w.n_steps, w.slo, w.seed, n_threads=NT)
+    np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+    np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"]), bo["goodput_mrps"])
+    np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
+
+
+def test_cfg1_reduced(cf, orc):
+    w = W.config1_mllm(n_req=3000, n_trials=2, n_rates=4)  # all 512 plans, c up to 39
+    check_eval(cf, orc, w)
+
+
+def test_cfg2_reduced(cf, orc):
+    w = W.config2_omni(n_req=2100, n_trials=2, n_rates=3, vectors_per_pattern=4)  # 32 topologies
+    check_eval(cf, orc, w)
+
+
+def test_cfg3_reduced(cf, orc):
+    w = W.config3_multireplica(n_req=1500, n_trials=2, n_rates=3, plans_per_topology=40)
+    check_eval(cf, orc, w)
+
+
+def test_cfg4_reduced_stream_and_bisect(cf, orc):
+    w = W.config4_sweep(n_req=1300, n_trials=2, n_steps=10, vectors_per_pattern=4, n_variants=3)
+    g, pl = w.graph, w.plans
+    w.plan_variant = ((np.arange(pl.n_plans) // 5) % 3).astype(np.uint32)
+    # materialised records == oracle records
+    rec = cf.cf_materialize_stream(g, w.seed, 0, w.n_variants)
+    want = orc.materialize_stream(g, w.seed, 0, w.n_variants)
+    np.testing.assert_array_equal(rec.cpu().numpy().reshape(-1), want.view(np.uint8).reshape(-1))
+    # stream evaluation == in-register evaluation == oracle, variant by variant
+    rates = W.rate_grid(W.flow_bound_mrps(g, pl), [0.6, 0.9])
+    got = cf.cf_eval_plans(g, pl, rates, w.slo, w.seed, stream_records=rec, n_variants=w.n_variants,
+                           plan_variant=w.plan_variant)
+    for v in range(w.n_variants):
+        idx = np.nonzero(w.plan_variant == v)[0]
+        o = orc.eval_plans(g, pl.subset(idx), rates[idx], w.slo, w.seed, v, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"])[idx], o["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"])[idx], o["dep_sum"])
+        reg = cf.cf_eval_plans(g, pl.subset(idx), rates[idx], w.slo, w.seed, v)
+        np.testing.assert_array_equal(cf.to_numpy_u32(reg["counts"]), o["counts"])
+    # default mapping p % n_variants
+    got = cf.cf_eval_plans(g, pl, rates, w.slo, w.seed, stream_records=rec, n_variants=w.n_variants)
+    for v in range(w.n_variants):
+        idx = np.nonzero(np.arange(pl.n_plans) % w.n_variants == v)[0]
+        o = orc.eval_plans(g, pl.subset(idx), rates[idx], w.slo, w.seed, v, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"])[idx], o["counts"])
+    # device-side bisection on the stream
+    b = cf.cf_goodput_bisect(g, pl, w.rate_hi_mrps, w.n_steps, w.slo, w.seed, stream_records=rec,
+                             n_variants=w.n_variants, plan_variant=w.plan_variant)
+    for v in range(w.n_variants):
+        idx = np.nonzero(w.plan_variant == v)[0]
+        bo = orc.goodput_bisect(g, pl.subset(idx), w.rate_hi_mrps[idx], w.n_steps, w.slo, w.seed, v,
+                                n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"])[idx], bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"])[idx], bo["goodput_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"])[idx], bo["counts"])
+    assert (cf.to_numpy_u32(b["rate_mrps"]) > 0).any()
+
+
+# ---------------------------------------------------------------------------------------------
+# traces, edge cases
+# ---------------------------------------------------------------------------------------------
+def test_trace_matches_oracle(cf, orc):
+    w = W.config2_omni(n_req=777, n_trials=3, n_rates=2, vectors_per_pattern=2, n_patterns=8)
+    w.graph.edge_delay_us = 10_000
+    for p in (0, 3, 7, 15):
+        for k in (0, 2):
+            rate = int(w.rate_mrps[p, 1])
+            t = cf.cf_trace_sim(w.graph, w.plans, p, rate, k, w.seed, variant=5)
+            o = orc.trace_sim(w.graph, w.plans, p, rate, k, w.seed, variant=5)
+            np.testing.assert_array_equal(t["arrival"].cpu().numpy(), o["arrival"])
+            np.testing.assert_array_equal(t["departure"].cpu().numpy(), o["departure"])
+            np.testing.assert_array_equal(t["type"].cpu().numpy(), o["type"])
+
+
+def test_edge_delay_and_variant(cf, orc):
+    w = W.config2_omni(n_req=900, n_trials=2, n_rates=2, vectors_per_pattern=2, n_patterns=32)
+    w.graph.edge_delay_us = 10_000
+    check_eval(cf, orc, w, variant=9)
+    w1 = W.config1_mllm(n_req=700, n_trials=2, n_rates=2, llm_max=6, e_steps=3)
+    w1.graph.edge_delay_us = 123
+    check_eval(cf, orc, w1, variant=1)
+
+
+@pytest.mark.parametrize("n_req", [1, 31, 32, 33, 127, 128, 129, 257])
+def test_ragged_request_counts(cf, orc, n_req):
+    w = W.config1_mllm(n_req=n_req, n_trials=3, n_rates=2, llm_max=5, e_steps=2)
+    check_eval(cf, orc, w)
+
+
+def test_eight_components_eight_stages(cf, orc):
+    # C = 8, T = 8, plans with up to 8 stages: the wide-record template
+    rng = np.random.default_rng(5)
+    C = T = 8
+    tabs = [W.lognormal_qtab(float(rng.integers(5_000, 60_000)), 0.5) for _ in range(C)]
+    masks = [int(m) | 1 << int(rng.integers(0, C)) for m in rng.integers(0, 256, T)]
+    masks[3] = 0  # a type with an empty route (R14)
+    frac = rng.dirichlet(np.ones(T))
+    svc_tab = np.repeat(np.arange(C, dtype=np.uint16), T)
+    edges = [[i, i + 1] for i in range(C - 1)]
+    g = W.Graph(C, T, 1000, 2, masks, W.mix_thresholds(frac), svc_tab, tabs,
+                W.gamma_qtab(0.5, 65536.0), edges, edge_delay_us=250)
+    plan_list = []
+    for _ in range(40):
+        cuts = sorted(rng.choice(np.arange(1, C), size=int(rng.integers(0, C)), replace=False).tolist())
+        bounds = [0] + cuts + [C]
+        plan_list.append([(sum(1 << i for i in range(a, b)), int(rng.integers(1, 9)))
+                          for a, b in zip(bounds, bounds[1:])])
+    pl = W.make_plans(plan_list, max_stages=8)
+    rates = W.rate_grid(W.flow_bound_mrps(g, pl), [0.5, 0.9, 1.3])
+    slo = W.Slo(rng.integers(50_000, 400_000, T), [9] * T, [10] * T)
+    w = W.Workload("c8", g, pl, slo, seed=99, rate_mrps=rates)
+    assert orc.validate(g, pl) == 0
+    got, want = check_eval(cf, orc, w)
+    assert want["counts"][..., 3, 0].sum() > 0
+    np.testing.assert_array_equal(want["counts"][..., 3, 0], want["counts"][..., 3, 1])
+
+
+def test_large_replica_counts(cf, orc):
+    # c far above N (never queues) and c = 59, 64, 200 (deep heaps)
+    tab = W.lognormal_qtab(50_000.0, 0.6)
+    g = W.Graph(1, 1, 600, 2, [1], W.mix_thresholds([1.0]), [0], [tab], W.exponential_qtab(65536.0),
+                np.zeros((0, 2)))
+    pl = W.make_plans([[(1, c)] for c in (1, 2, 3, 59, 64, 200, 700)])
+    rates = W.rate_grid(W.flow_bound_mrps(g, pl), [0.7, 1.5])
+    w = W.Workload("bigc", g, pl, W.Slo([80_000], [9], [10]), seed=6, rate_mrps=rates)
+    check_eval(cf, orc, w)
+
+
+def test_out_of_range_rates_zeroed_and_flagged(cf, orc):
+    w = W.config1_mllm(n_req=200, n_trials=2, n_rates=3, llm_max=4, e_steps=2)
+    rates = w.rate_mrps.copy()
+    rates[1, 2] = 0
+    rates[2, 0] = 1_000_000_001
+    got, want = check_eval(cf, orc, w, rates=rates)
+    assert want["rc"] == orc.ORC_ERR_RANGE
+    assert (cf.to_numpy_u32(got["counts"])[1, 2] == 0).all()
+    # arrival horizon beyond 2^62 us (R17)
+    g = W.Graph(1, 1, 1 << 12, 1, [1], W.mix_thresholds([1.0]), [0], [W.constant_qtab(5)],
+                W.constant_qtab(2**31 - 1), np.zeros((0, 2)))
+    pl = W.make_plans([[(1, 1)]])
+    w2 = W.Workload("horizon", g, pl, W.Slo([10], [9], [10]), seed=0,
+                    rate_mrps=np.array([[1, 1000, 1_000_000_000]], dtype=np.uint32))
+    got, want = check_eval(cf, orc, w2)
+    assert want["sim_status"].reshape(-1).tolist() == [orc.ORC_ERR_RANGE, orc.ORC_ERR_RANGE, 0]
+
+
+def test_bisect_parity_and_degenerate_brackets(cf, orc):
+    w = W.config1_mllm(n_req=1500, n_trials=3, n_rates=2, llm_max=8, e_steps=3)
+    R_p = W.flow_bound_mrps(w.graph, w.plans)
+    hi = np.ceil(1.5 * R_p).astype(np.uint32)
+    hi[0], hi[1], hi[2] = 0, 1, 2
+    for steps in (1, 5, 20):
+        b = cf.cf_goodput_bisect(w.graph, w.plans, hi, steps, w.slo, w.seed)
+        assert cf.cf_workspace_status(b["workspace"]) == 0
+        bo = orc.goodput_bisect(w.graph, w.plans, hi, steps, w.slo, w.seed, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"]), bo["goodput_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
+
+
+def test_host_errors_on_gpu(cf):
+    w = W.config1_mllm(n_req=100, n_trials=1, n_rates=1, llm_max=2, e_steps=1)
+    bad = W.make_plans([[(0b10, 1), (0b01, 1)]])
+    r = cf.cf_eval_plans(w.graph, bad, [[1000]], w.slo, 0, check=False)
+    assert r["rc"] == cf.CF_ERR_PLAN
+    with pytest.raises(cf.CfError):
+        cf.cf_eval_plans(w.graph, bad, [[1000]], w.slo, 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# full BASELINE sizes in the bench's launch configuration: sampled simulations vs the oracle
+# ---------------------------------------------------------------------------------------------
+def sampled_full_size(cf, orc, w, n_samples, seed):
+    got = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed)
+    assert cf.cf_workspace_status(got["workspace"]) == 0
+    counts = cf.to_numpy_u32(got["counts"])
+    dep = cf.to_numpy_u64(got["dep_sum"])
+    mk = got["makespan"].cpu().numpy()
+    rng = np.random.default_rng(seed)
+    P, R = w.rate_mrps.shape
+    ps = rng.integers(0, P, n_samples)
+    rs = rng.integers(0, R, n_samples)
+    o = orc.eval_plans(w.graph, w.plans.subset(ps), w.rate_mrps[ps, rs].reshape(-1, 1), w.slo, w.seed,
+                       n_threads=NT)
+    np.testing.assert_array_equal(counts[ps, rs], o["counts"][:, 0])
+    np.testing.assert_array_equal(dep[ps, rs], o["dep_sum"][:, 0])
+    np.testing.assert_array_equal(mk[ps, rs], o["makespan"][:, 0])
+    # properties that hold at any size
+    c = counts.astype(np.int64)
+    assert (c[..., 0].sum(-1) == w.graph.n_req).all()
+    assert (c[..., 1] <= c[..., 0]).all()
+    assert (c[..., 0] == c[0, 0][None, None, ..., 0]).all()  # CRN: type counts independent of plan
+    return counts
+
+
+def test_cfg1_full_size_sampled(cf, orc):
+    w = W.config1_mllm()
+    counts = sampled_full_size(cf, orc, w, 12, 1)
+    # R16: colocated plans with equal l+e are duplicates and must agree exactly (same rates)
+    pl = w.plans
+    seen = {}
+    for p in range(256):
+        key = (int(pl.stage_c[p, 0]), tuple(w.rate_mrps[p]))
+        if key in seen:
+            np.testing.assert_array_equal(counts[p], counts[seen[key]])
+        seen[key] = p
+
+
+def test_cfg2_full_size_sampled(cf, orc):
+    sampled_full_size(cf, orc, W.config2_omni(), 6, 2)
+
+
+def test_cfg3_full_size_sampled(cf, orc):
+    sampled_full_size(cf, orc, W.config3_multireplica(), 8, 3)

@@ -106,25 +106,17 @@ int32_t check_plans(const cf_graph* g, const cf_plans* pl) {
 // ------------------------------------------------------------------------------------------------
 // schedule
 // ------------------------------------------------------------------------------------------------
-struct Launch {
-  uint32_t cta_begin, n_ctas, smem_bytes;
-};
-
 struct Schedule {
   std::vector<TopoDesc> topos;
   std::vector<SimDesc> sims;
   std::vector<WarpDesc> warps;
   std::vector<CtaDesc> ctas;
-  std::vector<Launch> launches;
   std::vector<uint16_t> plan_c;  // [P*8]
   int vmax = 2;                  // template choice
   int cmax = 6;
+  uint32_t smem_bytes = 0;       // dynamic shared memory of the (single) launch
+  uint32_t ctas_per_sm = 1;
 };
-
-uint32_t heap_rows(uint32_t c) { return c >= 2 ? c : 0; }  // nodes 2..c+1
-
-const uint32_t kSmemClasses[] = {16u << 10, 24u << 10, 32u << 10, 48u << 10, 64u << 10,
-                                 96u << 10, 128u << 10, kMaxSmem};
 
 uint32_t fixed_smem(int vmax, int cmax) {
   if (cmax <= 6) {
@@ -135,7 +127,16 @@ uint32_t fixed_smem(int vmax, int cmax) {
   return SmemLayout<8, 8>::fixed_bytes;
 }
 
-// plan_sel: which plans take part (all if null); plan_variant: stream variant per plan (0 if null)
+// registers per thread of the kernel variant the schedule selects (occupancy model of the packing)
+int kernel_regs(int vmax, int cmax);
+
+// Simulations -> warps -> thread blocks.
+//  * a warp holds <= 32 simulations of one topology and one stream variant; within a topology plans
+//    are ordered by heap footprint so that a warp's lanes need similar amounts of shared memory;
+//  * a thread block holds <= kWarpsPerCta warps of one variant whose heap regions fit a common
+//    budget; the budget (= blocks per SM) is chosen to maximise resident warps per SM;
+//  * ONE launch covers everything; blocks are ordered heaviest first so the tail is short.
+// only_plan: schedule just that plan (cf_trace_sim); plan_variant: stream variant per plan.
 int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
                        const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
                        Schedule* out) {
@@ -144,7 +145,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   sc.plan_c.assign((size_t)P * 8, 1);
   uint32_t maxV = 1;
   std::map<std::vector<uint8_t>, uint32_t> topo_id;
-  std::vector<uint32_t> plan_topo(P);
+  std::vector<uint32_t> plan_topo(P), plan_pairs(P, 0);
   for (uint32_t p = 0; p < P; ++p) {
     const uint32_t V = pl->n_stages[p];
     maxV = std::max(maxV, V);
@@ -159,13 +160,16 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       sc.topos.push_back(td);
     }
     plan_topo[p] = it->second;
-    for (uint32_t s = 0; s < V; ++s) sc.plan_c[(size_t)p * 8 + s] = pl->stage_c[(size_t)p * MS + s];
+    for (uint32_t s = 0; s < V; ++s) {
+      const uint16_t c = pl->stage_c[(size_t)p * MS + s];
+      sc.plan_c[(size_t)p * 8 + s] = c;
+      plan_pairs[p] += heap_pairs(c);
+    }
   }
   sc.cmax = g->n_comp <= 6 ? 6 : 8;
   sc.vmax = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 6 ? 6 : 8));
   const uint32_t fixed = fixed_smem(sc.vmax, sc.cmax);
 
-  // order plans by (variant, topology, replica vector) so that warps are homogeneous
   std::vector<uint32_t> order;
   if (only_plan) order.push_back(*only_plan);
   else { order.resize(P); std::iota(order.begin(), order.end(), 0u); }
@@ -175,88 +179,117 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   };
   for (uint32_t p : order)
     if (variant_of(p) >= std::max(1u, n_variants)) return CF_ERR_ARG;
+  // (variant, topology, heap footprint descending, replica vector) -> homogeneous warps
   std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) {
     const uint32_t va = variant_of(a), vb = variant_of(b);
     if (va != vb) return va < vb;
     if (plan_topo[a] != plan_topo[b]) return plan_topo[a] < plan_topo[b];
-    // heavier heaps first within a topology, then lexicographic replica vector
+    if (plan_pairs[a] != plan_pairs[b]) return plan_pairs[a] > plan_pairs[b];
     return std::lexicographical_compare(sc.plan_c.begin() + (size_t)b * 8, sc.plan_c.begin() + (size_t)b * 8 + 8,
                                         sc.plan_c.begin() + (size_t)a * 8, sc.plan_c.begin() + (size_t)a * 8 + 8);
   });
 
-  // simulations -> warps (same variant and topology, <= 32 lanes)
-  std::vector<uint32_t> warp_variant;
-  std::vector<uint32_t> warp_heap_bytes;
+  // simulations -> warps
+  struct WarpInfo { WarpDesc wd; uint32_t variant, heap_bytes, cost; };
+  std::vector<WarpInfo> winfo;
   size_t i = 0;
   while (i < order.size()) {
     size_t j = i;
     while (j < order.size() && variant_of(order[j]) == variant_of(order[i]) &&
            plan_topo[order[j]] == plan_topo[order[i]])
       ++j;
-    // group [i, j): emit sims plan-major, rate-minor
     const size_t sim0 = sc.sims.size();
     for (size_t q = i; q < j; ++q)
       for (uint32_t r = 0; r < R; ++r) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
     const size_t n_group = sc.sims.size() - sim0;
     const TopoDesc& td = sc.topos[plan_topo[order[i]]];
     for (size_t w0 = 0; w0 < n_group; w0 += 32) {
-      WarpDesc wd;
-      std::memset(&wd, 0, sizeof(wd));
-      wd.sim_begin = (uint32_t)(sim0 + w0);
-      wd.n_lanes = (uint32_t)std::min<size_t>(32, n_group - w0);
-      wd.topo = plan_topo[order[i]];
-      uint32_t off = 0;
-      for (uint32_t s = 0; s < td.n_stages; ++s) {
-        uint32_t rows = 0;
-        for (uint32_t l = 0; l < wd.n_lanes; ++l)
-          rows = std::max(rows, heap_rows(sc.plan_c[(size_t)sc.sims[wd.sim_begin + l].plan * 8 + s]));
-        wd.heap_off[s] = off;
-        off += rows * 256u;
+      WarpInfo wi;
+      std::memset(&wi, 0, sizeof(wi));
+      wi.wd.sim_begin = (uint32_t)(sim0 + w0);
+      wi.wd.n_lanes = (uint32_t)std::min<size_t>(32, n_group - w0);
+      wi.wd.topo = plan_topo[order[i]];
+      uint32_t pairs = 0, cost = 0;
+      for (uint32_t l = 0; l < wi.wd.n_lanes; ++l) {
+        const uint32_t p = sc.sims[wi.wd.sim_begin + l].plan;
+        pairs = std::max(pairs, plan_pairs[p]);
+        uint32_t cp = 0;  // rough time of one request: 2 units per stage + 3 per heap level
+        for (uint32_t s = 0; s < td.n_stages; ++s) {
+          uint32_t c = sc.plan_c[(size_t)p * 8 + s], lv = 0;
+          while (c > 1) { ++lv; c >>= 1; }
+          cp += 2 + 3 * lv;
+        }
+        cost = std::max(cost, cp);
       }
-      if (fixed + off > kMaxSmem) return CF_ERR_RANGE;  // replica counts too large for one SM
-      sc.warps.push_back(wd);
-      warp_variant.push_back(variant_of(order[i]));
-      warp_heap_bytes.push_back(off);
+      wi.heap_bytes = pairs * 512u;
+      wi.cost = cost;
+      wi.variant = variant_of(order[i]);
+      if (fixed + wi.heap_bytes > kMaxSmem) return CF_ERR_RANGE;  // replica counts too large for one SM
+      winfo.push_back(wi);
     }
     i = j;
   }
+  // slow (deep-heap) warps together: a block advances tile by tile at the pace of its slowest warp
+  std::stable_sort(winfo.begin(), winfo.end(), [](const WarpInfo& a, const WarpInfo& b) {
+    if (a.variant != b.variant) return a.variant < b.variant;
+    if (a.heap_bytes != b.heap_bytes) return a.heap_bytes > b.heap_bytes;
+    return a.cost > b.cost;
+  });
+  uint32_t max_heap = 0;
+  for (const WarpInfo& wi : winfo) max_heap = std::max(max_heap, wi.heap_bytes);
 
-  // warps -> CTAs (same variant, <= kWarpsPerCta warps, shared memory within the limit)
-  std::vector<CtaDesc> ctas;
-  size_t w = 0;
-  while (w < sc.warps.size()) {
-    CtaDesc cd;
-    cd.warp_begin = (uint32_t)w;
-    cd.n_warps = 0;
-    cd.variant = warp_variant[w];
-    cd.heap_bytes = 0;
-    // keep CTAs at <= 64 KiB where possible so several fit on an SM
-    const uint32_t soft = std::max<uint32_t>(64u << 10, fixed + warp_heap_bytes[w]);
-    while (w < sc.warps.size() && cd.n_warps < (uint32_t)kWarpsPerCta && warp_variant[w] == cd.variant &&
-           fixed + cd.heap_bytes + warp_heap_bytes[w] <= soft) {
-      // heap offsets become CTA-relative
-      for (int s = 0; s < 8; ++s) sc.warps[w].heap_off[s] += cd.heap_bytes;
-      cd.heap_bytes += warp_heap_bytes[w];
-      ++cd.n_warps;
-      ++w;
+  // choose blocks per SM: pack under each candidate budget, keep the one with most resident warps
+  const uint32_t sm_smem = 228u * 1024u, reserved = 1024u;
+  const uint32_t reg_warps = 65536u / (32u * (uint32_t)std::max(32, kernel_regs(sc.vmax, sc.cmax)));
+  auto pack = [&](uint32_t budget, std::vector<CtaDesc>* ctas, std::vector<uint32_t>* woff) {
+    ctas->clear();
+    if (woff) woff->assign(winfo.size(), 0);
+    size_t w = 0;
+    while (w < winfo.size()) {
+      CtaDesc cd{(uint32_t)w, 0, winfo[w].variant, 0};
+      while (w < winfo.size() && cd.n_warps < (uint32_t)kWarpsPerCta && winfo[w].variant == cd.variant &&
+             (cd.n_warps == 0 || fixed + cd.heap_bytes + winfo[w].heap_bytes <= budget)) {
+        if (woff) (*woff)[w] = cd.heap_bytes;
+        cd.heap_bytes += winfo[w].heap_bytes;
+        ++cd.n_warps;
+        ++w;
+      }
+      ctas->push_back(cd);
     }
-    ctas.push_back(cd);
-  }
-  // launch classes by shared-memory size
-  auto cls = [&](const CtaDesc& c) {
-    const uint32_t need = fixed + c.heap_bytes;
-    for (uint32_t k : kSmemClasses)
-      if (need <= k) return k;
-    return kMaxSmem;
   };
-  std::stable_sort(ctas.begin(), ctas.end(), [&](const CtaDesc& a, const CtaDesc& b) { return cls(a) > cls(b); });
-  sc.ctas = ctas;
-  for (size_t c = 0; c < ctas.size();) {
-    size_t e = c;
-    while (e < ctas.size() && cls(ctas[e]) == cls(ctas[c])) ++e;
-    sc.launches.push_back(Launch{(uint32_t)c, (uint32_t)(e - c), cls(ctas[c])});
-    c = e;
+  double best_score = -1.0;
+  uint32_t best_m = 1, best_budget = kMaxSmem;
+  std::vector<CtaDesc> trial_ctas;
+  for (uint32_t m = 1; m <= 16; ++m) {
+    uint32_t budget = std::min(kMaxSmem, (sm_smem / m - reserved) & ~127u);
+    if (budget < fixed + max_heap) break;
+    pack(budget, &trial_ctas, nullptr);
+    const double warps_per_cta = (double)winfo.size() / (double)trial_ctas.size();
+    // every block owns kWarpsPerCta warp slots and their registers, however many warps are active
+    const double resident = std::min<double>({(double)m, (double)(reg_warps / kWarpsPerCta), 32.0}) * warps_per_cta;
+    if (resident > best_score * 1.02) { best_score = resident; best_m = m; best_budget = budget; }
   }
+  std::vector<uint32_t> woff;
+  pack(best_budget, &sc.ctas, &woff);
+  uint32_t need = fixed;
+  for (const CtaDesc& c : sc.ctas) need = std::max(need, fixed + c.heap_bytes);
+  sc.smem_bytes = need;
+  sc.ctas_per_sm = best_m;
+  sc.warps.resize(winfo.size());
+  for (size_t w = 0; w < winfo.size(); ++w) {
+    sc.warps[w] = winfo[w].wd;
+    sc.warps[w].heap_off = woff[w];
+  }
+  // heaviest blocks first
+  std::vector<uint32_t> cta_cost(sc.ctas.size(), 0), idx(sc.ctas.size());
+  for (size_t c = 0; c < sc.ctas.size(); ++c)
+    for (uint32_t w = 0; w < sc.ctas[c].n_warps; ++w)
+      cta_cost[c] = std::max(cta_cost[c], winfo[sc.ctas[c].warp_begin + w].cost);
+  std::iota(idx.begin(), idx.end(), 0u);
+  std::stable_sort(idx.begin(), idx.end(), [&](uint32_t a, uint32_t b) { return cta_cost[a] > cta_cost[b]; });
+  std::vector<CtaDesc> sorted(sc.ctas.size());
+  for (size_t c = 0; c < idx.size(); ++c) sorted[c] = sc.ctas[idx[c]];
+  sc.ctas.swap(sorted);
   return CF_OK;
 }
 
@@ -339,27 +372,45 @@ void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool
 // launches
 // ------------------------------------------------------------------------------------------------
 template <int VMAX, int CMAX, bool HAS_DELAY>
-cudaError_t launch_one(const KParams& kp, const Launch& L, uint32_t n_trials, cudaStream_t st) {
+cudaError_t launch_one(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
   auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
   if (e != cudaSuccess) return e;
-  // grid.y is limited to 65535: n_trials <= 65535 is validated
-  kern<<<dim3(L.n_ctas, n_trials), kThreads, L.smem_bytes, st>>>(kp, L.cta_begin);
+  kp.k_launch = n_trials;
+  // 1-D grid, block b = (CTA b / n_trials, trial b % n_trials): <= 2^31-1 blocks
+  const uint64_t blocks = (uint64_t)sc.ctas.size() * n_trials;
+  if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+  kern<<<(uint32_t)blocks, kThreads, sc.smem_bytes, st>>>(kp, 0u);
   ++g_launch_count;
   return cudaGetLastError();
 }
 
+template <int VMAX, int CMAX>
+int regs_of() {
+  static int regs = [] {
+    cudaFuncAttributes a;
+    if (cudaFuncGetAttributes(&a, cf_sim_kernel<VMAX, CMAX, false>) != cudaSuccess) {
+      cudaGetLastError();
+      return VMAX <= 2 ? 64 : 128;  // ptxas figures of this build; used when no device is present
+    }
+    return a.numRegs;
+  }();
+  return regs;
+}
+
 cudaError_t launch_sims(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
   const bool d = kp.edge_delay != 0;
-  for (const Launch& L : sc.launches) {
-    cudaError_t e;
-    if (sc.cmax == 8) e = d ? launch_one<8, 8, true>(kp, L, n_trials, st) : launch_one<8, 8, false>(kp, L, n_trials, st);
-    else if (sc.vmax == 2) e = d ? launch_one<2, 6, true>(kp, L, n_trials, st) : launch_one<2, 6, false>(kp, L, n_trials, st);
-    else if (sc.vmax == 6) e = d ? launch_one<6, 6, true>(kp, L, n_trials, st) : launch_one<6, 6, false>(kp, L, n_trials, st);
-    else e = d ? launch_one<8, 6, true>(kp, L, n_trials, st) : launch_one<8, 6, false>(kp, L, n_trials, st);
-    if (e != cudaSuccess) return e;
-  }
-  return cudaSuccess;
+  if (sc.cmax == 8) return d ? launch_one<8, 8, true>(kp, sc, n_trials, st) : launch_one<8, 8, false>(kp, sc, n_trials, st);
+  if (sc.vmax == 2) return d ? launch_one<2, 6, true>(kp, sc, n_trials, st) : launch_one<2, 6, false>(kp, sc, n_trials, st);
+  if (sc.vmax == 6) return d ? launch_one<6, 6, true>(kp, sc, n_trials, st) : launch_one<6, 6, false>(kp, sc, n_trials, st);
+  return d ? launch_one<8, 6, true>(kp, sc, n_trials, st) : launch_one<8, 6, false>(kp, sc, n_trials, st);
+}
+
+int kernel_regs(int vmax, int cmax) {
+  if (cmax == 8) return regs_of<8, 8>();
+  if (vmax == 2) return regs_of<2, 6>();
+  if (vmax == 6) return regs_of<6, 6>();
+  return regs_of<8, 6>();
 }
 
 int32_t check_workspace(void* ws, size_t have, size_t need) {

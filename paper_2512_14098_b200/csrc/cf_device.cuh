@@ -9,8 +9,8 @@
 //   * each warp holds simulations of one plan topology; it turns 32 component-level records into
 //     stage-level records (a4) once per chunk, so the per-request loop sees only {cu, type, S[s]};
 //   * a5/a6: the free-time multiset of a c-replica stage is a binary min-heap of int64 per thread,
-//     root in a register, nodes 2..c+1 in shared memory interleaved by lane (bank = lane, no
-//     conflicts); c = 1 degenerates to the Lindley recursion with no memory traffic;
+//     root in a register, nodes 2..c+1 in shared memory as sibling pairs interleaved by lane (one
+//     conflict-free LDS.128 per level); c = 1 degenerates to the Lindley recursion, no memory traffic;
 //   * a7 hand-off is the running x; a8 counters are packed per-type byte fields flushed per chunk.
 #pragma once
 #include <cstdint>
@@ -41,13 +41,18 @@ struct SimDesc {
 };
 
 struct WarpDesc {
-  uint32_t sim_begin, n_lanes, topo, pad;
-  uint32_t heap_off[8];  // byte offset of this warp's stage-s heap region in the CTA heap arena
+  uint32_t sim_begin, n_lanes, topo;
+  uint32_t heap_off;  // byte offset of this warp's heap region in the CTA heap arena
 };
 
 struct CtaDesc {
   uint32_t warp_begin, n_warps, variant, heap_bytes;
 };
+
+// Heap storage of one c-replica stage of one lane: floor(c/2) sibling pairs (nodes 2i, 2i+1), one
+// 512-byte row per pair (32 lanes x 16 B). A lane's stages follow one another, so a warp's region
+// is 512 B x max over its lanes of sum_s floor(c_s/2).
+__host__ __device__ __forceinline__ uint32_t heap_pairs(uint32_t c) { return c >> 1; }
 
 struct KParams {
   uint32_t C, T, N, K;
@@ -64,7 +69,8 @@ struct KParams {
   const uint4* stream;
   uint32_t variant_lo;
   uint32_t bisect_mode;  // rate 0 means "skip this simulation" instead of a range error
-  uint32_t trial_base;   // trial = trial_base + blockIdx.y (cf_trace_sim runs one trial)
+  uint32_t trial_base;   // trial = trial_base + blockIdx.x % k_launch (cf_trace_sim runs one trial)
+  uint32_t k_launch;     // trials per launch; CTA = blockIdx.x / k_launch (heavy CTAs first)
   // schedule
   const CtaDesc* ctas;
   const WarpDesc* warps;
@@ -191,44 +197,37 @@ __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_
 }
 
 // ------------------------------------------------------------------------------------------------
-// Min-heap replace-min (a6). root = current minimum (register); nodes 2..c live in shared memory at
-// heap + (j-2)*256 (256 B = 32 lanes x 8 B per node row), node c+1 holds +inf.
+// Min-heap replace-min (a6). root = current minimum (register). Nodes 2..c live in shared memory as
+// sibling pairs: pair i = nodes (2i, 2i+1) at hb + (i-1)*512 (+ lane*16 folded into hb), fetched
+// with one LDS.128; if c is even, node c+1 holds +inf. Top-down sift of the new value x.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int64_t lds64(const uint8_t* smem, uint32_t off) {
-  return *reinterpret_cast<const int64_t*>(smem + off);
-}
-__device__ __forceinline__ void sts64(uint8_t* smem, uint32_t off, int64_t v) {
-  *reinterpret_cast<int64_t*>(smem + off) = v;
-}
-
 __device__ __forceinline__ void heap_replace_min(uint8_t* smem, int64_t& root, uint32_t hb,
                                                  uint32_t c, int64_t x) {
   if (c < 2) {
     root = x;
     return;
   }
-  int64_t a = lds64(smem, hb), b = lds64(smem, hb + 256);
-  bool bl = b < a;
-  int64_t m = bl ? b : a;
+  longlong2 pr = *reinterpret_cast<const longlong2*>(smem + hb);
+  bool bl = pr.y < pr.x;
+  int64_t m = bl ? pr.y : pr.x;
   if (x <= m) {
     root = x;
     return;
   }
   root = m;
-  uint32_t i = 2u + (bl ? 1u : 0u);  // the hole
-  while (true) {
-    const uint32_t child = 2u * i;
-    if (child > c) break;
-    const uint32_t pa = hb + (child - 2u) * 256u;
-    a = lds64(smem, pa);
-    b = lds64(smem, pa + 256u);
-    bl = b < a;
-    m = bl ? b : a;
+  uint32_t i = 2u + (bl ? 1u : 0u);            // the hole (node index)
+  uint32_t hole = hb + (bl ? 8u : 0u);         // its byte address
+  while (2u * i <= c) {
+    const uint32_t pa = hb + (i - 1u) * 512u;  // pair i = children of node i
+    pr = *reinterpret_cast<const longlong2*>(smem + pa);
+    bl = pr.y < pr.x;
+    m = bl ? pr.y : pr.x;
     if (x <= m) break;
-    sts64(smem, hb + (i - 2u) * 256u, m);
-    i = child + (bl ? 1u : 0u);
+    *reinterpret_cast<int64_t*>(smem + hole) = m;
+    hole = pa + (bl ? 8u : 0u);
+    i = 2u * i + (bl ? 1u : 0u);
   }
-  sts64(smem, hb + (i - 2u) * 256u, x);
+  *reinterpret_cast<int64_t*>(smem + hole) = x;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -254,8 +253,8 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   using SL = SmemLayout<VMAX, CMAX>;
   extern __shared__ __align__(16) uint8_t smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t trial = prm.trial_base + blockIdx.y;
-  const CtaDesc cta = prm.ctas[cta_base + blockIdx.x];
+  const uint32_t trial = prm.trial_base + blockIdx.x % prm.k_launch;
+  const CtaDesc cta = prm.ctas[cta_base + blockIdx.x / prm.k_launch];
   const uint32_t variant = prm.variant_lo + cta.variant;
 
   uint4* tiles = reinterpret_cast<uint4*>(smem + SL::tiles);
@@ -290,13 +289,18 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
     } else {
       period = (1000000000u + rate / 2u) / rate;
     }
+    uint32_t row = 0;  // this lane's stages are laid out one after another
 #pragma unroll
     for (int s = 0; s < VMAX; ++s) {
       if (s < topo.n_stages) {
         sim_c[s] = prm.plan_c[sd.plan * 8 + s];
-        hb[s] = SL::heaps + wd.heap_off[s] + lane * 8;
-        for (uint32_t j = 2; j <= sim_c[s]; ++j) sts64(smem, hb[s] + (j - 2u) * 256u, 0);
-        if (sim_c[s] >= 2) sts64(smem, hb[s] + (sim_c[s] - 1u) * 256u, kInf);  // node c+1
+        hb[s] = SL::heaps + wd.heap_off + row * 512u + lane * 16u;
+        const uint32_t np = heap_pairs(sim_c[s]);
+        for (uint32_t j = 0; j < np; ++j) {
+          const bool sentinel = (j + 1 == np) && !(sim_c[s] & 1u);  // node c+1 closes an even heap
+          *reinterpret_cast<longlong2*>(smem + hb[s] + j * 512u) = make_longlong2(0, sentinel ? kInf : 0);
+        }
+        row += np;
       }
     }
   }

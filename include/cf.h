@@ -159,6 +159,15 @@ int32_t cf_workspace_status(const void* workspace, void* stream);
 /* Number of kernels the last call on this workspace's host thread enqueued (bench bookkeeping). */
 uint32_t cf_last_launch_count(void);
 
+/* The simulation runs on a 32-bit fast kernel (times as uint32 offsets from a per-tile origin,
+ * DESIGN.md 5.2) followed by the 64-bit kernel over exactly those simulations that left the 32-bit
+ * window; results are bit-identical either way. cf_workspace_wide_count synchronises `stream` and
+ * returns how many simulations of the last call on `workspace` were redone by the 64-bit kernel
+ * (>= 0), or a negative cf_status. cf_debug_kernel_mode (tests): 0 = automatic (default),
+ * 1 = 64-bit kernel only; applies to later calls made by the calling host thread. */
+int64_t cf_workspace_wide_count(const void* workspace, void* stream);
+int32_t cf_debug_kernel_mode(uint32_t mode);
+
 /* Micro-benchmark used by bench.py for the ALU roofline denominator: runs `iters` rounds of an
  * unrolled, independent 32-bit integer instruction mix on every SM and writes the number of
  * lane-operations executed to *out_ops (host). mix: 0 = IADD3/LOP3 only (ALU pipe), 1 = IMAD only

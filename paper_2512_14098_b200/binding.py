@@ -22,7 +22,8 @@ CF_OK, CF_ERR_ARG, CF_ERR_RANGE, CF_ERR_PLAN, CF_ERR_TABLE, CF_ERR_CUDA, CF_ERR_
 EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_stream_bytes",
            "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status",
-           "cf_last_launch_count", "cf_bench_int32_peak", "cf_strerror"]
+           "cf_last_launch_count", "cf_bench_int32_peak", "cf_strerror", "cf_workspace_wide_count",
+           "cf_debug_kernel_mode"]
 
 
 class CfError(RuntimeError):
@@ -64,6 +65,8 @@ _lib.cf_stream_bytes.restype = C.c_size_t
 _lib.cf_materialize_workspace_bytes.restype = C.c_size_t
 _lib.cf_strerror.restype = C.c_char_p
 _lib.cf_last_launch_count.restype = C.c_uint32
+_lib.cf_workspace_wide_count.restype = C.c_int64
+_lib.cf_debug_kernel_mode.restype = C.c_int32
 for _n in ("cf_eval_plans", "cf_goodput_bisect", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak"):
     getattr(_lib, _n).restype = C.c_int32
@@ -146,6 +149,18 @@ def _as_dev_u32(x, device) -> torch.Tensor:
 
 def cf_workspace_status(workspace: torch.Tensor, stream=None) -> int:
     return int(_lib.cf_workspace_status(_dp(workspace), _stream_ptr(stream)))
+
+
+def cf_workspace_wide_count(workspace: torch.Tensor, stream=None) -> int:
+    """Simulations of the last call on `workspace` that the 64-bit kernel had to redo."""
+    return int(_lib.cf_workspace_wide_count(_dp(workspace), _stream_ptr(stream)))
+
+
+def cf_debug_kernel_mode(mode: int) -> None:
+    """0 = automatic (32-bit fast kernel + 64-bit fixup), 1 = 64-bit kernel only (tests)."""
+    rc = int(_lib.cf_debug_kernel_mode(C.c_uint32(mode)))
+    if rc != CF_OK:
+        raise CfError(rc, "cf_debug_kernel_mode")
 
 
 def cf_last_launch_count() -> int:

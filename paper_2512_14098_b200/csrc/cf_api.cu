@@ -12,13 +12,14 @@
 #include <vector>
 
 #include "../../include/cf.h"
-#include "cf_device.cuh"
+#include "cf_rel32.cuh"
 
 using namespace cfk;
 
 namespace {
 
 thread_local uint32_t g_launch_count = 0;
+thread_local uint32_t g_kernel_mode = 0;  // cf_debug_kernel_mode: 0 auto, 1 = 64-bit kernel only
 
 constexpr size_t kAlign = 256;
 constexpr uint32_t kMaxSmem = 227u * 1024u;
@@ -112,9 +113,11 @@ struct Schedule {
   std::vector<WarpDesc> warps;
   std::vector<CtaDesc> ctas;
   std::vector<uint16_t> plan_c;  // [P*8]
-  int vmax = 2;                  // template choice
+  int vmax = 2;                  // template choice of the 64-bit kernel
+  int vmax32 = 2;                // ... and of the 32-bit kernel
   int cmax = 6;
-  uint32_t smem_bytes = 0;       // dynamic shared memory of the (single) launch
+  uint32_t smem_bytes = 0;       // dynamic shared memory of the 64-bit launch
+  uint32_t smem_bytes32 = 0;     // ... of the 32-bit launch
   uint32_t ctas_per_sm = 1;
 };
 
@@ -127,8 +130,19 @@ uint32_t fixed_smem(int vmax, int cmax) {
   return SmemLayout<8, 8>::fixed_bytes;
 }
 
+uint32_t fixed_smem32(int vmax, int cmax) {
+  if (cmax <= 6) {
+    if (vmax <= 2) return SmemLayout32<2, 6>::fixed_bytes;
+    if (vmax <= 4) return SmemLayout32<4, 6>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout32<6, 6>::fixed_bytes;
+    return SmemLayout32<8, 6>::fixed_bytes;
+  }
+  return SmemLayout32<8, 8>::fixed_bytes;
+}
+
 // registers per thread of the kernel variant the schedule selects (occupancy model of the packing)
 int kernel_regs(int vmax, int cmax);
+int kernel_regs32(int vmax, int cmax);
 
 // Simulations -> warps -> thread blocks.
 //  * a warp holds <= 32 simulations of one topology and one stream variant; within a topology plans
@@ -137,15 +151,17 @@ int kernel_regs(int vmax, int cmax);
 //    budget; the budget (= blocks per SM) is chosen to maximise resident warps per SM;
 //  * ONE launch covers everything; blocks are ordered heaviest first so the tail is short.
 // only_plan: schedule just that plan (cf_trace_sim); plan_variant: stream variant per plan.
+// fast: pack for the 32-bit kernel (its heap rows set the occupancy); the 64-bit kernel then reuses
+// the same warps and blocks with its own, larger heap offsets.
 int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
                        const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
-                       Schedule* out) {
+                       bool fast, Schedule* out) {
   const uint32_t P = pl->n_plans, MS = pl->max_stages;
   Schedule& sc = *out;
   sc.plan_c.assign((size_t)P * 8, 1);
   uint32_t maxV = 1;
   std::map<std::vector<uint8_t>, uint32_t> topo_id;
-  std::vector<uint32_t> plan_topo(P), plan_pairs(P, 0);
+  std::vector<uint32_t> plan_topo(P), plan_pairs(P, 0), plan_quads(P, 0);
   for (uint32_t p = 0; p < P; ++p) {
     const uint32_t V = pl->n_stages[p];
     maxV = std::max(maxV, V);
@@ -164,11 +180,14 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       const uint16_t c = pl->stage_c[(size_t)p * MS + s];
       sc.plan_c[(size_t)p * 8 + s] = c;
       plan_pairs[p] += heap_pairs(c);
+      plan_quads[p] += heap_quads(c);
     }
   }
   sc.cmax = g->n_comp <= 6 ? 6 : 8;
   sc.vmax = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 6 ? 6 : 8));
-  const uint32_t fixed = fixed_smem(sc.vmax, sc.cmax);
+  sc.vmax32 = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 4 ? 4 : (maxV <= 6 ? 6 : 8)));
+  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax), fixed_f = fixed_smem32(sc.vmax32, sc.cmax);
+  const uint32_t fixed = fast ? fixed_f : fixed_w;  // the layout that is packed for occupancy
 
   std::vector<uint32_t> order;
   if (only_plan) order.push_back(*only_plan);
@@ -184,13 +203,14 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
     const uint32_t va = variant_of(a), vb = variant_of(b);
     if (va != vb) return va < vb;
     if (plan_topo[a] != plan_topo[b]) return plan_topo[a] < plan_topo[b];
-    if (plan_pairs[a] != plan_pairs[b]) return plan_pairs[a] > plan_pairs[b];
+    const std::vector<uint32_t>& rows = fast ? plan_quads : plan_pairs;
+    if (rows[a] != rows[b]) return rows[a] > rows[b];
     return std::lexicographical_compare(sc.plan_c.begin() + (size_t)b * 8, sc.plan_c.begin() + (size_t)b * 8 + 8,
                                         sc.plan_c.begin() + (size_t)a * 8, sc.plan_c.begin() + (size_t)a * 8 + 8);
   });
 
   // simulations -> warps
-  struct WarpInfo { WarpDesc wd; uint32_t variant, heap_bytes, cost; };
+  struct WarpInfo { WarpDesc wd; uint32_t variant, heap_bytes, heap_w, heap_f, cost; };
   std::vector<WarpInfo> winfo;
   size_t i = 0;
   while (i < order.size()) {
@@ -209,10 +229,11 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       wi.wd.sim_begin = (uint32_t)(sim0 + w0);
       wi.wd.n_lanes = (uint32_t)std::min<size_t>(32, n_group - w0);
       wi.wd.topo = plan_topo[order[i]];
-      uint32_t pairs = 0, cost = 0;
+      uint32_t pairs = 0, quads = 0, cost = 0;
       for (uint32_t l = 0; l < wi.wd.n_lanes; ++l) {
         const uint32_t p = sc.sims[wi.wd.sim_begin + l].plan;
         pairs = std::max(pairs, plan_pairs[p]);
+        quads = std::max(quads, plan_quads[p]);
         uint32_t cp = 0;  // rough time of one request: 2 units per stage + 3 per heap level
         for (uint32_t s = 0; s < td.n_stages; ++s) {
           uint32_t c = sc.plan_c[(size_t)p * 8 + s], lv = 0;
@@ -221,10 +242,13 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
         }
         cost = std::max(cost, cp);
       }
-      wi.heap_bytes = pairs * 512u;
+      wi.heap_w = pairs * 512u;
+      wi.heap_f = quads * 512u;
+      wi.wd.heap_rows32 = quads;
+      wi.heap_bytes = fast ? wi.heap_f : wi.heap_w;
       wi.cost = cost;
       wi.variant = variant_of(order[i]);
-      if (fixed + wi.heap_bytes > kMaxSmem) return CF_ERR_RANGE;  // replica counts too large for one SM
+      if (fixed_w + wi.heap_w > kMaxSmem) return CF_ERR_RANGE;  // replica counts too large for one SM
       winfo.push_back(wi);
     }
     i = j;
@@ -240,17 +264,24 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
 
   // choose blocks per SM: pack under each candidate budget, keep the one with most resident warps
   const uint32_t sm_smem = 228u * 1024u, reserved = 1024u;
-  const uint32_t reg_warps = 65536u / (32u * (uint32_t)std::max(32, kernel_regs(sc.vmax, sc.cmax)));
-  auto pack = [&](uint32_t budget, std::vector<CtaDesc>* ctas, std::vector<uint32_t>* woff) {
+  const int regs = fast ? kernel_regs32(sc.vmax32, sc.cmax) : kernel_regs(sc.vmax, sc.cmax);
+  const uint32_t reg_warps = 65536u / (32u * (uint32_t)std::max(32, regs));
+  auto pack = [&](uint32_t budget, std::vector<CtaDesc>* ctas, bool assign) {
     ctas->clear();
-    if (woff) woff->assign(winfo.size(), 0);
     size_t w = 0;
     while (w < winfo.size()) {
-      CtaDesc cd{(uint32_t)w, 0, winfo[w].variant, 0};
+      CtaDesc cd{(uint32_t)w, 0, winfo[w].variant, 0, 0};
+      uint32_t packed = 0;  // heap bytes of the layout being packed
       while (w < winfo.size() && cd.n_warps < (uint32_t)kWarpsPerCta && winfo[w].variant == cd.variant &&
-             (cd.n_warps == 0 || fixed + cd.heap_bytes + winfo[w].heap_bytes <= budget)) {
-        if (woff) (*woff)[w] = cd.heap_bytes;
-        cd.heap_bytes += winfo[w].heap_bytes;
+             (cd.n_warps == 0 || (fixed + packed + winfo[w].heap_bytes <= budget &&
+                                  fixed_w + cd.heap_bytes + winfo[w].heap_w <= kMaxSmem))) {
+        if (assign) {
+          winfo[w].wd.heap_off = cd.heap_bytes;
+          winfo[w].wd.heap_off32 = cd.heap_bytes32;
+        }
+        packed += winfo[w].heap_bytes;
+        cd.heap_bytes += winfo[w].heap_w;
+        cd.heap_bytes32 += winfo[w].heap_f;
         ++cd.n_warps;
         ++w;
       }
@@ -263,23 +294,23 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   for (uint32_t m = 1; m <= 16; ++m) {
     uint32_t budget = std::min(kMaxSmem, (sm_smem / m - reserved) & ~127u);
     if (budget < fixed + max_heap) break;
-    pack(budget, &trial_ctas, nullptr);
+    pack(budget, &trial_ctas, false);
     const double warps_per_cta = (double)winfo.size() / (double)trial_ctas.size();
     // every block owns kWarpsPerCta warp slots and their registers, however many warps are active
     const double resident = std::min<double>({(double)m, (double)(reg_warps / kWarpsPerCta), 32.0}) * warps_per_cta;
     if (resident > best_score * 1.02) { best_score = resident; best_m = m; best_budget = budget; }
   }
-  std::vector<uint32_t> woff;
-  pack(best_budget, &sc.ctas, &woff);
-  uint32_t need = fixed;
-  for (const CtaDesc& c : sc.ctas) need = std::max(need, fixed + c.heap_bytes);
-  sc.smem_bytes = need;
+  pack(best_budget, &sc.ctas, true);
+  uint32_t need_w = fixed_w, need_f = fixed_f;
+  for (const CtaDesc& c : sc.ctas) {
+    need_w = std::max(need_w, fixed_w + c.heap_bytes);
+    need_f = std::max(need_f, fixed_f + c.heap_bytes32);
+  }
+  sc.smem_bytes = need_w;
+  sc.smem_bytes32 = need_f;
   sc.ctas_per_sm = best_m;
   sc.warps.resize(winfo.size());
-  for (size_t w = 0; w < winfo.size(); ++w) {
-    sc.warps[w] = winfo[w].wd;
-    sc.warps[w].heap_off = woff[w];
-  }
+  for (size_t w = 0; w < winfo.size(); ++w) sc.warps[w] = winfo[w].wd;
   // heaviest blocks first
   std::vector<uint32_t> cta_cost(sc.ctas.size(), 0), idx(sc.ctas.size());
   for (size_t c = 0; c < sc.ctas.size(); ++c)
@@ -411,6 +442,81 @@ int kernel_regs(int vmax, int cmax) {
   if (vmax == 2) return regs_of<2, 6>();
   if (vmax == 6) return regs_of<6, 6>();
   return regs_of<8, 6>();
+}
+
+// ---- the 32-bit fast kernel (cf_rel32.cuh) ---------------------------------------------------------
+template <int VMAX, int CMAX, bool HAS_DELAY>
+cudaError_t launch_one32(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  auto kern = cf_sim32_kernel<VMAX, CMAX, HAS_DELAY>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+  if (e != cudaSuccess) return e;
+  kp.k_launch = n_trials;
+  const uint64_t blocks = (uint64_t)sc.ctas.size() * n_trials;
+  if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+  kern<<<(uint32_t)blocks, kThreads, sc.smem_bytes32, st>>>(kp);
+  ++g_launch_count;
+  return cudaGetLastError();
+}
+
+template <int VMAX, int CMAX>
+int regs_of32() {
+  static int regs = [] {
+    cudaFuncAttributes a;
+    if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false>) != cudaSuccess) {
+      cudaGetLastError();
+      return 96;  // __launch_bounds__ cap of this build; used when no device is present
+    }
+    return a.numRegs;
+  }();
+  return regs;
+}
+
+int kernel_regs32(int vmax, int cmax) {
+  if (cmax == 8) return regs_of32<8, 8>();
+  if (vmax == 2) return regs_of32<2, 6>();
+  if (vmax == 4) return regs_of32<4, 6>();
+  if (vmax == 6) return regs_of32<6, 6>();
+  return regs_of32<8, 6>();
+}
+
+cudaError_t launch_sims32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  const bool d = kp.edge_delay != 0;
+  if (sc.cmax == 8) return d ? launch_one32<8, 8, true>(kp, sc, n_trials, st) : launch_one32<8, 8, false>(kp, sc, n_trials, st);
+  if (sc.vmax32 == 2) return d ? launch_one32<2, 6, true>(kp, sc, n_trials, st) : launch_one32<2, 6, false>(kp, sc, n_trials, st);
+  if (sc.vmax32 == 4) return d ? launch_one32<4, 6, true>(kp, sc, n_trials, st) : launch_one32<4, 6, false>(kp, sc, n_trials, st);
+  if (sc.vmax32 == 6) return d ? launch_one32<6, 6, true>(kp, sc, n_trials, st) : launch_one32<6, 6, false>(kp, sc, n_trials, st);
+  return d ? launch_one32<8, 6, true>(kp, sc, n_trials, st) : launch_one32<8, 6, false>(kp, sc, n_trials, st);
+}
+
+// The 32-bit kernel needs max(A, F) + S + delay to stay below 2^32 whenever its inputs are inside the
+// 2^31 window: the worst-case service of a request over all its stages plus all its hops is capped
+// at 2^30. Anything else runs on the 64-bit kernel alone.
+bool fast_path_ok(const cf_graph* g) {
+  if (g_kernel_mode == 1) return false;
+  int64_t worst = 0;
+  for (uint32_t i = 0; i < g->n_comp; ++i) {
+    int64_t mx = 0;
+    for (uint32_t t = 0; t < g->n_types; ++t)
+      if ((g->type_mask[t] >> i) & 1) {
+        const cf_qtab& tb = g->tabs[g->svc_tab[i * g->n_types + t]];
+        mx = std::max<int64_t>(mx, tb.q[tab_entries(tb) - 1]);
+      }
+    worst += mx;
+  }
+  return worst + 7 * g->edge_delay_us <= (1ll << 30);
+}
+
+// One pass over the schedule: the 32-bit kernel, then the 64-bit kernel over the simulations that
+// left the 32-bit window (normally none: its blocks exit at once) -- or the 64-bit kernel alone.
+cudaError_t launch_pass(KParams kp, const Schedule& sc, uint32_t n_trials, bool fast, cudaStream_t st) {
+  if (!fast) {
+    kp.fixup = 0;
+    return launch_sims(kp, sc, n_trials, st);
+  }
+  cudaError_t e = launch_sims32(kp, sc, n_trials, st);
+  if (e != cudaSuccess) return e;
+  kp.fixup = 1;
+  return launch_sims(kp, sc, n_trials, st);
 }
 
 int32_t check_workspace(void* ws, size_t have, size_t need) {
@@ -604,15 +710,17 @@ int32_t eval_impl(const EvalArgs& a) {
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
   if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
+  const bool fast = fast_path_ok(a.g);
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);  // status block
   KParams kp;
   const size_t pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &kp);
   const SchedOffsets so = add_schedule(sc, &blob);
-  if (blob.bytes.size() > a.ws_bytes) return CF_ERR_WORKSPACE;
+  const size_t flags_off = align_up(blob.bytes.size());  // [P*R*K] bytes, written by the 32-bit kernel
+  if (flags_off + (size_t)a.pl->n_plans * a.R * a.g->n_trials > a.ws_bytes) return CF_ERR_WORKSPACE;
   uint8_t* ws = static_cast<uint8_t*>(a.ws);
   if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, a.st)))
     return rc;
@@ -623,7 +731,8 @@ int32_t eval_impl(const EvalArgs& a) {
   kp.out_counts = a.out_counts;
   kp.out_dep_sum = a.out_dep_sum;
   kp.out_makespan = a.out_makespan;
-  return cuda_rc(launch_sims(kp, sc, a.g->n_trials, a.st));
+  kp.flags = ws + flags_off;
+  return cuda_rc(launch_pass(kp, sc, a.g->n_trials, fast, a.st));
 }
 
 struct BisectArgs {
@@ -642,8 +751,9 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
+  const bool fast = fast_path_ok(a.g);
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, 1, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, 1, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);
@@ -657,7 +767,8 @@ int32_t bisect_impl(const BisectArgs& a) {
                mid_off = blob.reserve((size_t)P * 4);
   const size_t blob_bytes = blob.bytes.size();
   const size_t probe_off = align_up(blob_bytes), at_lo_off = align_up(probe_off + P * per_plan * 4);
-  if (at_lo_off + P * per_plan * 4 > a.ws_bytes) return CF_ERR_WORKSPACE;
+  const size_t flags_off = align_up(at_lo_off + P * per_plan * 4);
+  if (flags_off + (size_t)P * K > a.ws_bytes) return CF_ERR_WORKSPACE;
   uint8_t* ws = static_cast<uint8_t*>(a.ws);
   if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob_bytes, cudaMemcpyHostToDevice, a.st)))
     return rc;
@@ -673,11 +784,12 @@ int32_t bisect_impl(const BisectArgs& a) {
   kp.bisect_mode = 1;
   kp.rates = bs.mid;
   kp.out_counts = bs.probe;
+  kp.flags = ws + flags_off;
   const uint32_t nb = (P + 127) / 128;
   bisect_init_kernel<<<nb, 128, 0, a.st>>>(bs, a.rate_hi_dev, P, (uint32_t)per_plan);
   ++g_launch_count;
   for (uint32_t step = 0; step < a.n_steps; ++step) {
-    if (int32_t rc = cuda_rc(launch_sims(kp, sc, K, a.st))) return rc;
+    if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, fast, a.st))) return rc;
     bisect_update_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, reinterpret_cast<const uint32_t*>(ws + att_off),
                                                reinterpret_cast<const uint32_t*>(ws + den_off), kp.status);
     ++g_launch_count;
@@ -709,6 +821,7 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   n += 2 * kAlign + 3 * align_up(P * 4);                    // bisection: att, lo/hi/mid
   n += 2 * align_up(P * K * T * 2 * 4) + kAlign;            // probe + at_lo counts
   n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch
+  n += align_up(P * R * K) + kAlign;                        // 32-bit window flags
   const size_t chunks = ((size_t)g->n_req + 31) / 32;
   (void)chunks;
   return n + 4 * kAlign;
@@ -808,7 +921,7 @@ int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint3
   if (int32_t rc = check_workspace(workspace, workspace_bytes, cf_workspace_bytes(g, pl, 1))) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   Schedule sc;
-  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, &sc)) return rc;
+  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, false, &sc)) return rc;
   // the single simulation reads rate slot `plan` (pr = plan*1 + 0): upload a full-length rate array
   Blob blob;
   blob.reserve(kAlign);
@@ -845,6 +958,21 @@ int32_t cf_workspace_status(const void* workspace, void* stream) {
 }
 
 uint32_t cf_last_launch_count(void) { return g_launch_count; }
+
+int32_t cf_debug_kernel_mode(uint32_t mode) {
+  if (mode > 1) return CF_ERR_ARG;
+  g_kernel_mode = mode;
+  return CF_OK;
+}
+
+int64_t cf_workspace_wide_count(const void* workspace, void* stream) {
+  if (!workspace) return CF_ERR_WORKSPACE;
+  uint32_t n = 0;
+  cudaError_t e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+  if (e == cudaSuccess) e = cudaMemcpy(&n, static_cast<const uint8_t*>(workspace) + 4, sizeof(n), cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) return cuda_rc(e);
+  return (int64_t)n;
+}
 
 int32_t cf_bench_int32_peak(uint32_t mix, uint32_t iters, uint64_t* out_ops, uint64_t* out_usec,
                             void* stream) {

@@ -42,17 +42,21 @@ struct SimDesc {
 
 struct WarpDesc {
   uint32_t sim_begin, n_lanes, topo;
-  uint32_t heap_off;  // byte offset of this warp's heap region in the CTA heap arena
+  uint32_t heap_off;    // byte offset of this warp's heap region in the CTA heap arena (64-bit kernel)
+  uint32_t heap_off32;  // same for the 32-bit kernel (4-ary heap of uint32 quads)
+  uint32_t heap_rows32; // 512-byte rows of that region
 };
 
 struct CtaDesc {
-  uint32_t warp_begin, n_warps, variant, heap_bytes;
+  uint32_t warp_begin, n_warps, variant, heap_bytes, heap_bytes32;
 };
 
 // Heap storage of one c-replica stage of one lane: floor(c/2) sibling pairs (nodes 2i, 2i+1), one
 // 512-byte row per pair (32 lanes x 16 B). A lane's stages follow one another, so a warp's region
 // is 512 B x max over its lanes of sum_s floor(c_s/2).
 __host__ __device__ __forceinline__ uint32_t heap_pairs(uint32_t c) { return c >> 1; }
+// 32-bit kernel: 4-ary heap, root in a register, nodes 1..c-1 in ceil((c-1)/4) quads (16 B per lane)
+__host__ __device__ __forceinline__ uint32_t heap_quads(uint32_t c) { return (c + 2) >> 2; }
 
 struct KParams {
   uint32_t C, T, N, K;
@@ -82,7 +86,11 @@ struct KParams {
   uint32_t* out_counts;    // [PR][K][T][2]
   uint64_t* out_dep_sum;   // [PR][K] or null
   int64_t* out_makespan;   // [PR][K] or null
-  int32_t* status;         // sticky device status
+  int32_t* status;         // sticky device status; status[1] = simulations sent to the 64-bit kernel
+  // 32-bit fast path (cf_rel32.cuh): flags[slot] = 1 <=> the simulation left the 32-bit window and
+  // must be redone by the 64-bit kernel, which then runs with fixup = 1 and touches only those.
+  uint8_t* flags;          // [PR][K] or null
+  uint32_t fixup;
   int64_t* tr_arrival;     // trace (single simulation) or null
   int64_t* tr_departure;
   uint8_t* tr_type;
@@ -197,6 +205,36 @@ __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_
 }
 
 // ------------------------------------------------------------------------------------------------
+// Producer of one CTA tile (kTile requests) into buffer tile_idx & 1: in-register Philox draws
+// (a1-a3) or a copy of the materialised stream (a10). Shared by both simulation kernels.
+// ------------------------------------------------------------------------------------------------
+template <int CMAX>
+__device__ __forceinline__ void produce_tile(const KParams& prm, uint32_t cta_variant, uint32_t trial,
+                                             uint32_t variant, uint32_t tile_idx, uint4* tiles,
+                                             uint64_t* totals, uint32_t* cnt_s, int tid, int warp,
+                                             int lane) {
+  const uint32_t buf = tile_idx & 1u;
+  uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
+  const uint32_t n0 = tile_idx * kTile;
+  if (prm.stream == nullptr) {
+    for (int ch = warp; ch < kChunks; ch += kWarpsPerCta)
+      produce_chunk_philox<CMAX>(prm, n0 + ch * 32, trial, variant,
+                                 tb + ch * 32 * CompRec<CMAX>::kWords, totals + buf * kChunks + ch,
+                                 cnt_s, lane);
+  } else {
+    // a10: copy kTile 32-byte records (2 x uint4 each) from the materialised stream; cu is absolute
+    const uint4* src = prm.stream + ((size_t)(cta_variant * prm.K + trial) * prm.N + n0) * 2;
+    const uint32_t n_words = min((uint32_t)kTile, prm.N - n0) * 2u;
+    for (uint32_t w = tid; w < n_words; w += kThreads) {
+      const uint4 v = __ldg(src + w);
+      tb[w] = v;
+      if ((w & 1u) == 0u) atomicAdd(&cnt_s[v.y >> 24], 1u);
+    }
+    if (tid < kChunks) totals[buf * kChunks + tid] = 0;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Min-heap replace-min (a6). root = current minimum (register). Nodes 2..c live in shared memory as
 // sibling pairs: pair i = nodes (2i, 2i+1) at hb + (i-1)*512 (+ lane*16 folded into hb), fetched
 // with one LDS.128; if c is even, node c+1 holds +inf. Top-down sift of the new value x.
@@ -304,6 +342,21 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
       }
     }
   }
+  // Nothing to do for this CTA? (bisection: every plan's bracket has closed, rate 0; fixup pass:
+  // no simulation of this CTA left the 32-bit window)
+  bool wanted = warp_active && lane_live && !skip;
+  if (prm.fixup) wanted = wanted && prm.flags[(size_t)pr * prm.K + trial] != 0;
+  const bool write_out = prm.fixup ? wanted : (warp_active && lane_live);
+  if (!__syncthreads_or(wanted)) {
+    if (write_out) {  // all-skip CTA: the contract still wants zeros
+      const size_t slot = (size_t)pr * prm.K + trial;
+      for (uint32_t t = 0; t < 2 * prm.T; ++t) prm.out_counts[slot * prm.T * 2 + t] = 0u;
+      if (prm.out_dep_sum) prm.out_dep_sum[slot] = 0ull;
+      if (prm.out_makespan) prm.out_makespan[slot] = 0ll;
+      if (rate_bad) atomicMin(prm.status, -2);
+    }
+    return;
+  }
   uint32_t hits[8];
 #pragma unroll
   for (int t = 0; t < 8; ++t) hits[t] = 0;
@@ -315,25 +368,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   // ---- producer for one tile -----------------------------------------------------------------
   const uint32_t n_tiles = (prm.N + kTile - 1) / kTile;
   auto produce = [&](uint32_t tile_idx) {
-    const uint32_t buf = tile_idx & 1u;
-    uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
-    const uint32_t n0 = tile_idx * kTile;
-    if (prm.stream == nullptr) {
-      for (int ch = warp; ch < kChunks; ch += kWarpsPerCta)
-        produce_chunk_philox<CMAX>(prm, n0 + ch * 32, trial, variant,
-                                   tb + ch * 32 * CompRec<CMAX>::kWords, totals + buf * kChunks + ch,
-                                   cnt_s, lane);
-    } else {
-      // a10: copy kTile 32-byte records (2 x uint4 each) from the materialised stream; cu is absolute
-      const uint4* src = prm.stream + ((size_t)(cta.variant * prm.K + trial) * prm.N + n0) * 2;
-      const uint32_t n_words = min((uint32_t)kTile, prm.N - n0) * 2u;
-      for (uint32_t w = tid; w < n_words; w += kThreads) {
-        const uint4 v = __ldg(src + w);
-        tb[w] = v;
-        if ((w & 1u) == 0u) atomicAdd(&cnt_s[v.y >> 24], 1u);
-      }
-      if (tid < kChunks) totals[buf * kChunks + tid] = 0;
-    }
+    produce_tile<CMAX>(prm, cta.variant, trial, variant, tile_idx, tiles, totals, cnt_s, tid, warp, lane);
   };
 
   __syncthreads();
@@ -443,7 +478,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   }
 
   // ---- outputs ---------------------------------------------------------------------------------
-  if (warp_active && lane_live) {
+  if (write_out) {
     // DESIGN.md R17: the arrival horizon CU_N * period + 2^15 must stay below 2^62
     bool bad = rate_bad;
     if (!bad && !skip) {

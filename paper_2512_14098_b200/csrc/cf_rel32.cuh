@@ -1,0 +1,372 @@
+// cf_rel32.cuh -- the fast path of the simulation kernel (sm_100a). See DESIGN.md section 5.
+//
+// Same mapping as cf_device.cuh (one thread per simulation, CTA-shared request tiles, per-warp
+// stage records), re-coded so that the Kiefer-Wolfowitz heaps -- where the time goes -- work on
+// 32-bit keys:
+//
+//   * every time inside a tile of kTile requests is an offset from a per-lane TILE ORIGIN O = the
+//     system arrival of the last request of the previous tile. a3: A_n - O = (r0 + d_n*period) >> 16
+//     with d_n the tile-relative cumulative gap (u32) and r0 the low 16 bits of CU_prev*period + 2^15:
+//     one IMAD.WIDE and one funnel shift. The running departure x is a 64-bit offset (waits are
+//     unbounded under overload);
+//   * every stage of every lane has its own 64-bit STAGE BASE (an offset from O); the free times
+//     of its c replicas are 30-bit keys relative to that base: the root in the lane's state record,
+//     nodes 1..c-1 in a 4-ary min-heap of quads (16 B per lane, interleaved by lane: one
+//     conflict-free LDS.128 fetches all four children). A stored key is (key << 2) | slot, so the
+//     minimum of the four packed words is the minimum key AND names its slot: no index arithmetic;
+//   * the per-request record lists only the stages the request visits (stage ids + services), so a
+//     stage that is not visited costs nothing; per-lane stage state lives in shared memory;
+//   * a8: hit <=> x <= (A_n - O) + min(L_t, 2^31-1); per-type hit counters are byte fields of two
+//     32-bit words flushed once per tile.
+//
+// At every tile boundary the origin moves forward and every stage base moves to
+// max(earliest free time of the stage, new origin); keys below the new base are clamped to it.
+// Clamping at the origin is exact: every later request reaches every stage at or after its own
+// system arrival >= origin, so a replica that is free before the origin is simply "free"
+// (max(arrival, F) = arrival either way) -- DESIGN.md 5.2.
+//
+// A lane leaves the fast path when a key does not fit 30 bits (free times of ONE stage more than
+// 17.9 minutes apart), a tile spans >= 2^31 us or >= 2^32 gap units, the rate is outside [1, 1e9]
+// or the R17 horizon is exceeded. It then sets flags[slot] and writes nothing; the 64-bit kernel
+// of cf_device.cuh runs in fixup mode over exactly those simulations. Results are bit-identical.
+#pragma once
+#include "cf_device.cuh"
+
+namespace cfk {
+
+constexpr uint32_t kInf32 = 0xffffffffu;
+constexpr uint32_t kFull = 0xffffffffu;
+constexpr uint32_t kKeyLimit = (1u << 30) - 4u;  // keys must stay below this
+
+// Stage-level record of the fast kernel (a warp builds 32 of them per chunk for its topology):
+//   w0 = { d (tile-relative cumulative gap, Q16), min(L_t, 2^31-1), hit increment for types 0..3,
+//          hit increment for types 4..7 }   (one byte field per type; 0 if L_t < 0)
+//   w1 = { stage ids of visits 0..3 (one byte each, 0xff = end), of visits 4..7, S_0, S_1 }
+//   w2 = { S_2 .. S_5 },  w3 = { S_6, S_7, -, - }        (S_j = service of the j-th visit)
+template <int VMAX>
+struct StageRec32 {
+  static constexpr int kWords = VMAX <= 2 ? 2 : (VMAX <= 6 ? 3 : 4);
+};
+
+// Per-lane, per-stage state record (16 B): { base_lo, base_hi, root key, heap_row | nq << 16 }
+template <int VMAX, int CMAX>
+struct SmemLayout32 {
+  static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
+  static constexpr uint32_t kStageRecBytes = StageRec32<VMAX>::kWords * 16;
+  static constexpr uint32_t tiles = 0;
+  static constexpr uint32_t totals = tiles + 2 * kTile * kCompRecBytes;
+  static constexpr uint32_t cnt = totals + 2 * kChunks * 8;
+  static constexpr uint32_t l32 = cnt + 8 * 4;
+  static constexpr uint32_t inc = l32 + 8 * 4;  // 8 x {lo, hi}
+  static constexpr uint32_t wbuf = inc + 8 * 8;
+  static constexpr uint32_t state = wbuf + kWarpsPerCta * 32 * kStageRecBytes;  // [warp][stage][lane] x 16 B
+  static constexpr uint32_t heaps = state + kWarpsPerCta * VMAX * 512;
+  static constexpr uint32_t fixed_bytes = heaps;
+};
+
+__device__ __forceinline__ uint64_t mad_wide_u32(uint32_t a, uint32_t b, uint64_t c) {
+  uint64_t d;
+  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
+  return d;
+}
+
+// explicit shared-window accesses (32-bit shared addresses: no generic-address arithmetic)
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6: replace-min on a 4-ary min-heap of packed keys. The root key (node 0) is passed in/out in a
+// register; quad g holds the children 4g+1..4g+4 of node g at hb + g*512 (lane*16 folded into hb),
+// each stored as (key << 2) | slot; nodes >= c hold +inf. nq = heap_quads(c) >= 1.
+// Returns the new root key.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t heap4_replace_min(uint32_t hb, uint32_t nq512, uint32_t key) {
+  const uint32_t xk = key << 2;
+  uint4 q = lds128(hb);
+  uint32_t m = min(min(q.x, q.y), min(q.z, q.w));
+  if (xk <= m) return key;  // x <= every child
+  const uint32_t new_root = m >> 2;
+  uint32_t k = m & 3u;
+  uint32_t hole = hb + 4u * k;       // byte address of the hole; its slot is k
+  uint32_t rel = (k + 1u) << 9;      // 512 * node index of the hole = byte offset of its children quad
+  while (rel < nq512) {
+    const uint32_t qa = hb + rel;
+    q = lds128(qa);
+    m = min(min(q.x, q.y), min(q.z, q.w));
+    if (xk <= m) break;
+    sts32(hole, (m & ~3u) | k);      // the smallest child moves up into the hole (slot k)
+    k = m & 3u;
+    hole = qa + 4u * k;
+    rel = 4u * rel + ((k + 1u) << 9);
+  }
+  sts32(hole, xk | k);
+  return new_root;
+}
+
+// packed key p of slot k -> rebased by sh4 = shift << 2 (clamped at 0); +inf stays +inf
+__device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint32_t k) {
+  const uint32_t v = (max(p, sh4) - sh4) | k;
+  return p == kInf32 ? kInf32 : v;
+}
+
+template <int VMAX, int CMAX, bool HAS_DELAY>
+#ifndef CF_MINB32
+#define CF_MINB32 5
+#endif
+__global__ void __launch_bounds__(kThreads, CF_MINB32)
+cf_sim32_kernel(const __grid_constant__ KParams prm) {
+  using SL = SmemLayout32<VMAX, CMAX>;
+  constexpr int kW = StageRec32<VMAX>::kWords;
+  extern __shared__ __align__(16) uint8_t smem[];
+  const uint32_t smem_sa = (uint32_t)__cvta_generic_to_shared(smem);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t trial = prm.trial_base + blockIdx.x % prm.k_launch;
+  const CtaDesc cta = prm.ctas[blockIdx.x / prm.k_launch];
+  const uint32_t variant = prm.variant_lo + cta.variant;
+
+  uint4* tiles = reinterpret_cast<uint4*>(smem + SL::tiles);
+  uint64_t* totals = reinterpret_cast<uint64_t*>(smem + SL::totals);
+  uint32_t* cnt_s = reinterpret_cast<uint32_t*>(smem + SL::cnt);
+  uint32_t* l32_s = reinterpret_cast<uint32_t*>(smem + SL::l32);
+  uint2* inc_s = reinterpret_cast<uint2*>(smem + SL::inc);
+  uint4* wbuf = reinterpret_cast<uint4*>(smem + SL::wbuf) + warp * 32 * kW;
+  // shared addresses of this lane's state records (stage s at + s*512) and of its heap column
+  const uint32_t st_sa = smem_sa + SL::state + (uint32_t)warp * VMAX * 512u + (uint32_t)lane * 16u;
+
+  if (tid < 8) {
+    cnt_s[tid] = 0;
+    const int64_t L = prm.L_us[tid];
+    l32_s[tid] = (uint32_t)(L < 0 ? 0 : (L > 0x7fffffffll ? 0x7fffffffll : L));
+    const uint32_t one = (L < 0) ? 0u : (1u << (8 * (tid & 3)));  // L < 0: never a hit
+    inc_s[tid] = make_uint2(tid < 4 ? one : 0u, tid < 4 ? 0u : one);
+  }
+
+  // ---- per-lane simulation setup -------------------------------------------------------------
+  const bool warp_active = warp < (int)cta.n_warps;
+  WarpDesc wd;
+  wd.heap_off32 = 0; wd.heap_rows32 = 0; wd.topo = 0;
+  uint32_t period = 1, pr = 0, plan = 0, n_stages = 0;
+  bool lane_live = false, skip = false, flagged = false;
+  if (warp_active) {
+    wd = prm.warps[cta.warp_begin + warp];
+    n_stages = prm.topos[wd.topo].n_stages;
+    lane_live = lane < (int)wd.n_lanes;
+    const SimDesc sd = prm.sims[wd.sim_begin + (lane_live ? lane : 0)];  // idle lanes mirror lane 0
+    pr = sd.pr;
+    plan = sd.plan;
+    const uint32_t rate = prm.rates[pr];
+    if (rate < 1u || rate > 1000000000u) {
+      if (prm.bisect_mode && rate == 0u) skip = true; else flagged = true;  // bad rate: the 64-bit kernel reports it
+    } else {
+      period = (1000000000u + rate / 2u) / rate;
+    }
+  }
+  const bool wanted = warp_active && lane_live && !skip;
+  const size_t slot = (size_t)pr * prm.K + trial;
+  if (!__syncthreads_or(wanted)) {  // bisection: every bracket of this CTA has closed
+    if (warp_active && lane_live) {
+      for (uint32_t t = 0; t < 2 * prm.T; ++t) prm.out_counts[slot * prm.T * 2 + t] = 0u;
+      if (prm.out_dep_sum) prm.out_dep_sum[slot] = 0ull;
+      if (prm.out_makespan) prm.out_makespan[slot] = 0ll;
+      prm.flags[slot] = 0;
+    }
+    return;
+  }
+  const uint32_t heap_sa = smem_sa + SL::heaps + wd.heap_off32 + (uint32_t)lane * 16u;
+  if (warp_active) {
+    // all replicas free at time 0: every key 0 (packed with its slot), +inf beyond node c-1
+    for (uint32_t j = 0; j < wd.heap_rows32; ++j) sts128(heap_sa + j * 512u, make_uint4(0u, 1u, 2u, 3u));
+    uint32_t row = 0;  // this lane's stages are laid out one after another
+    for (uint32_t s = 0; s < (uint32_t)VMAX; ++s) {
+      uint32_t nq = 0;
+      if (s < n_stages) {
+        const uint32_t c = prm.plan_c[plan * 8 + s];
+        nq = heap_quads(c);
+        if (nq) {
+          const uint32_t j = nq - 1u;  // only the last quad can hold nodes >= c
+          uint32_t v[4];
+#pragma unroll
+          for (uint32_t e = 0; e < 4; ++e) v[e] = (4u * j + 1u + e >= c) ? kInf32 : e;
+          sts128(heap_sa + (row + j) * 512u, make_uint4(v[0], v[1], v[2], v[3]));
+        }
+      }
+      sts128(st_sa + s * 512u, make_uint4(0u, 0u, 0u, row | (nq << 16)));
+      row += nq;
+    }
+  }
+  TopoDesc topo;
+  if (warp_active) topo = prm.topos[wd.topo];
+  uint32_t hits[8];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) hits[t] = 0;
+  uint64_t dep_sum = 0, cu_base = 0, tile_base = 0, last_cu = 0;
+  uint64_t origin = 0;  // O: absolute time of offset 0 (microseconds)
+  uint64_t makespan = 0;
+  const uint64_t delay = (uint64_t)prm.edge_delay;
+
+  const uint32_t n_tiles = (prm.N + kTile - 1) / kTile;
+  __syncthreads();
+  produce_tile<CMAX>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
+  __syncthreads();
+
+  for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
+    if (tile_idx + 1 < n_tiles)
+      produce_tile<CMAX>(prm, cta.variant, trial, variant, tile_idx + 1, tiles, totals, cnt_s, tid, warp, lane);
+    if (warp_active) {
+      const uint32_t buf = tile_idx & 1u;
+      const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
+      const uint32_t n0 = tile_idx * kTile;
+      // ---- tile prologue: move the origin to the arrival of the last request before the tile,
+      //      every stage base to max(earliest free time, origin), and re-key the stage's heap
+      const uint64_t acc0 = tile_base * (uint64_t)period + 32768ull;  // wraps only if R17 fails later
+      const uint32_t r0 = (uint32_t)acc0 & 0xffffu;
+      if (tile_idx != 0) {
+        const uint64_t o_new = acc0 >> 16;
+        const uint64_t delta = o_new - origin;
+        origin = o_new;
+        for (uint32_t s = 0; s < n_stages; ++s) {
+          const uint32_t sa = st_sa + s * 512u;
+          const uint4 st = lds128(sa);
+          const uint64_t base = ((uint64_t)st.y << 32) | st.x;
+          const uint64_t fmin = base + st.z;
+          const uint64_t nb = fmin > delta ? fmin : delta;  // new base, still relative to the old origin
+          const uint64_t shift = nb - base;                 // >= root key: the new root key is 0
+          const uint64_t nbr = nb - delta;                  // ... relative to the new origin
+          sts128(sa, make_uint4((uint32_t)nbr, (uint32_t)(nbr >> 32), 0u, st.w));
+          const uint32_t sh4 = shift >= (1ull << 30) ? 0xfffffffcu : ((uint32_t)shift << 2);
+          const uint32_t nq = st.w >> 16, ha = heap_sa + (st.w & 0xffffu) * 512u;
+          if (sh4 != 0u)
+            for (uint32_t j = 0; j < nq; ++j) {
+              uint4 q = lds128(ha + j * 512u);
+              q.x = rebase_packed(q.x, sh4, 0u); q.y = rebase_packed(q.y, sh4, 1u);
+              q.z = rebase_packed(q.z, sh4, 2u); q.w = rebase_packed(q.w, sh4, 3u);
+              sts128(ha + j * 512u, q);
+            }
+        }
+      }
+      uint32_t hlo = 0, hhi = 0;
+      uint64_t dep = 0, mk = 0;
+#pragma unroll 1
+      for (int ch = 0; ch < kChunks; ++ch) {
+        const uint32_t nc0 = n0 + ch * 32;
+        if (nc0 >= prm.N) break;
+        const int n_here = (int)min(32u, prm.N - nc0);
+        // ---- a4: component-level record -> list of visited stages for this warp's topology ----
+        {
+          const uint4* src = tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
+          const uint4 w0 = src[0], w1 = src[1];
+          int32_t svc[8];
+          svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x;
+          svc[3] = (int32_t)w1.y; svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w;
+          svc[6] = 0; svc[7] = 0;
+          if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
+          const uint32_t t = w0.y >> 24;
+          const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;  // absolute
+          const uint64_t d64 = cu - tile_base;
+          if (__any_sync(kFull, lane < n_here && (d64 >> 32) != 0)) flagged = true;  // tile too long
+          last_cu = __shfl_sync(kFull, cu, n_here - 1);
+          const uint32_t tm = prm.type_mask[t];
+          const uint2 inc = inc_s[t];
+          uint8_t* dst = reinterpret_cast<uint8_t*>(wbuf + lane * kW);
+          *reinterpret_cast<uint4*>(dst) = make_uint4((uint32_t)d64, l32_s[t], inc.x, inc.y);
+          *reinterpret_cast<uint2*>(dst + 16) = make_uint2(0xffffffffu, 0xffffffffu);  // no visits yet
+          uint32_t nv = 0;
+#pragma unroll
+          for (int s = 0; s < VMAX; ++s) {
+            const uint32_t sm = (s < (int)n_stages) ? topo.mask[s] : 0u;
+            if (sm & tm) {
+              int32_t acc = 0;
+#pragma unroll
+              for (int i = 0; i < CMAX; ++i) acc += ((sm >> i) & 1u) ? svc[i] : 0;
+              dst[16 + nv] = (uint8_t)s;
+              *reinterpret_cast<int32_t*>(dst + 24 + 4 * nv) = acc;
+              ++nv;
+            }
+          }
+        }
+        __syncwarp();
+        // ---- the per-request loop: every lane runs its own simulation over the same 32 requests
+#pragma unroll 1
+        for (int r = 0; r < n_here; ++r) {
+          const uint4* rp = wbuf + r * kW;
+          const uint4 w0 = rp[0], w1 = rp[1];
+          uint4 w2 = make_uint4(0, 0, 0, 0), w3 = make_uint4(0, 0, 0, 0);
+          if (kW > 2) w2 = rp[2];
+          if (kW > 3) w3 = rp[3];
+          // a3: A - O = (r0 + d * period) >> 16
+          const uint32_t a = (uint32_t)(mad_wide_u32(w0.x, period, (uint64_t)r0) >> 16);
+          uint64_t x = a;
+#pragma unroll
+          for (int j = 0; j < VMAX; ++j) {
+            const uint32_t sid = ((j < 4 ? w1.x : w1.y) >> (8 * (j & 3))) & 0xffu;
+            if (sid == 0xffu) break;  // warp-uniform: all lanes see the same request
+            const uint32_t S = j == 0 ? w1.z : j == 1 ? w1.w : j == 2 ? w2.x : j == 3 ? w2.y
+                             : j == 4 ? w2.z : j == 5 ? w2.w : j == 6 ? w3.x : w3.y;
+            const uint32_t sa = st_sa + sid * 512u;
+            const uint4 st = lds128(sa);
+            const uint64_t base = ((uint64_t)st.y << 32) | st.x;
+            const uint64_t f = base + st.z;  // earliest free time of the stage
+            if (HAS_DELAY && j > 0) x += delay;
+            x = (x > f ? x : f) + S;         // a5/a6: start at max(arrival, earliest free)
+            const uint64_t key64 = x - base;
+            if (key64 >= (uint64_t)kKeyLimit) flagged = true;
+            uint32_t key = (uint32_t)key64;
+            if (st.w >> 16) key = heap4_replace_min(heap_sa + (st.w & 0xffffu) * 512u, (st.w >> 16) << 9, key);
+            sts32(sa + 8u, key);
+          }
+          // a8
+          if (x <= (uint64_t)a + w0.y) { hlo += w0.z; hhi += w0.w; }
+          dep += x;
+          mk = x > mk ? x : mk;
+        }
+        __syncwarp();
+        cu_base += totals[buf * kChunks + ch];
+      }
+      // ---- tile epilogue: absolute outputs, window checks
+      const uint32_t n_in_tile = min((uint32_t)kTile, prm.N - n0);
+      dep_sum += dep + (uint64_t)n_in_tile * origin;
+      makespan = max(makespan, origin + mk);
+      if (mad_wide_u32((uint32_t)(last_cu - tile_base), period, (uint64_t)r0) >> 47) flagged = true;
+      tile_base = last_cu;
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        hits[t] += (hlo >> (8 * t)) & 0xffu;
+        hits[t + 4] += (hhi >> (8 * t)) & 0xffu;
+      }
+    }
+    __syncthreads();
+  }
+
+  // ---- outputs ---------------------------------------------------------------------------------
+  if (warp_active && lane_live) {
+    if (!skip && !flagged) {  // DESIGN.md R17: the 64-bit kernel zeroes the outputs and raises the status
+      const uint64_t hi = __umul64hi(last_cu, (uint64_t)period);
+      const uint64_t lo = last_cu * (uint64_t)period;
+      if (hi != 0 || lo >= (1ull << 62) - 32768ull) flagged = true;
+    }
+    const bool redo = flagged && !skip;
+    prm.flags[slot] = redo ? 1 : 0;
+    if (redo) {
+      atomicAdd(reinterpret_cast<uint32_t*>(prm.status) + 1, 1u);
+    } else {
+      uint32_t* oc = prm.out_counts + slot * prm.T * 2;
+      for (uint32_t t = 0; t < prm.T; ++t) {
+        oc[2 * t + 0] = skip ? 0u : cnt_s[t];
+        oc[2 * t + 1] = skip ? 0u : hits[t];
+      }
+      if (prm.out_dep_sum) prm.out_dep_sum[slot] = skip ? 0ull : dep_sum;
+      if (prm.out_makespan) prm.out_makespan[slot] = skip ? 0ll : (int64_t)makespan;
+    }
+  }
+}
+
+}  // namespace cfk

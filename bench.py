@@ -59,12 +59,6 @@ def workload_name(cfg: int) -> str:
             "cfg4 coarse-to-fine sweep, 4096 plans x 32-step bisection x 8 trials x 2^18 req, stream in HBM"][cfg]
 
 
-def expected_heap_levels(w) -> float:
-    """Upper bound of heap levels per update used by the algorithmic op model: floor(log2 c) of the
-    stage, weighted by how often each stage is visited (exact visit counts come from out_counts)."""
-    return 0.0
-
-
 class ClockSampler:
     """nvidia-smi clocks/throttle reasons during the timed region (B200_PROFILING.md recipe)."""
 
@@ -302,25 +296,36 @@ def main():
 
     # ---- exact update count of one step (outside the timed region)
     updates = 0
+    heap_levels = 0
+    requests = 0
+    wide = 0
     h2d = d2h = 0
     for c in calls:
         w = c["w"]
+        wide += cf.cf_workspace_wide_count(c["ws"])
         if w.rate_mrps is not None:
-            updates += W.count_updates(w.graph, w.plans, cf.to_numpy_u32(c["counts"]))
+            cnts = cf.to_numpy_u32(c["counts"])
+            updates += W.count_updates(w.graph, w.plans, cnts)
+            heap_levels += W.count_heap_levels(w.graph, w.plans, cnts)
+            requests += int(np.prod(w.rate_mrps.shape)) * w.graph.n_trials * w.graph.n_req
             h2d += c["rates_host"].numel() * 4
             d2h += c["h_counts"].numel() * 4 + c["h_dep"].numel() * 8 + c["h_mk"].numel() * 8
         else:
-            # every bisection step that was not a no-op simulated P*K sims; count visits exactly from
-            # the type counts (identical for every rate, R4) x steps actually run per plan
-            counts = cf.to_numpy_u32(c["bisect"]["counts"])  # [P,K,T,2] at rate*
-            # plans whose bracket closed early run fewer probes; bound by the step count
+            # bisection: only the probes ON the bisection path count (the library reports how many
+            # each plan had; closed brackets are no-ops, speculative tree nodes are overhead). The
+            # type counts of a (variant, trial) do not depend on the rate (common random numbers,
+            # R4), so one probe of plan p does count_updates(type counts of its stream) updates.
             P = w.plans.n_plans
-            probes = np.full(P, w.n_steps, dtype=np.int64)
-            hi = w.rate_hi_mrps.astype(np.int64)
-            probes = np.minimum(probes, np.ceil(np.log2(np.maximum(hi, 2))).astype(np.int64))
-            ref = W.count_updates(w.graph, w.plans, np.broadcast_to(
-                counts.max(axis=0, keepdims=True), counts.shape)[:, None])  # one probe of every plan
-            updates += int(ref * float(probes.mean()))
+            probes = cf.cf_bisect_probes(c["ws"], P).astype(np.int64)
+            ones = np.ones((P, 1), dtype=np.uint32)
+            c1 = cf.cf_eval_plans(w.graph, w.plans, np.maximum(w.rate_hi_mrps.reshape(P, 1) // 4, 1) * ones, w.slo,
+                                  w.seed, stream_records=c["stream_records"], n_variants=w.n_variants,
+                                  plan_variant=w.plan_variant, aux=False)
+            cnts = cf.to_numpy_u32(c1["counts"])  # [P,1,K,T,2]
+            updates += int((probes * W.count_updates(w.graph, w.plans, cnts, per_plan=True)).sum())
+            heap_levels += int((probes * W.count_heap_levels(w.graph, w.plans, cnts, per_plan=True)).sum())
+            requests += int(probes.sum()) * w.graph.n_trials * w.graph.n_req
+            c["probes_total"] = int(probes.sum())
             h2d += c["hi_host"].numel() * 4
             d2h += P * 4 + P * w.graph.n_types * 4
 
@@ -346,16 +351,32 @@ def main():
         sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
         sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         peak_tops = sm_count * 4 * 32 * sm_mhz * 1e6 / 1e12  # 4 schedulers x 32 lanes x 1 inst/clk
-        requests = sum(int(np.prod(c["w"].rate_mrps.shape)) * c["w"].graph.n_trials * c["w"].graph.n_req
-                       for c in calls if c["w"].rate_mrps is not None)
-        alg_ops = OPS_PER_REQUEST * requests + OPS_PER_UPDATE * updates
-        achieved = alg_ops * args.steps / (dev_ms / 1000.0) / 1e12
-        roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tops, "unit": "Tlane-op/s",
-                    "frac": achieved / peak_tops, "traffic": None,
-                    "peak_source": f"derived: {sm_count} SMs x 4 schedulers x 32 lanes x {sm_mhz:.0f} MHz",
-                    "measured_int32_peaks_tops": peaks,
-                    "ops_model": {"per_request": OPS_PER_REQUEST, "per_update": OPS_PER_UPDATE,
-                                  "heap_levels": "not counted (lower bound)"}}
+        step_s = dev_ms / 1000.0 / args.steps
+        alg_ops = OPS_PER_REQUEST * requests + OPS_PER_UPDATE * updates + OPS_PER_HEAP_LEVEL * heap_levels
+        achieved = alg_ops / step_s / 1e12
+        alu = {"bound": "alu", "achieved": achieved, "peak": peak_tops, "unit": "Tlane-op/s",
+               "frac": achieved / peak_tops, "traffic": None,
+               "peak_source": f"derived: {sm_count} SMs x 4 schedulers x 32 lanes x {sm_mhz:.0f} MHz",
+               "measured_int32_peaks_tops": peaks,
+               "ops_model": {"per_request": OPS_PER_REQUEST, "per_update": OPS_PER_UPDATE,
+                             "per_heap_level": OPS_PER_HEAP_LEVEL, "requests": requests, "updates": updates,
+                             "heap_levels": heap_levels}}
+        if args.config == 4:
+            # materialised variant: algorithmic bytes = one 32-byte record per request per simulation
+            # on the bisection path; peak = measured HBM copy bandwidth
+            try:
+                peak_gbs = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+                peak_src = "MEASURED_PEAKS.json hbm_gbs (measured)"
+            except (OSError, KeyError, ValueError):
+                peak_gbs, peak_src = 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+            gbs = 32.0 * requests / step_s / 1e9
+            roofline = {"bound": "hbm", "achieved": gbs, "peak": peak_gbs, "unit": "GB/s", "frac": gbs / peak_gbs,
+                        "traffic": None, "peak_source": peak_src,
+                        "note": "a thread block reads each record once for all its simulations, so DRAM traffic "
+                                "is far below the algorithmic bytes; the kernel is latency/ALU-bound: see alu",
+                        "alu": alu}
+        else:
+            roofline = alu
         cpu = None
         if not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
@@ -366,6 +387,7 @@ def main():
                 "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
                 "config": {"workload": workload_name(args.config), "scale": args.scale,
                            "updates_per_step": total_updates, "l2": "flushed between timed steps (256 MiB fill)",
+                           "wide_fixups": wide, "bisect_probes": sum(c.get("probes_total", 0) for c in calls),
                            "parallelism": f"replicas x{world} (one Philox variant per rank)"},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},

@@ -168,6 +168,18 @@ uint32_t cf_last_launch_count(void);
 int64_t cf_workspace_wide_count(const void* workspace, void* stream);
 int32_t cf_debug_kernel_mode(uint32_t mode);
 
+/* cf_goodput_bisect[_stream] simulate, in one pass, the complete decision tree of the next `depth`
+ * bisection steps of every plan (2^depth - 1 candidate rates) and then walk the path the sequential
+ * algorithm takes: identical results, `depth` times fewer passes, more simulations in flight.
+ * depth = 0 (default): chosen from P*K so that a pass fills the GPU; 1..4: fixed (tests, tuning).
+ * Applies to later calls made by the calling host thread. */
+int32_t cf_debug_bisect_depth(uint32_t depth);
+
+/* Bench bookkeeping: synchronises `stream` and copies to out_probes (host, [n_plans]) how many
+ * probes (simulated rates) lay on the bisection path of each plan in the last cf_goodput_bisect*
+ * call on `workspace` (steps whose bracket had already closed are no-ops and do not count). */
+int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_probes, void* stream);
+
 /* Micro-benchmark used by bench.py for the ALU roofline denominator: runs `iters` rounds of an
  * unrolled, independent 32-bit integer instruction mix on every SM and writes the number of
  * lane-operations executed to *out_ops (host). mix: 0 = IADD3/LOP3 only (ALU pipe), 1 = IMAD only

@@ -23,7 +23,7 @@ EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_strea
            "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status",
            "cf_last_launch_count", "cf_bench_int32_peak", "cf_strerror", "cf_workspace_wide_count",
-           "cf_debug_kernel_mode"]
+           "cf_debug_kernel_mode", "cf_debug_bisect_depth", "cf_bisect_probes"]
 
 
 class CfError(RuntimeError):
@@ -67,6 +67,8 @@ _lib.cf_strerror.restype = C.c_char_p
 _lib.cf_last_launch_count.restype = C.c_uint32
 _lib.cf_workspace_wide_count.restype = C.c_int64
 _lib.cf_debug_kernel_mode.restype = C.c_int32
+_lib.cf_debug_bisect_depth.restype = C.c_int32
+_lib.cf_bisect_probes.restype = C.c_int32
 for _n in ("cf_eval_plans", "cf_goodput_bisect", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak"):
     getattr(_lib, _n).restype = C.c_int32
@@ -161,6 +163,22 @@ def cf_debug_kernel_mode(mode: int) -> None:
     rc = int(_lib.cf_debug_kernel_mode(C.c_uint32(mode)))
     if rc != CF_OK:
         raise CfError(rc, "cf_debug_kernel_mode")
+
+
+def cf_bisect_probes(workspace: torch.Tensor, n_plans: int, stream=None) -> np.ndarray:
+    """Probes on the bisection path of each plan in the last cf_goodput_bisect call on `workspace`."""
+    out = np.zeros(n_plans, dtype=np.uint32)
+    rc = int(_lib.cf_bisect_probes(_dp(workspace), C.c_uint32(n_plans), _hp(out, C.c_uint32), _stream_ptr(stream)))
+    if rc != CF_OK:
+        raise CfError(rc, "cf_bisect_probes")
+    return out
+
+
+def cf_debug_bisect_depth(depth: int) -> None:
+    """Bisection steps simulated per pass: 0 = automatic, 1..4 = fixed (tests, tuning)."""
+    rc = int(_lib.cf_debug_bisect_depth(C.c_uint32(depth)))
+    if rc != CF_OK:
+        raise CfError(rc, "cf_debug_bisect_depth")
 
 
 def cf_last_launch_count() -> int:

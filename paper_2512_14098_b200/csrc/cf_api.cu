@@ -20,6 +20,8 @@ namespace {
 
 thread_local uint32_t g_launch_count = 0;
 thread_local uint32_t g_kernel_mode = 0;  // cf_debug_kernel_mode: 0 auto, 1 = 64-bit kernel only
+thread_local uint32_t g_rate_major = 0;   // bisection lane order (probe knob, see build_schedule)
+thread_local uint32_t g_spec_depth = 0;   // cf_debug_bisect_depth: 0 auto, 1..4 = bisection steps per pass
 
 constexpr size_t kAlign = 256;
 constexpr uint32_t kMaxSmem = 227u * 1024u;
@@ -155,7 +157,7 @@ int kernel_regs32(int vmax, int cmax);
 // the same warps and blocks with its own, larger heap offsets.
 int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
                        const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
-                       bool fast, Schedule* out) {
+                       bool fast, bool rate_major, Schedule* out) {
   const uint32_t P = pl->n_plans, MS = pl->max_stages;
   Schedule& sc = *out;
   sc.plan_c.assign((size_t)P * 8, 1);
@@ -219,8 +221,16 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
            plan_topo[order[j]] == plan_topo[order[i]])
       ++j;
     const size_t sim0 = sc.sims.size();
-    for (size_t q = i; q < j; ++q)
-      for (uint32_t r = 0; r < R; ++r) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
+    // plan-major: the R rates of a plan share replica counts (uniform heap depths in a warp);
+    // rate-major (bisection): the same tree node of many plans, so that the simulations that
+    // leave the fast window (the overloaded nodes) cluster in few warps
+    if (rate_major) {
+      for (uint32_t r = 0; r < R; ++r)
+        for (size_t q = i; q < j; ++q) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
+    } else {
+      for (size_t q = i; q < j; ++q)
+        for (uint32_t r = 0; r < R; ++r) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
+    }
     const size_t n_group = sc.sims.size() - sim0;
     const TopoDesc& td = sc.topos[plan_topo[order[i]]];
     for (size_t w0 = 0; w0 < n_group; w0 += 32) {
@@ -527,33 +537,68 @@ int32_t check_workspace(void* ws, size_t have, size_t need) {
 // ------------------------------------------------------------------------------------------------
 // bisection kernels (a9): all bracket state lives in the workspace, no host round trips
 // ------------------------------------------------------------------------------------------------
+// Speculative bisection: one pass simulates, for every plan, the complete decision tree of the next
+// `depth` bisection steps (2^depth - 1 candidate rates, heap order: node i has children 2i [probe i
+// infeasible: hi = rate_i] and 2i+1 [feasible: lo = rate_i]); the update kernel then walks the path
+// the sequential algorithm would have taken. Every probe on that path is exactly the probe of the
+// sequential bisection, so results are identical; the other nodes only buy parallelism.
+constexpr uint32_t kMaxSpecDepth = 4;
+constexpr uint32_t kMaxSpecNodes = (1u << kMaxSpecDepth) - 1u;
+
 struct BisectState {
-  uint32_t* lo; uint32_t* hi; uint32_t* mid;  // [P]; mid == 0 <=> this step is a no-op for the plan
-  uint32_t* probe;                            // [P][K][T][2] counts of the current probe
-  uint32_t* at_lo;                            // [P][K][T][2] counts remembered for lo
+  uint32_t* lo; uint32_t* hi;  // [P]
+  uint32_t* tree;              // [P][R] rates of the decision tree; 0 = no-op node (mid == lo, or too deep)
+  uint32_t* probe;             // [P][R][K][T][2] counts of the current pass
+  uint32_t* at_lo;             // [P][K][T][2] counts remembered for lo
+  uint32_t* n_probes;          // [P] probes on the bisection path so far (bench bookkeeping)
+  uint32_t R;                  // nodes per plan = 2^depth - 1
 };
 
-__global__ void bisect_init_kernel(BisectState bs, const uint32_t* rate_hi, uint32_t P, uint32_t per_plan) {
+// tree of the next `levels` steps for bracket [lo, hi)
+__device__ void bisect_build_tree(uint32_t* tree, uint32_t R, uint32_t lo, uint32_t hi, uint32_t levels) {
+  uint32_t nlo[kMaxSpecNodes + 1], nhi[kMaxSpecNodes + 1];
+  nlo[1] = lo; nhi[1] = hi;
+  for (uint32_t i = 1; i <= R; ++i) {
+    uint32_t level = 0;
+    for (uint32_t j = i; j; j >>= 1) ++level;  // node i sits on level floor(log2 i) + 1
+    const uint32_t l = nlo[i], h = nhi[i];
+    const uint32_t mid = l + (h - l) / 2;
+    const bool noop = level > levels || h < l || mid == l;  // h < l marks a dead subtree
+    tree[i - 1] = noop ? 0u : mid;
+    if (2 * i + 1 <= R) {
+      nlo[2 * i] = noop ? 1u : l;   nhi[2 * i] = noop ? 0u : mid;
+      nlo[2 * i + 1] = noop ? 1u : mid; nhi[2 * i + 1] = noop ? 0u : h;
+    }
+  }
+}
+
+__global__ void bisect_init_kernel(BisectState bs, const uint32_t* rate_hi, uint32_t P, uint32_t per_plan,
+                                   uint32_t levels) {
   const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
   const uint32_t lo = 0, hi = rate_hi[p];
-  const uint32_t mid = lo + (hi - lo) / 2;
   bs.lo[p] = lo;
   bs.hi[p] = hi;
-  bs.mid[p] = (mid == lo) ? 0u : mid;
+  bs.n_probes[p] = 0;
   for (uint32_t i = 0; i < per_plan; ++i) bs.at_lo[(size_t)p * per_plan + i] = 0;
+  bisect_build_tree(bs.tree + (size_t)p * bs.R, bs.R, lo, hi, levels);
 }
 
-// one thread per plan: pool the probe counts over trials, test feasibility, move the bracket
+// one thread per plan: walk `levels` steps through the simulated tree (pool the probe counts over
+// trials, test feasibility, move the bracket), then lay out the tree of the next pass
 __global__ void bisect_update_kernel(BisectState bs, uint32_t P, uint32_t K, uint32_t T,
                                      const uint32_t* att_num, const uint32_t* att_den,
-                                     int32_t* status) {
+                                     uint32_t levels, uint32_t next_levels) {
   const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
   uint32_t lo = bs.lo[p], hi = bs.hi[p];
-  const uint32_t mid = bs.mid[p];
-  if (mid != 0) {
-    const uint32_t* pc = bs.probe + (size_t)p * K * T * 2;
+  const uint32_t* tree = bs.tree + (size_t)p * bs.R;
+  uint32_t node = 1;
+  for (uint32_t step = 0; step < levels; ++step) {
+    const uint32_t mid = tree[node - 1];
+    if (mid == 0) break;  // no-op step: the bracket has closed, every later step is a no-op too
+    ++bs.n_probes[p];
+    const uint32_t* pc = bs.probe + ((size_t)p * bs.R + (node - 1)) * K * T * 2;
     bool feasible = true;
     for (uint32_t k = 0; k < K; ++k) {  // DESIGN.md R18: an out-of-range probe (zeroed) is infeasible
       uint64_t n = 0;
@@ -569,14 +614,15 @@ __global__ void bisect_update_kernel(BisectState bs, uint32_t P, uint32_t K, uin
       lo = mid;
       uint32_t* al = bs.at_lo + (size_t)p * K * T * 2;
       for (uint32_t i = 0; i < K * T * 2; ++i) al[i] = pc[i];
+      node = 2 * node + 1;
     } else {
       hi = mid;
+      node = 2 * node;
     }
-    bs.lo[p] = lo;
-    bs.hi[p] = hi;
   }
-  const uint32_t nm = lo + (hi - lo) / 2;
-  bs.mid[p] = (nm == lo) ? 0u : nm;
+  bs.lo[p] = lo;
+  bs.hi[p] = hi;
+  bisect_build_tree(bs.tree + (size_t)p * bs.R, bs.R, lo, hi, next_levels);
 }
 
 __global__ void bisect_final_kernel(BisectState bs, uint32_t P, uint32_t K, uint32_t T, uint32_t N,
@@ -712,7 +758,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   const bool fast = fast_path_ok(a.g);
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, false, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);  // status block
@@ -752,23 +798,34 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
   const bool fast = fast_path_ok(a.g);
+  // speculation depth: enough simulations per pass to fill the GPU (one thread each), no more
+  uint32_t depth = g_spec_depth;
+  if (depth == 0) {
+    depth = 1;
+    while (depth < kMaxSpecDepth && (uint64_t)P * K * ((1u << depth) - 1u) < 90000ull) ++depth;
+  }
+  depth = std::min(depth, std::max(1u, a.n_steps));
+  const uint32_t R = (1u << depth) - 1u;
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, 1, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast,
+                                  g_rate_major != 0, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);
+  const size_t np_off = blob.reserve((size_t)P * 4);  // == kAlign: cf_bisect_probes reads it there
   KParams kp;
   const size_t pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &kp);
   const SchedOffsets so = add_schedule(sc, &blob);
   const size_t att_off = blob.add(a.slo->att_num, T * 4);
   const size_t den_off = blob.add(a.slo->att_den, T * 4);
   const size_t per_plan = (size_t)K * T * 2;
-  const size_t lo_off = blob.reserve((size_t)P * 4), hi_off = blob.reserve((size_t)P * 4),
-               mid_off = blob.reserve((size_t)P * 4);
   const size_t blob_bytes = blob.bytes.size();
-  const size_t probe_off = align_up(blob_bytes), at_lo_off = align_up(probe_off + P * per_plan * 4);
+  const size_t lo_off = align_up(blob_bytes), hi_off = align_up(lo_off + (size_t)P * 4);
+  const size_t tree_off = align_up(hi_off + (size_t)P * 4);
+  const size_t probe_off = align_up(tree_off + (size_t)P * R * 4);
+  const size_t at_lo_off = align_up(probe_off + P * R * per_plan * 4);
   const size_t flags_off = align_up(at_lo_off + P * per_plan * 4);
-  if (flags_off + (size_t)P * K > a.ws_bytes) return CF_ERR_WORKSPACE;
+  if (flags_off + (size_t)P * R * K > a.ws_bytes) return CF_ERR_WORKSPACE;
   uint8_t* ws = static_cast<uint8_t*>(a.ws);
   if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob_bytes, cudaMemcpyHostToDevice, a.st)))
     return rc;
@@ -776,22 +833,26 @@ int32_t bisect_impl(const BisectArgs& a) {
   BisectState bs;
   bs.lo = reinterpret_cast<uint32_t*>(ws + lo_off);
   bs.hi = reinterpret_cast<uint32_t*>(ws + hi_off);
-  bs.mid = reinterpret_cast<uint32_t*>(ws + mid_off);
+  bs.tree = reinterpret_cast<uint32_t*>(ws + tree_off);
   bs.probe = reinterpret_cast<uint32_t*>(ws + probe_off);
   bs.at_lo = reinterpret_cast<uint32_t*>(ws + at_lo_off);
+  bs.n_probes = reinterpret_cast<uint32_t*>(ws + np_off);
+  bs.R = R;
   kp.stream = static_cast<const uint4*>(a.stream_records);
   kp.variant_lo = a.stream_records ? 0 : a.variant;
   kp.bisect_mode = 1;
-  kp.rates = bs.mid;
+  kp.rates = bs.tree;
   kp.out_counts = bs.probe;
   kp.flags = ws + flags_off;
   const uint32_t nb = (P + 127) / 128;
-  bisect_init_kernel<<<nb, 128, 0, a.st>>>(bs, a.rate_hi_dev, P, (uint32_t)per_plan);
+  bisect_init_kernel<<<nb, 128, 0, a.st>>>(bs, a.rate_hi_dev, P, (uint32_t)per_plan, std::min(depth, a.n_steps));
   ++g_launch_count;
-  for (uint32_t step = 0; step < a.n_steps; ++step) {
+  for (uint32_t step = 0; step < a.n_steps; step += depth) {
+    const uint32_t levels = std::min(depth, a.n_steps - step);
+    const uint32_t next_levels = std::min(depth, a.n_steps - step - levels);
     if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, fast, a.st))) return rc;
     bisect_update_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, reinterpret_cast<const uint32_t*>(ws + att_off),
-                                               reinterpret_cast<const uint32_t*>(ws + den_off), kp.status);
+                                               reinterpret_cast<const uint32_t*>(ws + den_off), levels, next_levels);
     ++g_launch_count;
   }
   bisect_final_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, a.g->n_req, a.out_rate, a.out_goodput, a.out_counts);
@@ -810,6 +871,8 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   if (!g || !pl || !g->tabs) return 0;
   const size_t P = pl->n_plans, K = g->n_trials, T = g->n_types;
   if (R < 1) R = 1;
+  const size_t Rb = kMaxSpecNodes;                          // bisection: rates per plan and pass
+  R = std::max<size_t>(R, Rb);
   size_t n = kAlign;                                        // status
   n += align_up(pool_entries(g) * 4);
   n += align_up(P * sizeof(TopoDesc));
@@ -818,8 +881,8 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   n += align_up(max_warps * sizeof(WarpDesc));
   n += align_up(max_warps * sizeof(CtaDesc));
   n += align_up(P * 8 * 2);
-  n += 2 * kAlign + 3 * align_up(P * 4);                    // bisection: att, lo/hi/mid
-  n += 2 * align_up(P * K * T * 2 * 4) + kAlign;            // probe + at_lo counts
+  n += 4 * kAlign + 3 * align_up(P * 4) + align_up(P * Rb * 4);  // bisection: att, lo/hi, probes, tree
+  n += align_up(P * Rb * K * T * 2 * 4) + align_up(P * K * T * 2 * 4) + kAlign;  // probe + at_lo counts
   n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch
   n += align_up(P * R * K) + kAlign;                        // 32-bit window flags
   const size_t chunks = ((size_t)g->n_req + 31) / 32;
@@ -921,7 +984,7 @@ int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint3
   if (int32_t rc = check_workspace(workspace, workspace_bytes, cf_workspace_bytes(g, pl, 1))) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   Schedule sc;
-  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, false, &sc)) return rc;
+  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, false, false, &sc)) return rc;
   // the single simulation reads rate slot `plan` (pr = plan*1 + 0): upload a full-length rate array
   Blob blob;
   blob.reserve(kAlign);
@@ -962,6 +1025,24 @@ uint32_t cf_last_launch_count(void) { return g_launch_count; }
 int32_t cf_debug_kernel_mode(uint32_t mode) {
   if (mode > 1) return CF_ERR_ARG;
   g_kernel_mode = mode;
+  return CF_OK;
+}
+
+int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_probes, void* stream) {
+  if (!workspace || !out_probes) return CF_ERR_ARG;
+  cudaError_t e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+  if (e == cudaSuccess)
+    e = cudaMemcpy(out_probes, static_cast<const uint8_t*>(workspace) + kAlign, (size_t)n_plans * 4, cudaMemcpyDeviceToHost);
+  return e == cudaSuccess ? CF_OK : cuda_rc(e);
+}
+
+int32_t cf_debug_bisect_depth(uint32_t depth) {
+  if (depth >= 16) {  // 16/17: plan-major / rate-major lane order of the bisection passes
+    g_rate_major = depth & 1u;
+    return CF_OK;
+  }
+  if (depth > kMaxSpecDepth) return CF_ERR_ARG;
+  g_spec_depth = depth;
   return CF_OK;
 }
 

@@ -375,9 +375,12 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   produce(0);
   __syncthreads();
 
+  // a warp none of whose lanes has work (closed brackets; fixup pass: no flagged lane) only helps
+  // producing the tiles
+  const bool consume = __any_sync(0xffffffffu, wanted);
   for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
     if (tile_idx + 1 < n_tiles) produce(tile_idx + 1);
-    if (warp_active) {
+    if (consume) {
       const uint32_t buf = tile_idx & 1u;
       const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
       const uint32_t n0 = tile_idx * kTile;

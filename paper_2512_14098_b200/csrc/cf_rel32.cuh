@@ -214,6 +214,8 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   const uint64_t delay = (uint64_t)prm.edge_delay;
 
   const uint32_t n_tiles = (prm.N + kTile - 1) / kTile;
+  // a warp whose lanes all skip (closed brackets) only helps producing the tiles
+  const bool consume = __any_sync(kFull, wanted);
   __syncthreads();
   produce_tile<CMAX>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
   __syncthreads();
@@ -221,7 +223,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
     if (tile_idx + 1 < n_tiles)
       produce_tile<CMAX>(prm, cta.variant, trial, variant, tile_idx + 1, tiles, totals, cnt_s, tid, warp, lane);
-    if (warp_active) {
+    if (consume) {
       const uint32_t buf = tile_idx & 1u;
       const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
       const uint32_t n0 = tile_idx * kTile;

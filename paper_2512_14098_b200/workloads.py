@@ -442,7 +442,7 @@ def config4_sweep(n_req: int = 1 << 18, n_trials: int = 8, n_steps: int = 32,
                     n_variants=n_variants, plan_variant=pv)
 
 
-def count_updates(graph: Graph, plans: Plans, counts: np.ndarray) -> int:
+def count_updates(graph: Graph, plans: Plans, counts: np.ndarray, per_plan: bool = False):
     """Exact number of request-stage updates from out_counts [P][R][K][T][2]: sum over sims and
     types of cnt_t * (number of stages of plan p that type t visits)."""
     P = plans.n_plans
@@ -453,4 +453,25 @@ def count_updates(graph: Graph, plans: Plans, counts: np.ndarray) -> int:
             valid = s < plans.n_stages.astype(np.int64)
             nvis[:, t] += ((plans.stage_mask[:, s].astype(np.int64) & tm) != 0) & valid
     c = np.asarray(counts).reshape(P, -1, graph.n_types, 2)[..., 0].astype(np.int64)
+    if per_plan:
+        return np.einsum("pst,pt->p", c, nvis)
     return int(np.einsum("pst,pt->", c, nvis))
+
+
+def count_heap_levels(graph: Graph, plans: Plans, counts: np.ndarray, per_plan: bool = False):
+    """Sum over all request-stage updates of floor(log2 c) of the visited stage: the comparison
+    levels a replace-min on a c-entry binary heap descends at most (0 for c = 1, the plain Lindley
+    recursion). Used by bench.py's algorithmic-operation model."""
+    P = plans.n_plans
+    lev = np.zeros((P, graph.n_types), dtype=np.int64)
+    for t in range(graph.n_types):
+        tm = int(graph.type_mask[t])
+        for s in range(plans.max_stages):
+            valid = s < plans.n_stages.astype(np.int64)
+            visit = ((plans.stage_mask[:, s].astype(np.int64) & tm) != 0) & valid
+            c = np.maximum(plans.stage_c[:, s].astype(np.int64), 1)
+            lev[:, t] += visit * np.floor(np.log2(c)).astype(np.int64)
+    c = np.asarray(counts).reshape(P, -1, graph.n_types, 2)[..., 0].astype(np.int64)
+    if per_plan:
+        return np.einsum("pst,pt->p", c, lev)
+    return int(np.einsum("pst,pt->", c, lev))

@@ -474,7 +474,7 @@ int regs_of32() {
     cudaFuncAttributes a;
     if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false>) != cudaSuccess) {
       cudaGetLastError();
-      return 96;  // __launch_bounds__ cap of this build; used when no device is present
+      return 128;  // __launch_bounds__ cap of this build; used when no device is present
     }
     return a.numRegs;
   }();

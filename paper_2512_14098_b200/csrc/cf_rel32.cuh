@@ -89,9 +89,8 @@ __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
 // each stored as (key << 2) | slot; nodes >= c hold +inf. nq = heap_quads(c) >= 1.
 // Returns the new root key.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t heap4_replace_min(uint32_t hb, uint32_t nq512, uint32_t key) {
-  const uint32_t xk = key << 2;
-  uint4 q = lds128(hb);
+__device__ __forceinline__ uint32_t heap4_replace_min(uint32_t hb, uint32_t nq512, uint32_t key, uint4 q) {
+  const uint32_t xk = key << 2;  // q = the top quad (at hb), loaded by the caller ahead of time
   uint32_t m = min(min(q.x, q.y), min(q.z, q.w));
   if (xk <= m) return key;  // x <= every child
   const uint32_t new_root = m >> 2;
@@ -120,7 +119,7 @@ __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint
 
 template <int VMAX, int CMAX, bool HAS_DELAY>
 #ifndef CF_MINB32
-#define CF_MINB32 5
+#define CF_MINB32 4
 #endif
 __global__ void __launch_bounds__(kThreads, CF_MINB32)
 cf_sim32_kernel(const __grid_constant__ KParams prm) {
@@ -296,33 +295,54 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           }
         }
         __syncwarp();
-        // ---- the per-request loop: every lane runs its own simulation over the same 32 requests
+        // ---- the per-request loop: every lane runs its own simulation over the same 32 requests.
+        // Loads are issued ahead of their use by hand (the shared-memory accesses are ordered asm):
+        // the next record during the current request, the next visit's state record and the current
+        // stage's top heap quad before the 64-bit max/add chain.
+        const uint32_t wb_sa = smem_sa + SL::wbuf + (uint32_t)warp * 32u * kW * 16u;
+        uint4 n0w = lds128(wb_sa), n1w = lds128(wb_sa + 16u);
+        uint4 n2w = make_uint4(0, 0, 0, 0), n3w = make_uint4(0, 0, 0, 0);
+        if (kW > 2) n2w = lds128(wb_sa + 32u);
+        if (kW > 3) n3w = lds128(wb_sa + 48u);
 #pragma unroll 1
         for (int r = 0; r < n_here; ++r) {
-          const uint4* rp = wbuf + r * kW;
-          const uint4 w0 = rp[0], w1 = rp[1];
-          uint4 w2 = make_uint4(0, 0, 0, 0), w3 = make_uint4(0, 0, 0, 0);
-          if (kW > 2) w2 = rp[2];
-          if (kW > 3) w3 = rp[3];
+          const uint4 w0 = n0w, w1 = n1w, w2 = n2w, w3 = n3w;
+          uint32_t sid = w1.x & 0xffu;
+          uint4 st = make_uint4(0, 0, 0, 0);
+          if (sid != 0xffu) st = lds128(st_sa + sid * 512u);
+          {  // next record (the buffer has 32 records; reading one past the chunk's last is harmless)
+            const uint32_t na = wb_sa + (uint32_t)min(r + 1, 31) * (kW * 16u);
+            n0w = lds128(na); n1w = lds128(na + 16u);
+            if (kW > 2) n2w = lds128(na + 32u);
+            if (kW > 3) n3w = lds128(na + 48u);
+          }
           // a3: A - O = (r0 + d * period) >> 16
           const uint32_t a = (uint32_t)(mad_wide_u32(w0.x, period, (uint64_t)r0) >> 16);
           uint64_t x = a;
 #pragma unroll
           for (int j = 0; j < VMAX; ++j) {
-            const uint32_t sid = ((j < 4 ? w1.x : w1.y) >> (8 * (j & 3))) & 0xffu;
             if (sid == 0xffu) break;  // warp-uniform: all lanes see the same request
             const uint32_t S = j == 0 ? w1.z : j == 1 ? w1.w : j == 2 ? w2.x : j == 3 ? w2.y
                              : j == 4 ? w2.z : j == 5 ? w2.w : j == 6 ? w3.x : w3.y;
             const uint32_t sa = st_sa + sid * 512u;
-            const uint4 st = lds128(sa);
-            const uint64_t base = ((uint64_t)st.y << 32) | st.x;
-            const uint64_t f = base + st.z;  // earliest free time of the stage
+            const uint4 cur = st;
+            const uint32_t nq = cur.w >> 16, hb = heap_sa + (cur.w & 0xffffu) * 512u;
+            uint4 q = make_uint4(0, 0, 0, 0);
+            if (nq) q = lds128(hb);  // top quad of this stage's heap
+            if (j + 1 < VMAX) {      // state record of the next visit
+              sid = ((j + 1 < 4 ? w1.x : w1.y) >> (8 * ((j + 1) & 3))) & 0xffu;
+              if (sid != 0xffu) st = lds128(st_sa + sid * 512u);
+            } else {
+              sid = 0xffu;
+            }
+            const uint64_t base = ((uint64_t)cur.y << 32) | cur.x;
+            const uint64_t f = base + cur.z;  // earliest free time of the stage
             if (HAS_DELAY && j > 0) x += delay;
-            x = (x > f ? x : f) + S;         // a5/a6: start at max(arrival, earliest free)
+            x = (x > f ? x : f) + S;          // a5/a6: start at max(arrival, earliest free)
             const uint64_t key64 = x - base;
             if (key64 >= (uint64_t)kKeyLimit) flagged = true;
             uint32_t key = (uint32_t)key64;
-            if (st.w >> 16) key = heap4_replace_min(heap_sa + (st.w & 0xffffu) * 512u, (st.w >> 16) << 9, key);
+            if (nq) key = heap4_replace_min(hb, nq << 9, key, q);
             sts32(sa + 8u, key);
           }
           // a8

@@ -1,0 +1,146 @@
+"""GPU parity of the fast kernel's machinery: the 30-bit key window and its
+64-bit fixup pass, the forced 64-bit mode, clamped / negative latency targets, and the speculative
+bisection at every depth. Everything is compared bit for bit with the CPU oracle."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2512_14098_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+NT = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def cf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2512_14098_b200 import binding
+    yield binding
+    binding.cf_debug_kernel_mode(0)
+    binding.cf_debug_bisect_depth(0)
+
+
+def eval_both_modes(cf, orc, w, variant=0):
+    """auto mode (fast kernel + fixup) and forced 64-bit mode against the oracle; returns the number
+    of simulations the fixup pass had to redo in auto mode."""
+    want = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, variant, n_threads=NT)
+    wide = None
+    for mode in (0, 1):
+        cf.cf_debug_kernel_mode(mode)
+        try:
+            got = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, variant)
+            assert cf.cf_workspace_status(got["workspace"]) == want["rc"]
+            n_wide = cf.cf_workspace_wide_count(got["workspace"])
+        finally:
+            cf.cf_debug_kernel_mode(0)
+        np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+        np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+        if mode == 0:
+            wide = n_wide
+        else:
+            assert n_wide == 0  # the 64-bit kernel alone never defers anything
+    return wide
+
+
+def test_both_kernels_on_the_configs(cf, orc):
+    assert eval_both_modes(cf, orc, W.config1_mllm(n_req=1100, n_trials=2, n_rates=3)) == 0
+    assert eval_both_modes(cf, orc, W.config2_omni(n_req=900, n_trials=2, n_rates=3, vectors_per_pattern=3)) == 0
+    assert eval_both_modes(cf, orc, W.config3_multireplica(n_req=700, n_trials=2, n_rates=2,
+                                                           plans_per_topology=24)) == 0
+
+
+def one_stage(service_tab, arr_tab, n_req, cs, rates, L=(10_000_000,), n_trials=2, seed=11):
+    g = W.Graph(1, 1, n_req, n_trials, [1], W.mix_thresholds([1.0]), [0], [service_tab], arr_tab,
+                np.zeros((0, 2)))
+    pl = W.make_plans([[(1, c)] for c in cs])
+    r = np.tile(np.asarray(rates, dtype=np.uint32), (len(cs), 1))
+    return W.Workload("one", g, pl, W.Slo(list(L), [9], [10]), seed=seed, rate_mrps=r)
+
+
+def test_key_window_exit_goes_through_the_fixup_pass(cf, orc):
+    # 1000 s services on mostly idle replicas: a request that arrives 74 s or more into a tile
+    # gets a key >= 2^30 (free time - stage base); those lanes are redone by the 64-bit kernel.
+    w = one_stage(W.constant_qtab(1_000_000_000), W.exponential_qtab(65536.0), 700, (1, 50, 200),
+                  (1000, 500, 200_000))
+    wide = eval_both_modes(cf, orc, w)
+    assert wide > 0
+    # a tile of 128 requests spanning more than 2^31 us (rate 1 milli-request/s)
+    w = one_stage(W.lognormal_qtab(50_000.0, 0.5), W.exponential_qtab(65536.0), 400, (1, 3), (1, 8, 5000))
+    assert eval_both_modes(cf, orc, w) > 0
+    # a tile spanning more than 2^32 gap units
+    w = one_stage(W.constant_qtab(700), W.constant_qtab(2**31 - 1), 300, (1, 2), (1_000_000, 1_000_000_000))
+    assert eval_both_modes(cf, orc, w) > 0
+
+
+def test_unbounded_waits_stay_on_the_fast_path(cf, orc):
+    # 3x overload, 20 000 requests of 1 s: waits reach hours (far beyond 32 bits of microseconds),
+    # yet the keys stay small because they are relative to the stage base
+    w = one_stage(W.lognormal_qtab(1_000_000.0, 0.3), W.exponential_qtab(65536.0), 20_000, (1, 2, 5),
+                  (3000, 6000, 15_000), n_trials=1)
+    assert eval_both_modes(cf, orc, w) == 0
+    got = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed)
+    assert int(got["makespan"].max()) > 1 << 32
+
+
+def test_services_too_long_for_the_fast_path(cf, orc):
+    # worst-case service above 2^30 us: the host never admits the fast kernel
+    w = one_stage(W.constant_qtab(1_200_000_000), W.exponential_qtab(65536.0), 300, (1, 4), (1, 1000))
+    assert eval_both_modes(cf, orc, w) == 0
+
+
+def test_negative_and_huge_latency_targets(cf, orc):
+    w = W.config1_mllm(n_req=800, n_trials=2, n_rates=3, llm_max=6, e_steps=3)
+    w.slo = W.Slo([-5, 1 << 40], [9, 9], [10, 10])
+    eval_both_modes(cf, orc, w)
+    want = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, n_threads=NT)
+    assert (want["counts"][..., 0, 1] == 0).all()                             # L < 0: never a hit
+    np.testing.assert_array_equal(want["counts"][..., 1, 1], want["counts"][..., 1, 0])  # always a hit
+    w.slo = W.Slo([0, 2**31 - 1], [9, 9], [10, 10])
+    eval_both_modes(cf, orc, w)
+
+
+def test_speculative_bisection_depths(cf, orc):
+    w = W.config2_omni(n_req=600, n_trials=2, n_rates=2, vectors_per_pattern=2, n_patterns=16)
+    R_p = W.flow_bound_mrps(w.graph, w.plans)
+    hi = np.ceil(1.5 * R_p).astype(np.uint32)
+    hi[0], hi[1], hi[2], hi[3] = 0, 1, 2, 3
+    slo = W.Slo(w.slo.L_us, [9] * w.graph.n_types, [10] * w.graph.n_types)
+    for steps in (1, 3, 7, 18):
+        bo = orc.goodput_bisect(w.graph, w.plans, hi, steps, slo, w.seed, n_threads=NT)
+        for depth in (1, 2, 3, 4, 0):
+            cf.cf_debug_bisect_depth(depth)
+            try:
+                b = cf.cf_goodput_bisect(w.graph, w.plans, hi, steps, slo, w.seed)
+                probes = cf.cf_bisect_probes(b["workspace"], w.plans.n_plans)
+            finally:
+                cf.cf_debug_bisect_depth(0)
+            np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+            np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"]), bo["goodput_mrps"])
+            np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
+            # real probes: none for an empty bracket, one for [0,2), never more than steps or log2(hi)+1
+            assert probes[0] == 0 and probes[1] == 0 and probes[2] == 1
+            assert (probes <= steps).all()
+            assert (probes <= np.floor(np.log2(np.maximum(hi, 1))) + 1).all()
+
+
+def test_bisection_with_window_exits(cf, orc):
+    # probes far above capacity with long services leave the key window; the bisection result
+    # must not notice
+    w = one_stage(W.constant_qtab(900_000_000), W.exponential_qtab(65536.0), 500, (40, 100, 300),
+                  (1000,), L=(1_000_000_000,), n_trials=2)
+    hi = np.array([4000, 4000, 4000], dtype=np.uint32)
+    bo = orc.goodput_bisect(w.graph, w.plans, hi, 9, w.slo, w.seed, n_threads=NT)
+    for depth in (1, 3):
+        cf.cf_debug_bisect_depth(depth)
+        try:
+            b = cf.cf_goodput_bisect(w.graph, w.plans, hi, 9, w.slo, w.seed)
+        finally:
+            cf.cf_debug_bisect_depth(0)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"]), bo["goodput_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])

@@ -18,7 +18,10 @@
 
 namespace cfk {
 
-constexpr int kWarpsPerCta = 4;
+#ifndef CF_WARPS
+#define CF_WARPS 8
+#endif
+constexpr int kWarpsPerCta = CF_WARPS;
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kTile = 128;              // requests per CTA tile
 constexpr int kChunks = kTile / 32;     // 32-request chunks per tile

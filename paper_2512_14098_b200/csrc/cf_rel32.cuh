@@ -119,7 +119,7 @@ __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint
 
 template <int VMAX, int CMAX, bool HAS_DELAY>
 #ifndef CF_MINB32
-#define CF_MINB32 4
+#define CF_MINB32 2
 #endif
 __global__ void __launch_bounds__(kThreads, CF_MINB32)
 cf_sim32_kernel(const __grid_constant__ KParams prm) {
@@ -300,13 +300,9 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         // the next record during the current request, the next visit's state record and the current
         // stage's top heap quad before the 64-bit max/add chain.
         const uint32_t wb_sa = smem_sa + SL::wbuf + (uint32_t)warp * 32u * kW * 16u;
-        uint4 n0w = lds128(wb_sa), n1w = lds128(wb_sa + 16u);
-        uint4 n2w = make_uint4(0, 0, 0, 0), n3w = make_uint4(0, 0, 0, 0);
-        if (kW > 2) n2w = lds128(wb_sa + 32u);
-        if (kW > 3) n3w = lds128(wb_sa + 48u);
-#pragma unroll 1
-        for (int r = 0; r < n_here; ++r) {
-          const uint4 w0 = n0w, w1 = n1w, w2 = n2w, w3 = n3w;
+        // one request: the record is in (w0..w3); the next record is loaded into (n0..n3)
+        auto request = [&](const uint4& w0, const uint4& w1, const uint4& w2, const uint4& w3,
+                           uint4& n0w, uint4& n1w, uint4& n2w, uint4& n3w, int r) {
           uint32_t sid = w1.x & 0xffu;
           uint4 st = make_uint4(0, 0, 0, 0);
           if (sid != 0xffu) st = lds128(st_sa + sid * 512u);
@@ -349,7 +345,19 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           if (x <= (uint64_t)a + w0.y) { hlo += w0.z; hhi += w0.w; }
           dep += x;
           mk = x > mk ? x : mk;
+        };
+        uint4 a0 = lds128(wb_sa), a1 = lds128(wb_sa + 16u);
+        uint4 a2 = make_uint4(0, 0, 0, 0), a3 = make_uint4(0, 0, 0, 0);
+        if (kW > 2) a2 = lds128(wb_sa + 32u);
+        if (kW > 3) a3 = lds128(wb_sa + 48u);
+        uint4 b0, b1, b2 = make_uint4(0, 0, 0, 0), b3 = make_uint4(0, 0, 0, 0);
+        int r = 0;
+#pragma unroll 1
+        for (; r + 1 < n_here; r += 2) {  // two requests per trip: the record registers ping-pong
+          request(a0, a1, a2, a3, b0, b1, b2, b3, r);
+          request(b0, b1, b2, b3, a0, a1, a2, a3, r + 1);
         }
+        if (r < n_here) request(a0, a1, a2, a3, b0, b1, b2, b3, r);
         __syncwarp();
         cu_base += totals[buf * kChunks + ch];
       }

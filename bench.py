@@ -37,6 +37,11 @@ OPS_PER_REQUEST = 18
 OPS_PER_UPDATE = 7
 OPS_PER_HEAP_LEVEL = 11
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the simulation kernel, per launch at full size,
+# from the ncu captures in profiles/r01_ncu_full_cfg1_cfg2_fullsize_fast_kernel.txt (the outputs
+# stay in the 126 MB L2 past the end of the launch, so almost nothing is written back in time)
+NCU_TRAFFIC_BYTES = {1: 683_776, 2: 1_176_576}
+
 
 def make_workload(cfg: int, scale: float = 1.0):
     if cfg == 0:
@@ -355,7 +360,10 @@ def main():
         alg_ops = OPS_PER_REQUEST * requests + OPS_PER_UPDATE * updates + OPS_PER_HEAP_LEVEL * heap_levels
         achieved = alg_ops / step_s / 1e12
         alu = {"bound": "alu", "achieved": achieved, "peak": peak_tops, "unit": "Tlane-op/s",
-               "frac": achieved / peak_tops, "traffic": None,
+               "frac": achieved / peak_tops,
+               "traffic": NCU_TRAFFIC_BYTES.get(args.config) if args.scale == 1.0 else None,
+               "traffic_unit": "bytes per launch (ncu dram read+write, profiles/)",
+               "frac_of_measured_alu_pipe_peak": (achieved / peaks["alu_pipe"]) if "alu_pipe" in peaks else None,
                "peak_source": f"derived: {sm_count} SMs x 4 schedulers x 32 lanes x {sm_mhz:.0f} MHz",
                "measured_int32_peaks_tops": peaks,
                "ops_model": {"per_request": OPS_PER_REQUEST, "per_update": OPS_PER_UPDATE,

@@ -260,3 +260,34 @@ def test_cfg2_full_size_sampled(cf, orc):
 
 def test_cfg3_full_size_sampled(cf, orc):
     sampled_full_size(cf, orc, W.config3_multireplica(), 8, 3)
+
+
+def test_cfg4_full_size_sampled(cf, orc):
+    """configs[4] exactly as bench.py runs it (4 GiB materialised stream, 32-step device-side
+    bisection, speculative passes, fixup pass): sampled plans against the oracle's bisection."""
+    w = W.config4_sweep()
+    rec = cf.cf_materialize_stream(w.graph, w.seed, 0, w.n_variants)
+    b = cf.cf_goodput_bisect(w.graph, w.plans, w.rate_hi_mrps, w.n_steps, w.slo, w.seed, stream_records=rec,
+                             n_variants=w.n_variants, plan_variant=w.plan_variant)
+    assert cf.cf_workspace_status(b["workspace"]) == 0
+    rate = cf.to_numpy_u32(b["rate_mrps"])
+    good = cf.to_numpy_u32(b["goodput_mrps"])
+    counts = cf.to_numpy_u32(b["counts"])
+    probes = cf.cf_bisect_probes(b["workspace"], w.plans.n_plans)
+    rng = np.random.default_rng(4)
+    for p in rng.integers(0, w.plans.n_plans, 4):
+        idx = np.array([p])
+        bo = orc.goodput_bisect(w.graph, w.plans.subset(idx), w.rate_hi_mrps[idx], w.n_steps, w.slo, w.seed,
+                                int(w.plan_variant[p]), n_threads=NT)
+        np.testing.assert_array_equal(rate[idx], bo["rate_mrps"])
+        np.testing.assert_array_equal(good[idx], bo["goodput_mrps"])
+        np.testing.assert_array_equal(counts[idx], bo["counts"])
+    # properties that hold at any size
+    assert (rate < w.rate_hi_mrps).all() and (rate > 0).any()
+    assert (probes <= w.n_steps).all() and (probes >= 1).all()
+    c = counts.astype(np.int64)
+    feasible = rate > 0
+    assert (c[feasible][..., 0].sum(-1) == w.graph.n_req).all()
+    assert (c[~feasible] == 0).all()
+    att_ok = c[feasible][..., 1].sum(1) * 10 >= 9 * c[feasible][..., 0].sum(1)  # pooled 90 % per type
+    assert att_ok.all()

@@ -30,6 +30,8 @@
 // or the R17 horizon is exceeded. It then sets flags[slot] and writes nothing; the 64-bit kernel
 // of cf_device.cuh runs in fixup mode over exactly those simulations. Results are bit-identical.
 #pragma once
+#include <type_traits>
+
 #include "cf_device.cuh"
 
 namespace cfk {
@@ -261,6 +263,8 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         const uint32_t nc0 = n0 + ch * 32;
         if (nc0 >= prm.N) break;
         const int n_here = (int)min(32u, prm.N - nc0);
+        bool chunk_long = false;
+        uint64_t chunk_work = 0;
         // ---- a4: component-level record -> list of visited stages for this warp's topology ----
         {
           const uint4* src = tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
@@ -280,7 +284,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           uint8_t* dst = reinterpret_cast<uint8_t*>(wbuf + lane * kW);
           *reinterpret_cast<uint4*>(dst) = make_uint4((uint32_t)d64, l32_s[t], inc.x, inc.y);
           *reinterpret_cast<uint2*>(dst + 16) = make_uint2(0xffffffffu, 0xffffffffu);  // no visits yet
-          uint32_t nv = 0;
+          uint32_t nv = 0, work = 0;  // work: this request's services (the host caps the worst case at 2^30)
 #pragma unroll
           for (int s = 0; s < VMAX; ++s) {
             const uint32_t sm = (s < (int)n_stages) ? topo.mask[s] : 0u;
@@ -290,9 +294,15 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
               for (int i = 0; i < CMAX; ++i) acc += ((sm >> i) & 1u) ? svc[i] : 0;
               dst[16 + nv] = (uint8_t)s;
               *reinterpret_cast<int32_t*>(dst + 24 + 4 * nv) = acc;
+              work += (uint32_t)acc;
               ++nv;
             }
           }
+          if (lane >= n_here) work = 0;
+          // services of the whole chunk (each request's share clamped to 2^26 so the sum fits 32 bits;
+          // a longer one makes the chunk "long") plus every possible hop
+          chunk_long = __any_sync(kFull, work >= (1u << 26));
+          chunk_work = (uint64_t)__reduce_add_sync(kFull, min(work, 1u << 26)) + 32ull * 7ull * delay;
         }
         __syncwarp();
         // ---- the per-request loop: every lane runs its own simulation over the same 32 requests.
@@ -300,9 +310,14 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         // the next record during the current request, the next visit's state record and the current
         // stage's top heap quad before the 64-bit max/add chain.
         const uint32_t wb_sa = smem_sa + SL::wbuf + (uint32_t)warp * 32u * kW * 16u;
-        // one request: the record is in (w0..w3); the next record is loaded into (n0..n3)
-        auto request = [&](const uint4& w0, const uint4& w1, const uint4& w2, const uint4& w3,
+        // one request: the record is in (w0..w3); the next record is loaded into (n0..n3).
+        // NARROW: every time of this chunk provably fits 32 bits (see the bound below): x, the free
+        // times and the SLO test are 32-bit; otherwise the running departure x is 64-bit.
+        uint32_t kmax = 0, mk32 = 0;
+        auto request = [&](auto narrow_tag, const uint4& w0, const uint4& w1, const uint4& w2, const uint4& w3,
                            uint4& n0w, uint4& n1w, uint4& n2w, uint4& n3w, int r) {
+          constexpr bool NARROW = decltype(narrow_tag)::value;
+          using X = typename std::conditional<NARROW, uint32_t, uint64_t>::type;
           uint32_t sid = w1.x & 0xffu;
           uint4 st = make_uint4(0, 0, 0, 0);
           if (sid != 0xffu) st = lds128(st_sa + sid * 512u);
@@ -314,7 +329,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           }
           // a3: A - O = (r0 + d * period) >> 16
           const uint32_t a = (uint32_t)(mad_wide_u32(w0.x, period, (uint64_t)r0) >> 16);
-          uint64_t x = a;
+          X x = a;
 #pragma unroll
           for (int j = 0; j < VMAX; ++j) {
             if (sid == 0xffu) break;  // warp-uniform: all lanes see the same request
@@ -331,33 +346,69 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
             } else {
               sid = 0xffu;
             }
-            const uint64_t base = ((uint64_t)cur.y << 32) | cur.x;
-            const uint64_t f = base + cur.z;  // earliest free time of the stage
-            if (HAS_DELAY && j > 0) x += delay;
-            x = (x > f ? x : f) + S;          // a5/a6: start at max(arrival, earliest free)
-            const uint64_t key64 = x - base;
-            if (key64 >= (uint64_t)kKeyLimit) flagged = true;
-            uint32_t key = (uint32_t)key64;
+            uint32_t key;
+            if (NARROW) {
+              const uint32_t f = cur.x + cur.z;  // earliest free time of the stage (base_hi == 0)
+              if (HAS_DELAY && j > 0) x += (X)delay;
+              x = max((uint32_t)x, f) + S;       // a5/a6: start at max(arrival, earliest free)
+              key = (uint32_t)x - cur.x;
+              kmax = max(kmax, key);             // window check after the chunk
+            } else {
+              const uint64_t base = ((uint64_t)cur.y << 32) | cur.x;
+              const uint64_t f = base + cur.z;
+              if (HAS_DELAY && j > 0) x += (X)delay;
+              x = (X)(((uint64_t)x > f ? (uint64_t)x : f) + S);
+              const uint64_t key64 = (uint64_t)x - base;
+              if (key64 >= (uint64_t)kKeyLimit) flagged = true;
+              key = (uint32_t)key64;
+            }
             if (nq) key = heap4_replace_min(hb, nq << 9, key, q);
             sts32(sa + 8u, key);
           }
           // a8
-          if (x <= (uint64_t)a + w0.y) { hlo += w0.z; hhi += w0.w; }
-          dep += x;
-          mk = x > mk ? x : mk;
+          if (NARROW) {
+            if ((uint32_t)x <= a + w0.y) { hlo += w0.z; hhi += w0.w; }
+            dep = mad_wide_u32((uint32_t)x, 1u, dep);
+            mk32 = max(mk32, (uint32_t)x);
+          } else {
+            if ((uint64_t)x <= (uint64_t)a + w0.y) { hlo += w0.z; hhi += w0.w; }
+            dep += (uint64_t)x;
+            mk = (uint64_t)x > mk ? (uint64_t)x : mk;
+          }
         };
+        // Bound for the chunk: every departure is at most M + (all services and hops of the chunk),
+        // M = max(latest departure so far, last arrival of the chunk), both relative to the origin
+        // (induction over x = max(arrival, F) + S; every free time is some earlier departure).
+        const uint32_t a_last = (uint32_t)(mad_wide_u32((uint32_t)(last_cu - tile_base), period, (uint64_t)r0) >> 16);
+        uint64_t seen = makespan > origin ? makespan - origin : 0;
+        if (mk > seen) seen = mk;
+        if (a_last > seen) seen = a_last;
+        const bool narrow = __all_sync(kFull, !chunk_long && seen + chunk_work < 0xffffffffull);
         uint4 a0 = lds128(wb_sa), a1 = lds128(wb_sa + 16u);
         uint4 a2 = make_uint4(0, 0, 0, 0), a3 = make_uint4(0, 0, 0, 0);
         if (kW > 2) a2 = lds128(wb_sa + 32u);
         if (kW > 3) a3 = lds128(wb_sa + 48u);
         uint4 b0, b1, b2 = make_uint4(0, 0, 0, 0), b3 = make_uint4(0, 0, 0, 0);
         int r = 0;
+        if (narrow) {
+          const std::true_type tag;
 #pragma unroll 1
-        for (; r + 1 < n_here; r += 2) {  // two requests per trip: the record registers ping-pong
-          request(a0, a1, a2, a3, b0, b1, b2, b3, r);
-          request(b0, b1, b2, b3, a0, a1, a2, a3, r + 1);
+          for (; r + 1 < n_here; r += 2) {  // two requests per trip: the record registers ping-pong
+            request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
+            request(tag, b0, b1, b2, b3, a0, a1, a2, a3, r + 1);
+          }
+          if (r < n_here) request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
+          if (kmax >= kKeyLimit) flagged = true;
+          if (mk32 > mk) mk = mk32;
+        } else {
+          const std::false_type tag;
+#pragma unroll 1
+          for (; r + 1 < n_here; r += 2) {
+            request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
+            request(tag, b0, b1, b2, b3, a0, a1, a2, a3, r + 1);
+          }
+          if (r < n_here) request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
         }
-        if (r < n_here) request(a0, a1, a2, a3, b0, b1, b2, b3, r);
         __syncwarp();
         cu_base += totals[buf * kChunks + ch];
       }

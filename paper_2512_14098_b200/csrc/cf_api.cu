@@ -455,9 +455,9 @@ int kernel_regs(int vmax, int cmax) {
 }
 
 // ---- the 32-bit fast kernel (cf_rel32.cuh) ---------------------------------------------------------
-template <int VMAX, int CMAX, bool HAS_DELAY>
+template <int VMAX, int CMAX, bool HAS_DELAY, bool T8>
 cudaError_t launch_one32(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  auto kern = cf_sim32_kernel<VMAX, CMAX, HAS_DELAY>;
+  auto kern = cf_sim32_kernel<VMAX, CMAX, HAS_DELAY, T8>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
   if (e != cudaSuccess) return e;
   kp.k_launch = n_trials;
@@ -472,7 +472,7 @@ template <int VMAX, int CMAX>
 int regs_of32() {
   static int regs = [] {
     cudaFuncAttributes a;
-    if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false>) != cudaSuccess) {
+    if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false, true>) != cudaSuccess) {
       cudaGetLastError();
       return 128;  // __launch_bounds__ cap of this build; used when no device is present
     }
@@ -489,13 +489,19 @@ int kernel_regs32(int vmax, int cmax) {
   return regs_of32<8, 6>();
 }
 
+template <int VMAX, int CMAX>
+cudaError_t launch_v32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  const bool d = kp.edge_delay != 0, t8 = kp.T > 4;
+  if (d) return t8 ? launch_one32<VMAX, CMAX, true, true>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, true, false>(kp, sc, n_trials, st);
+  return t8 ? launch_one32<VMAX, CMAX, false, true>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, false, false>(kp, sc, n_trials, st);
+}
+
 cudaError_t launch_sims32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  const bool d = kp.edge_delay != 0;
-  if (sc.cmax == 8) return d ? launch_one32<8, 8, true>(kp, sc, n_trials, st) : launch_one32<8, 8, false>(kp, sc, n_trials, st);
-  if (sc.vmax32 == 2) return d ? launch_one32<2, 6, true>(kp, sc, n_trials, st) : launch_one32<2, 6, false>(kp, sc, n_trials, st);
-  if (sc.vmax32 == 4) return d ? launch_one32<4, 6, true>(kp, sc, n_trials, st) : launch_one32<4, 6, false>(kp, sc, n_trials, st);
-  if (sc.vmax32 == 6) return d ? launch_one32<6, 6, true>(kp, sc, n_trials, st) : launch_one32<6, 6, false>(kp, sc, n_trials, st);
-  return d ? launch_one32<8, 6, true>(kp, sc, n_trials, st) : launch_one32<8, 6, false>(kp, sc, n_trials, st);
+  if (sc.cmax == 8) return launch_v32<8, 8>(kp, sc, n_trials, st);
+  if (sc.vmax32 == 2) return launch_v32<2, 6>(kp, sc, n_trials, st);
+  if (sc.vmax32 == 4) return launch_v32<4, 6>(kp, sc, n_trials, st);
+  if (sc.vmax32 == 6) return launch_v32<6, 6>(kp, sc, n_trials, st);
+  return launch_v32<8, 6>(kp, sc, n_trials, st);
 }
 
 // The 32-bit kernel needs max(A, F) + S + delay to stay below 2^32 whenever its inputs are inside the

@@ -119,7 +119,8 @@ __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint
   return p == kInf32 ? kInf32 : v;
 }
 
-template <int VMAX, int CMAX, bool HAS_DELAY>
+// T8: more than 4 request types (a second word of hit-counter byte fields)
+template <int VMAX, int CMAX, bool HAS_DELAY, bool T8>
 #ifndef CF_MINB32
 #define CF_MINB32 2
 #endif
@@ -206,9 +207,10 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   }
   TopoDesc topo;
   if (warp_active) topo = prm.topos[wd.topo];
-  uint32_t hits[8];
+  constexpr int kTypes = T8 ? 8 : 4;
+  uint32_t hits[kTypes];
 #pragma unroll
-  for (int t = 0; t < 8; ++t) hits[t] = 0;
+  for (int t = 0; t < kTypes; ++t) hits[t] = 0;
   uint64_t dep_sum = 0, cu_base = 0, tile_base = 0, last_cu = 0;
   uint64_t origin = 0;  // O: absolute time of offset 0 (microseconds)
   uint64_t makespan = 0;
@@ -367,11 +369,11 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           }
           // a8
           if (NARROW) {
-            if ((uint32_t)x <= a + w0.y) { hlo += w0.z; hhi += w0.w; }
+            if ((uint32_t)x <= a + w0.y) { hlo += w0.z; if (T8) hhi += w0.w; }
             dep = mad_wide_u32((uint32_t)x, 1u, dep);
             mk32 = max(mk32, (uint32_t)x);
           } else {
-            if ((uint64_t)x <= (uint64_t)a + w0.y) { hlo += w0.z; hhi += w0.w; }
+            if ((uint64_t)x <= (uint64_t)a + w0.y) { hlo += w0.z; if (T8) hhi += w0.w; }
             dep += (uint64_t)x;
             mk = (uint64_t)x > mk ? (uint64_t)x : mk;
           }
@@ -421,7 +423,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
 #pragma unroll
       for (int t = 0; t < 4; ++t) {
         hits[t] += (hlo >> (8 * t)) & 0xffu;
-        hits[t + 4] += (hhi >> (8 * t)) & 0xffu;
+        if (T8) hits[T8 ? t + 4 : t] += (hhi >> (8 * t)) & 0xffu;
       }
     }
     __syncthreads();
@@ -442,7 +444,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
       uint32_t* oc = prm.out_counts + slot * prm.T * 2;
       for (uint32_t t = 0; t < prm.T; ++t) {
         oc[2 * t + 0] = skip ? 0u : cnt_s[t];
-        oc[2 * t + 1] = skip ? 0u : hits[t];
+        oc[2 * t + 1] = skip ? 0u : hits[t < (uint32_t)kTypes ? t : 0];
       }
       if (prm.out_dep_sum) prm.out_dep_sum[slot] = skip ? 0ull : dep_sum;
       if (prm.out_makespan) prm.out_makespan[slot] = skip ? 0ll : (int64_t)makespan;

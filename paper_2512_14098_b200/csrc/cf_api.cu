@@ -200,15 +200,47 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   };
   for (uint32_t p : order)
     if (variant_of(p) >= std::max(1u, n_variants)) return CF_ERR_ARG;
-  // (variant, topology, heap footprint descending, replica vector) -> homogeneous warps
+  // (variant, topology, then similar heap depths) -> homogeneous warps. A warp executes every
+  // replace-min to the depth of its deepest lane, so plans are ordered by the vector of their
+  // stages' heap depths, the most visited stage first (mix-weighted), then by the replica counts.
+  std::vector<uint64_t> plan_key(P, 0);  // 8 stages x (2 bits depth class | 6 bits of c), most visited stage first
+  {
+    std::vector<double> pi(g->n_types);
+    for (uint32_t t = 0; t < g->n_types; ++t) {
+      const double hi = t + 1 == g->n_types ? 4294967296.0 : (double)g->type_thresh[t];
+      const double lo = t == 0 ? 0.0 : (double)g->type_thresh[t - 1];
+      pi[t] = std::max(0.0, hi - lo);
+    }
+    std::vector<std::vector<uint32_t>> topo_order(sc.topos.size());
+    for (size_t ti = 0; ti < sc.topos.size(); ++ti) {
+      const TopoDesc& td = sc.topos[ti];
+      std::vector<double> wgt(td.n_stages, 0.0);
+      for (uint32_t st = 0; st < td.n_stages; ++st)
+        for (uint32_t t = 0; t < g->n_types; ++t)
+          if (td.mask[st] & g->type_mask[t]) wgt[st] += pi[t];
+      topo_order[ti].resize(td.n_stages);
+      std::iota(topo_order[ti].begin(), topo_order[ti].end(), 0u);
+      std::stable_sort(topo_order[ti].begin(), topo_order[ti].end(),
+                       [&](uint32_t x, uint32_t y) { return wgt[x] > wgt[y]; });
+    }
+    for (uint32_t p = 0; p < P; ++p) {
+      uint64_t kd = 0, kc = 0;
+      for (uint32_t st : topo_order[plan_topo[p]]) {
+        const uint32_t c = sc.plan_c[(size_t)p * 8 + st];
+        uint32_t depth = 0;  // levels of the 4-ary heap (fast kernel) / a proxy for the binary one
+        if (fast) depth = c <= 1 ? 0 : (c <= 5 ? 1 : (c <= 21 ? 2 : 3));
+        else depth = c <= 1 ? 0 : (c <= 3 ? 1 : (c <= 15 ? 2 : 3));
+        kd = (kd << 2) | depth;
+        kc = (kc << 6) | std::min(c, 63u);
+      }
+      plan_key[p] = (kd << 48) | kc;  // <= 16 bits of depths, <= 48 bits of replica counts
+    }
+  }
   std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) {
     const uint32_t va = variant_of(a), vb = variant_of(b);
     if (va != vb) return va < vb;
     if (plan_topo[a] != plan_topo[b]) return plan_topo[a] < plan_topo[b];
-    const std::vector<uint32_t>& rows = fast ? plan_quads : plan_pairs;
-    if (rows[a] != rows[b]) return rows[a] > rows[b];
-    return std::lexicographical_compare(sc.plan_c.begin() + (size_t)b * 8, sc.plan_c.begin() + (size_t)b * 8 + 8,
-                                        sc.plan_c.begin() + (size_t)a * 8, sc.plan_c.begin() + (size_t)a * 8 + 8);
+    return plan_key[a] > plan_key[b];
   });
 
   // simulations -> warps

@@ -622,6 +622,56 @@ __global__ void bisect_init_kernel(BisectState bs, const uint32_t* rate_hi, uint
   bisect_build_tree(bs.tree + (size_t)p * bs.R, bs.R, lo, hi, levels);
 }
 
+// pooled feasibility of one probe: counts pc[K][T][2] (R12, R18)
+__device__ bool probe_feasible(const uint32_t* pc, uint32_t K, uint32_t T, const uint32_t* att_num,
+                               const uint32_t* att_den) {
+  bool feasible = true;
+  for (uint32_t k = 0; k < K; ++k) {  // R18: an out-of-range probe (zeroed) is infeasible
+    uint64_t n = 0;
+    for (uint32_t t = 0; t < T; ++t) n += pc[(k * T + t) * 2];
+    if (n == 0) feasible = false;
+  }
+  for (uint32_t t = 0; t < T; ++t) {
+    uint64_t cnt = 0, hits = 0;
+    for (uint32_t k = 0; k < K; ++k) { cnt += pc[(k * T + t) * 2]; hits += pc[(k * T + t) * 2 + 1]; }
+    if (cnt > 0 && hits * (uint64_t)att_den[t] < (uint64_t)att_num[t] * cnt) feasible = false;
+  }
+  return feasible;
+}
+
+// Between the fast kernel and its fixup pass: walk the tree as far as the verdicts are already known
+// (a node none of whose K trials left the fast window); the flagged simulations of every node that
+// can no longer lie on the bisection path are dropped, so the 64-bit kernel does not redo them.
+__global__ void bisect_triage_kernel(BisectState bs, uint32_t P, uint32_t K, uint32_t T,
+                                     const uint32_t* att_num, const uint32_t* att_den, uint32_t levels,
+                                     uint8_t* flags) {
+  const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const uint32_t* tree = bs.tree + (size_t)p * bs.R;
+  auto node_flagged = [&](uint32_t node) {
+    bool f = false;
+    for (uint32_t k = 0; k < K; ++k) f = f || flags[((size_t)p * bs.R + (node - 1)) * K + k] != 0;
+    return f;
+  };
+  uint32_t node = 1, keep_root = 0;  // keep_root: the subtree whose flagged simulations stay
+  for (uint32_t step = 0; step < levels; ++step) {
+    if (tree[node - 1] == 0) break;
+    if (node_flagged(node)) { keep_root = node; break; }
+    const uint32_t* pc = bs.probe + ((size_t)p * bs.R + (node - 1)) * K * T * 2;
+    node = probe_feasible(pc, K, T, att_num, att_den) ? 2 * node + 1 : 2 * node;
+  }
+  for (uint32_t i = 1; i <= bs.R; ++i) {
+    bool keep = false;
+    if (keep_root) {
+      uint32_t a = i;
+      while (a > keep_root) a >>= 1;  // is keep_root an ancestor of (or equal to) i?
+      keep = a == keep_root;
+    }
+    if (!keep)
+      for (uint32_t k = 0; k < K; ++k) flags[((size_t)p * bs.R + (i - 1)) * K + k] = 0;
+  }
+}
+
 // one thread per plan: walk `levels` steps through the simulated tree (pool the probe counts over
 // trials, test feasibility, move the bracket), then lay out the tree of the next pass
 __global__ void bisect_update_kernel(BisectState bs, uint32_t P, uint32_t K, uint32_t T,
@@ -637,18 +687,7 @@ __global__ void bisect_update_kernel(BisectState bs, uint32_t P, uint32_t K, uin
     if (mid == 0) break;  // no-op step: the bracket has closed, every later step is a no-op too
     ++bs.n_probes[p];
     const uint32_t* pc = bs.probe + ((size_t)p * bs.R + (node - 1)) * K * T * 2;
-    bool feasible = true;
-    for (uint32_t k = 0; k < K; ++k) {  // DESIGN.md R18: an out-of-range probe (zeroed) is infeasible
-      uint64_t n = 0;
-      for (uint32_t t = 0; t < T; ++t) n += pc[(k * T + t) * 2];
-      if (n == 0) feasible = false;
-    }
-    for (uint32_t t = 0; t < T; ++t) {
-      uint64_t cnt = 0, hits = 0;
-      for (uint32_t k = 0; k < K; ++k) { cnt += pc[(k * T + t) * 2]; hits += pc[(k * T + t) * 2 + 1]; }
-      if (cnt > 0 && hits * (uint64_t)att_den[t] < (uint64_t)att_num[t] * cnt) feasible = false;
-    }
-    if (feasible) {
+    if (probe_feasible(pc, K, T, att_num, att_den)) {
       lo = mid;
       uint32_t* al = bs.at_lo + (size_t)p * K * T * 2;
       for (uint32_t i = 0; i < K * T * 2; ++i) al[i] = pc[i];
@@ -888,7 +927,17 @@ int32_t bisect_impl(const BisectArgs& a) {
   for (uint32_t step = 0; step < a.n_steps; step += depth) {
     const uint32_t levels = std::min(depth, a.n_steps - step);
     const uint32_t next_levels = std::min(depth, a.n_steps - step - levels);
-    if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, fast, a.st))) return rc;
+    if (!fast) {
+      if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, false, a.st))) return rc;
+    } else {
+      if (int32_t rc = cuda_rc(launch_sims32(kp, sc, K, a.st))) return rc;
+      bisect_triage_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, reinterpret_cast<const uint32_t*>(ws + att_off),
+                                                 reinterpret_cast<const uint32_t*>(ws + den_off), levels, kp.flags);
+      ++g_launch_count;
+      KParams kf = kp;
+      kf.fixup = 1;
+      if (int32_t rc = cuda_rc(launch_sims(kf, sc, K, a.st))) return rc;
+    }
     bisect_update_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, reinterpret_cast<const uint32_t*>(ws + att_off),
                                                reinterpret_cast<const uint32_t*>(ws + den_off), levels, next_levels);
     ++g_launch_count;

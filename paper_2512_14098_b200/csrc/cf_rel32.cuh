@@ -223,6 +223,31 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   produce_tile<CMAX>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
   __syncthreads();
 
+  // the origin moves forward by delta: every stage base goes to max(earliest free time, new origin)
+  // and the stage's heap is re-keyed (keys below the new base are clamped to it: DESIGN.md 5.2)
+  auto rebase_all = [&](uint64_t delta) {
+    for (uint32_t s = 0; s < n_stages; ++s) {
+      const uint32_t sa = st_sa + s * 512u;
+      const uint4 st = lds128(sa);
+      const uint64_t base = ((uint64_t)st.y << 32) | st.x;
+      const uint64_t fmin = base + st.z;
+      const uint64_t nb = fmin > delta ? fmin : delta;  // new base, still relative to the old origin
+      const uint64_t shift = nb - base;                 // >= root key: the new root key is 0
+      const uint64_t nbr = nb - delta;                  // ... relative to the new origin
+      sts128(sa, make_uint4((uint32_t)nbr, (uint32_t)(nbr >> 32), 0u, st.w));
+      const uint32_t sh4 = shift >= (1ull << 30) ? 0xfffffffcu : ((uint32_t)shift << 2);
+      const uint32_t nq = st.w >> 16, ha = heap_sa + (st.w & 0xffffu) * 512u;
+      if (sh4 != 0u)
+        for (uint32_t j = 0; j < nq; ++j) {
+          uint4 q = lds128(ha + j * 512u);
+          q.x = rebase_packed(q.x, sh4, 0u); q.y = rebase_packed(q.y, sh4, 1u);
+          q.z = rebase_packed(q.z, sh4, 2u); q.w = rebase_packed(q.w, sh4, 3u);
+          sts128(ha + j * 512u, q);
+        }
+    }
+  };
+  uint32_t flush_idx = 0;  // requests [flush_idx, current) are accumulated in dep relative to origin
+
   for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
     if (tile_idx + 1 < n_tiles)
       produce_tile<CMAX>(prm, cta.variant, trial, variant, tile_idx + 1, tiles, totals, cnt_s, tid, warp, lane);
@@ -233,30 +258,13 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
       // ---- tile prologue: move the origin to the arrival of the last request before the tile,
       //      every stage base to max(earliest free time, origin), and re-key the stage's heap
       const uint64_t acc0 = tile_base * (uint64_t)period + 32768ull;  // wraps only if R17 fails later
-      const uint32_t r0 = (uint32_t)acc0 & 0xffffu;
+      // a3 constant of this lane: A_n - O = (C + d_n * period) >> 16 (C = the low 16 bits of acc0
+      // while O is the tile origin; moving the origin forward by m microseconds subtracts m << 16)
+      uint64_t C = acc0 & 0xffffull;
       if (tile_idx != 0) {
         const uint64_t o_new = acc0 >> 16;
-        const uint64_t delta = o_new - origin;
+        rebase_all(o_new - origin);
         origin = o_new;
-        for (uint32_t s = 0; s < n_stages; ++s) {
-          const uint32_t sa = st_sa + s * 512u;
-          const uint4 st = lds128(sa);
-          const uint64_t base = ((uint64_t)st.y << 32) | st.x;
-          const uint64_t fmin = base + st.z;
-          const uint64_t nb = fmin > delta ? fmin : delta;  // new base, still relative to the old origin
-          const uint64_t shift = nb - base;                 // >= root key: the new root key is 0
-          const uint64_t nbr = nb - delta;                  // ... relative to the new origin
-          sts128(sa, make_uint4((uint32_t)nbr, (uint32_t)(nbr >> 32), 0u, st.w));
-          const uint32_t sh4 = shift >= (1ull << 30) ? 0xfffffffcu : ((uint32_t)shift << 2);
-          const uint32_t nq = st.w >> 16, ha = heap_sa + (st.w & 0xffffu) * 512u;
-          if (sh4 != 0u)
-            for (uint32_t j = 0; j < nq; ++j) {
-              uint4 q = lds128(ha + j * 512u);
-              q.x = rebase_packed(q.x, sh4, 0u); q.y = rebase_packed(q.y, sh4, 1u);
-              q.z = rebase_packed(q.z, sh4, 2u); q.w = rebase_packed(q.w, sh4, 3u);
-              sts128(ha + j * 512u, q);
-            }
-        }
       }
       uint32_t hlo = 0, hhi = 0;
       uint64_t dep = 0, mk = 0;
@@ -313,12 +321,16 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         // stage's top heap quad before the 64-bit max/add chain.
         const uint32_t wb_sa = smem_sa + SL::wbuf + (uint32_t)warp * 32u * kW * 16u;
         // one request: the record is in (w0..w3); the next record is loaded into (n0..n3).
-        // NARROW: every time of this chunk provably fits 32 bits (see the bound below): x, the free
-        // times and the SLO test are 32-bit; otherwise the running departure x is 64-bit.
+        // Mode 0 (narrow): every time of this chunk provably fits 32 bits (see the bound below): x,
+        // the free times and the SLO test are 32-bit. Mode 1: the running departure x is 64-bit.
+        // Mode 2 (sparse arrivals): as mode 1, and a lane whose arrival is 2^29 us or more past its
+        // origin first moves its origin to that arrival (a private, exact rebase), so that keys and
+        // arrival offsets stay small however long the gaps are.
         uint32_t kmax = 0, mk32 = 0;
-        auto request = [&](auto narrow_tag, const uint4& w0, const uint4& w1, const uint4& w2, const uint4& w3,
+        auto request = [&](auto mode_tag, const uint4& w0, const uint4& w1, const uint4& w2, const uint4& w3,
                            uint4& n0w, uint4& n1w, uint4& n2w, uint4& n3w, int r) {
-          constexpr bool NARROW = decltype(narrow_tag)::value;
+          constexpr int MODE = decltype(mode_tag)::value;
+          constexpr bool NARROW = MODE == 0;
           using X = typename std::conditional<NARROW, uint32_t, uint64_t>::type;
           uint32_t sid = w1.x & 0xffu;
           uint4 st = make_uint4(0, 0, 0, 0);
@@ -329,8 +341,23 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
             if (kW > 2) n2w = lds128(na + 32u);
             if (kW > 3) n3w = lds128(na + 48u);
           }
-          // a3: A - O = (r0 + d * period) >> 16
-          const uint32_t a = (uint32_t)(mad_wide_u32(w0.x, period, (uint64_t)r0) >> 16);
+          // a3: A - O = (C + d * period) >> 16
+          uint64_t a64 = mad_wide_u32(w0.x, period, C) >> 16;
+          if (MODE == 2 && a64 >= (1ull << 29)) {
+            const uint32_t idx = nc0 + (uint32_t)r;  // requests [flush_idx, idx) are in dep
+            dep_sum += dep + (uint64_t)(idx - flush_idx) * origin;
+            flush_idx = idx;
+            dep = 0;
+            if (origin + mk > makespan) makespan = origin + mk;
+            mk = mk > a64 ? mk - a64 : 0;
+            rebase_all(a64);
+            origin += a64;
+            C -= a64 << 16;
+            a64 = 0;
+            // the state record of the first visit was loaded before the rebase: reload it
+            if ((w1.x & 0xffu) != 0xffu) st = lds128(st_sa + (w1.x & 0xffu) * 512u);
+          }
+          const uint32_t a = (uint32_t)a64;
           X x = a;
 #pragma unroll
           for (int j = 0; j < VMAX; ++j) {
@@ -381,10 +408,11 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         // Bound for the chunk: every departure is at most M + (all services and hops of the chunk),
         // M = max(latest departure so far, last arrival of the chunk), both relative to the origin
         // (induction over x = max(arrival, F) + S; every free time is some earlier departure).
-        const uint32_t a_last = (uint32_t)(mad_wide_u32((uint32_t)(last_cu - tile_base), period, (uint64_t)r0) >> 16);
+        const uint64_t a_last = mad_wide_u32((uint32_t)(last_cu - tile_base), period, C) >> 16;
         uint64_t seen = makespan > origin ? makespan - origin : 0;
         if (mk > seen) seen = mk;
         if (a_last > seen) seen = a_last;
+        const bool sparse = __any_sync(kFull, a_last >= (1ull << 29));
         const bool narrow = __all_sync(kFull, !chunk_long && seen + chunk_work < 0xffffffffull);
         uint4 a0 = lds128(wb_sa), a1 = lds128(wb_sa + 16u);
         uint4 a2 = make_uint4(0, 0, 0, 0), a3 = make_uint4(0, 0, 0, 0);
@@ -392,8 +420,15 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         if (kW > 3) a3 = lds128(wb_sa + 48u);
         uint4 b0, b1, b2 = make_uint4(0, 0, 0, 0), b3 = make_uint4(0, 0, 0, 0);
         int r = 0;
-        if (narrow) {
-          const std::true_type tag;
+        if (sparse) {
+          const std::integral_constant<int, 2> tag;
+#pragma unroll 1
+          for (; r < n_here; ++r) {
+            request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
+            a0 = b0; a1 = b1; a2 = b2; a3 = b3;
+          }
+        } else if (narrow) {
+          const std::integral_constant<int, 0> tag;
 #pragma unroll 1
           for (; r + 1 < n_here; r += 2) {  // two requests per trip: the record registers ping-pong
             request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
@@ -403,7 +438,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           if (kmax >= kKeyLimit) flagged = true;
           if (mk32 > mk) mk = mk32;
         } else {
-          const std::false_type tag;
+          const std::integral_constant<int, 1> tag;
 #pragma unroll 1
           for (; r + 1 < n_here; r += 2) {
             request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
@@ -415,10 +450,10 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         cu_base += totals[buf * kChunks + ch];
       }
       // ---- tile epilogue: absolute outputs, window checks
-      const uint32_t n_in_tile = min((uint32_t)kTile, prm.N - n0);
-      dep_sum += dep + (uint64_t)n_in_tile * origin;
+      const uint32_t idx_end = min(n0 + (uint32_t)kTile, prm.N);
+      dep_sum += dep + (uint64_t)(idx_end - flush_idx) * origin;
+      flush_idx = idx_end;
       makespan = max(makespan, origin + mk);
-      if (mad_wide_u32((uint32_t)(last_cu - tile_base), period, (uint64_t)r0) >> 47) flagged = true;
       tile_base = last_cu;
 #pragma unroll
       for (int t = 0; t < 4; ++t) {

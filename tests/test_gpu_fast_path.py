@@ -69,12 +69,25 @@ def test_key_window_exit_goes_through_the_fixup_pass(cf, orc):
                   (1000, 500, 200_000))
     wide = eval_both_modes(cf, orc, w)
     assert wide > 0
-    # a tile of 128 requests spanning more than 2^31 us (rate 1 milli-request/s)
-    w = one_stage(W.lognormal_qtab(50_000.0, 0.5), W.exponential_qtab(65536.0), 400, (1, 3), (1, 8, 5000))
-    assert eval_both_modes(cf, orc, w) > 0
     # a tile spanning more than 2^32 gap units
     w = one_stage(W.constant_qtab(700), W.constant_qtab(2**31 - 1), 300, (1, 2), (1_000_000, 1_000_000_000))
     assert eval_both_modes(cf, orc, w) > 0
+
+
+def test_sparse_arrivals_stay_on_the_fast_path(cf, orc):
+    # rates down to 1 milli-request/s: consecutive arrivals are up to hours apart, a tile of 128
+    # requests spans far more than 2^31 us; lanes move their origin request by request instead
+    w = one_stage(W.lognormal_qtab(50_000.0, 0.5), W.exponential_qtab(65536.0), 400, (1, 3), (1, 8, 5000))
+    assert eval_both_modes(cf, orc, w) == 0
+    # the same with long services on many replicas (a mix of busy and idle replicas at every arrival)
+    w = one_stage(W.lognormal_qtab(5_000_000.0, 0.5), W.gamma_qtab(1.0 / 9.0, 65536.0), 900, (2, 7, 40),
+                  (1, 3, 40, 700), L=(40_000_000,))
+    assert eval_both_modes(cf, orc, w) == 0
+    # multi-stage graph with an edge delay, rates from sparse to overloaded in one call
+    w2 = W.config2_omni(n_req=500, n_trials=2, n_rates=2, vectors_per_pattern=2, n_patterns=32)
+    w2.graph.edge_delay_us = 10_000
+    w2.rate_mrps = np.tile(np.array([[1, 30, 900, 60_000]], dtype=np.uint32), (w2.plans.n_plans, 1))
+    assert eval_both_modes(cf, orc, w2) == 0
 
 
 def test_unbounded_waits_stay_on_the_fast_path(cf, orc):

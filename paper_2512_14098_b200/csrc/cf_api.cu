@@ -121,25 +121,34 @@ struct Schedule {
   uint32_t smem_bytes = 0;       // dynamic shared memory of the 64-bit launch
   uint32_t smem_bytes32 = 0;     // ... of the 32-bit launch
   uint32_t ctas_per_sm = 1;
+  int warps_per_cta = 8;         // 4 or 8 (template choice of both kernels)
 };
 
-uint32_t fixed_smem(int vmax, int cmax) {
+template <int W>
+uint32_t fixed_smem_w(int vmax, int cmax) {
   if (cmax <= 6) {
-    if (vmax <= 2) return SmemLayout<2, 6>::fixed_bytes;
-    if (vmax <= 6) return SmemLayout<6, 6>::fixed_bytes;
-    return SmemLayout<8, 6>::fixed_bytes;
+    if (vmax <= 2) return SmemLayout<2, 6, W>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout<6, 6, W>::fixed_bytes;
+    return SmemLayout<8, 6, W>::fixed_bytes;
   }
-  return SmemLayout<8, 8>::fixed_bytes;
+  return SmemLayout<8, 8, W>::fixed_bytes;
+}
+uint32_t fixed_smem(int vmax, int cmax, int warps) {
+  return warps == 4 ? fixed_smem_w<4>(vmax, cmax) : fixed_smem_w<8>(vmax, cmax);
 }
 
-uint32_t fixed_smem32(int vmax, int cmax) {
+template <int W>
+uint32_t fixed_smem32_w(int vmax, int cmax) {
   if (cmax <= 6) {
-    if (vmax <= 2) return SmemLayout32<2, 6>::fixed_bytes;
-    if (vmax <= 4) return SmemLayout32<4, 6>::fixed_bytes;
-    if (vmax <= 6) return SmemLayout32<6, 6>::fixed_bytes;
-    return SmemLayout32<8, 6>::fixed_bytes;
+    if (vmax <= 2) return SmemLayout32<2, 6, W>::fixed_bytes;
+    if (vmax <= 4) return SmemLayout32<4, 6, W>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout32<6, 6, W>::fixed_bytes;
+    return SmemLayout32<8, 6, W>::fixed_bytes;
   }
-  return SmemLayout32<8, 8>::fixed_bytes;
+  return SmemLayout32<8, 8, W>::fixed_bytes;
+}
+uint32_t fixed_smem32(int vmax, int cmax, int warps) {
+  return warps == 4 ? fixed_smem32_w<4>(vmax, cmax) : fixed_smem32_w<8>(vmax, cmax);
 }
 
 // registers per thread of the kernel variant the schedule selects (occupancy model of the packing)
@@ -149,7 +158,7 @@ int kernel_regs32(int vmax, int cmax);
 // Simulations -> warps -> thread blocks.
 //  * a warp holds <= 32 simulations of one topology and one stream variant; within a topology plans
 //    are ordered by heap footprint so that a warp's lanes need similar amounts of shared memory;
-//  * a thread block holds <= kWarpsPerCta warps of one variant whose heap regions fit a common
+//  * a thread block holds <= warps_per_cta (4 or 8) warps of one variant whose heap regions fit a common
 //    budget; the budget (= blocks per SM) is chosen to maximise resident warps per SM;
 //  * ONE launch covers everything; blocks are ordered heaviest first so the tail is short.
 // only_plan: schedule just that plan (cf_trace_sim); plan_variant: stream variant per plan.
@@ -188,7 +197,13 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   sc.cmax = g->n_comp <= 6 ? 6 : 8;
   sc.vmax = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 6 ? 6 : 8));
   sc.vmax32 = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 4 ? 4 : (maxV <= 6 ? 6 : 8)));
-  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax), fixed_f = fixed_smem32(sc.vmax32, sc.cmax);
+  // 8 warps per block amortise the tile over more simulations and win when a warp's lanes are
+  // alike (>= 8 rates per plan); with many different plans per warp (bisection passes, few rates)
+  // warps of a block drift apart between the per-tile barriers and 4 per block are faster (measured)
+  sc.warps_per_cta = R >= 8 ? 8 : 4;
+  const uint32_t kWarpsPerCta = (uint32_t)sc.warps_per_cta;
+  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax, sc.warps_per_cta),
+                 fixed_f = fixed_smem32(sc.vmax32, sc.cmax, sc.warps_per_cta);
   const uint32_t fixed = fast ? fixed_f : fixed_w;  // the layout that is packed for occupancy
 
   std::vector<uint32_t> order;
@@ -314,7 +329,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
     while (w < winfo.size()) {
       CtaDesc cd{(uint32_t)w, 0, winfo[w].variant, 0, 0};
       uint32_t packed = 0;  // heap bytes of the layout being packed
-      while (w < winfo.size() && cd.n_warps < (uint32_t)kWarpsPerCta && winfo[w].variant == cd.variant &&
+      while (w < winfo.size() && cd.n_warps < kWarpsPerCta && winfo[w].variant == cd.variant &&
              (cd.n_warps == 0 || (fixed + packed + winfo[w].heap_bytes <= budget &&
                                   fixed_w + cd.heap_bytes + winfo[w].heap_w <= kMaxSmem))) {
         if (assign) {
@@ -444,16 +459,16 @@ void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool
 // ------------------------------------------------------------------------------------------------
 // launches
 // ------------------------------------------------------------------------------------------------
-template <int VMAX, int CMAX, bool HAS_DELAY>
+template <int VMAX, int CMAX, bool HAS_DELAY, int W>
 cudaError_t launch_one(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY>;
+  auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY, W>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
   if (e != cudaSuccess) return e;
   kp.k_launch = n_trials;
   // 1-D grid, block b = (CTA b / n_trials, trial b % n_trials): <= 2^31-1 blocks
   const uint64_t blocks = (uint64_t)sc.ctas.size() * n_trials;
   if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-  kern<<<(uint32_t)blocks, kThreads, sc.smem_bytes, st>>>(kp, 0u);
+  kern<<<(uint32_t)blocks, W * 32, sc.smem_bytes, st>>>(kp, 0u);
   ++g_launch_count;
   return cudaGetLastError();
 }
@@ -462,7 +477,7 @@ template <int VMAX, int CMAX>
 int regs_of() {
   static int regs = [] {
     cudaFuncAttributes a;
-    if (cudaFuncGetAttributes(&a, cf_sim_kernel<VMAX, CMAX, false>) != cudaSuccess) {
+    if (cudaFuncGetAttributes(&a, cf_sim_kernel<VMAX, CMAX, false, 8>) != cudaSuccess) {
       cudaGetLastError();
       return VMAX <= 2 ? 64 : 128;  // ptxas figures of this build; used when no device is present
     }
@@ -471,12 +486,19 @@ int regs_of() {
   return regs;
 }
 
-cudaError_t launch_sims(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+template <int VMAX, int CMAX>
+cudaError_t launch_v(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
   const bool d = kp.edge_delay != 0;
-  if (sc.cmax == 8) return d ? launch_one<8, 8, true>(kp, sc, n_trials, st) : launch_one<8, 8, false>(kp, sc, n_trials, st);
-  if (sc.vmax == 2) return d ? launch_one<2, 6, true>(kp, sc, n_trials, st) : launch_one<2, 6, false>(kp, sc, n_trials, st);
-  if (sc.vmax == 6) return d ? launch_one<6, 6, true>(kp, sc, n_trials, st) : launch_one<6, 6, false>(kp, sc, n_trials, st);
-  return d ? launch_one<8, 6, true>(kp, sc, n_trials, st) : launch_one<8, 6, false>(kp, sc, n_trials, st);
+  if (sc.warps_per_cta == 4)
+    return d ? launch_one<VMAX, CMAX, true, 4>(kp, sc, n_trials, st) : launch_one<VMAX, CMAX, false, 4>(kp, sc, n_trials, st);
+  return d ? launch_one<VMAX, CMAX, true, 8>(kp, sc, n_trials, st) : launch_one<VMAX, CMAX, false, 8>(kp, sc, n_trials, st);
+}
+
+cudaError_t launch_sims(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  if (sc.cmax == 8) return launch_v<8, 8>(kp, sc, n_trials, st);
+  if (sc.vmax == 2) return launch_v<2, 6>(kp, sc, n_trials, st);
+  if (sc.vmax == 6) return launch_v<6, 6>(kp, sc, n_trials, st);
+  return launch_v<8, 6>(kp, sc, n_trials, st);
 }
 
 int kernel_regs(int vmax, int cmax) {
@@ -487,15 +509,15 @@ int kernel_regs(int vmax, int cmax) {
 }
 
 // ---- the 32-bit fast kernel (cf_rel32.cuh) ---------------------------------------------------------
-template <int VMAX, int CMAX, bool HAS_DELAY, bool T8>
+template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int W>
 cudaError_t launch_one32(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  auto kern = cf_sim32_kernel<VMAX, CMAX, HAS_DELAY, T8>;
+  auto kern = cf_sim32_kernel<VMAX, CMAX, HAS_DELAY, T8, W>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
   if (e != cudaSuccess) return e;
   kp.k_launch = n_trials;
   const uint64_t blocks = (uint64_t)sc.ctas.size() * n_trials;
   if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-  kern<<<(uint32_t)blocks, kThreads, sc.smem_bytes32, st>>>(kp);
+  kern<<<(uint32_t)blocks, W * 32, sc.smem_bytes32, st>>>(kp);
   ++g_launch_count;
   return cudaGetLastError();
 }
@@ -504,7 +526,7 @@ template <int VMAX, int CMAX>
 int regs_of32() {
   static int regs = [] {
     cudaFuncAttributes a;
-    if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false, true>) != cudaSuccess) {
+    if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false, true, 8>) != cudaSuccess) {
       cudaGetLastError();
       return 128;  // __launch_bounds__ cap of this build; used when no device is present
     }
@@ -521,11 +543,16 @@ int kernel_regs32(int vmax, int cmax) {
   return regs_of32<8, 6>();
 }
 
+template <int VMAX, int CMAX, int W>
+cudaError_t launch_w32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  const bool d = kp.edge_delay != 0, t8 = kp.T > 4;
+  if (d) return t8 ? launch_one32<VMAX, CMAX, true, true, W>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, true, false, W>(kp, sc, n_trials, st);
+  return t8 ? launch_one32<VMAX, CMAX, false, true, W>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, false, false, W>(kp, sc, n_trials, st);
+}
+
 template <int VMAX, int CMAX>
 cudaError_t launch_v32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  const bool d = kp.edge_delay != 0, t8 = kp.T > 4;
-  if (d) return t8 ? launch_one32<VMAX, CMAX, true, true>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, true, false>(kp, sc, n_trials, st);
-  return t8 ? launch_one32<VMAX, CMAX, false, true>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, false, false>(kp, sc, n_trials, st);
+  return sc.warps_per_cta == 4 ? launch_w32<VMAX, CMAX, 4>(kp, sc, n_trials, st) : launch_w32<VMAX, CMAX, 8>(kp, sc, n_trials, st);
 }
 
 cudaError_t launch_sims32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {

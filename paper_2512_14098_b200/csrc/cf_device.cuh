@@ -18,11 +18,8 @@
 
 namespace cfk {
 
-#ifndef CF_WARPS
-#define CF_WARPS 8
-#endif
-constexpr int kWarpsPerCta = CF_WARPS;
-constexpr int kThreads = kWarpsPerCta * 32;
+// warps per thread block: a template parameter of the kernels (4 or 8, chosen by the schedule)
+constexpr int kMaxWarpsPerCta = 8;
 constexpr int kTile = 128;              // requests per CTA tile
 constexpr int kChunks = kTile / 32;     // 32-request chunks per tile
 constexpr int64_t kInf = INT64_MAX;
@@ -211,7 +208,7 @@ __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_
 // Producer of one CTA tile (kTile requests) into buffer tile_idx & 1: in-register Philox draws
 // (a1-a3) or a copy of the materialised stream (a10). Shared by both simulation kernels.
 // ------------------------------------------------------------------------------------------------
-template <int CMAX>
+template <int CMAX, int WARPS>
 __device__ __forceinline__ void produce_tile(const KParams& prm, uint32_t cta_variant, uint32_t trial,
                                              uint32_t variant, uint32_t tile_idx, uint4* tiles,
                                              uint64_t* totals, uint32_t* cnt_s, int tid, int warp,
@@ -220,7 +217,7 @@ __device__ __forceinline__ void produce_tile(const KParams& prm, uint32_t cta_va
   uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
   const uint32_t n0 = tile_idx * kTile;
   if (prm.stream == nullptr) {
-    for (int ch = warp; ch < kChunks; ch += kWarpsPerCta)
+    for (int ch = warp; ch < kChunks; ch += WARPS)
       produce_chunk_philox<CMAX>(prm, n0 + ch * 32, trial, variant,
                                  tb + ch * 32 * CompRec<CMAX>::kWords, totals + buf * kChunks + ch,
                                  cnt_s, lane);
@@ -228,7 +225,7 @@ __device__ __forceinline__ void produce_tile(const KParams& prm, uint32_t cta_va
     // a10: copy kTile 32-byte records (2 x uint4 each) from the materialised stream; cu is absolute
     const uint4* src = prm.stream + ((size_t)(cta_variant * prm.K + trial) * prm.N + n0) * 2;
     const uint32_t n_words = min((uint32_t)kTile, prm.N - n0) * 2u;
-    for (uint32_t w = tid; w < n_words; w += kThreads) {
+    for (uint32_t w = tid; w < n_words; w += WARPS * 32) {
       const uint4 v = __ldg(src + w);
       tb[w] = v;
       if ((w & 1u) == 0u) atomicAdd(&cnt_s[v.y >> 24], 1u);
@@ -275,7 +272,7 @@ __device__ __forceinline__ void heap_replace_min(uint8_t* smem, int64_t& root, u
 // The simulation kernel. grid = (CTAs of this launch, K trials); block = kThreads.
 // Dynamic shared memory: [tiles 2 x kTile x CompRec][chunk totals][cnt][L][warp stage buffers][heaps]
 // ------------------------------------------------------------------------------------------------
-template <int VMAX, int CMAX>
+template <int VMAX, int CMAX, int WARPS>
 struct SmemLayout {
   static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
   static constexpr uint32_t kStageRecBytes = StageRec<VMAX>::kWords * 16;
@@ -284,14 +281,14 @@ struct SmemLayout {
   static constexpr uint32_t cnt = totals + 2 * kChunks * 8;
   static constexpr uint32_t lus = cnt + 8 * 4;
   static constexpr uint32_t wbuf = lus + 8 * 8;
-  static constexpr uint32_t heaps = wbuf + kWarpsPerCta * 32 * kStageRecBytes;
+  static constexpr uint32_t heaps = wbuf + WARPS * 32 * kStageRecBytes;
   static constexpr uint32_t fixed_bytes = heaps;
 };
 
-template <int VMAX, int CMAX, bool HAS_DELAY>
-__global__ void __launch_bounds__(kThreads)
+template <int VMAX, int CMAX, bool HAS_DELAY, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
 cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
-  using SL = SmemLayout<VMAX, CMAX>;
+  using SL = SmemLayout<VMAX, CMAX, WARPS>;
   extern __shared__ __align__(16) uint8_t smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t trial = prm.trial_base + blockIdx.x % prm.k_launch;
@@ -371,7 +368,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   // ---- producer for one tile -----------------------------------------------------------------
   const uint32_t n_tiles = (prm.N + kTile - 1) / kTile;
   auto produce = [&](uint32_t tile_idx) {
-    produce_tile<CMAX>(prm, cta.variant, trial, variant, tile_idx, tiles, totals, cnt_s, tid, warp, lane);
+    produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, tile_idx, tiles, totals, cnt_s, tid, warp, lane);
   };
 
   __syncthreads();

@@ -25,10 +25,13 @@
 // system arrival >= origin, so a replica that is free before the origin is simply "free"
 // (max(arrival, F) = arrival either way) -- DESIGN.md 5.2.
 //
+// A lane whose arrivals are sparse (an arrival 2^29 us or more past its origin) moves its own origin
+// to that arrival in the middle of a tile (same exact rebase), so any rate down to 1 mrps stays here.
+//
 // A lane leaves the fast path when a key does not fit 30 bits (free times of ONE stage more than
-// 17.9 minutes apart), a tile spans >= 2^31 us or >= 2^32 gap units, the rate is outside [1, 1e9]
-// or the R17 horizon is exceeded. It then sets flags[slot] and writes nothing; the 64-bit kernel
-// of cf_device.cuh runs in fixup mode over exactly those simulations. Results are bit-identical.
+// 17.9 minutes apart), a tile spans >= 2^32 gap units, the rate is outside [1, 1e9] or the R17
+// horizon is exceeded. It then sets flags[slot] and writes nothing; the 64-bit kernel of
+// cf_device.cuh runs in fixup mode over exactly those simulations. Results are bit-identical.
 #pragma once
 #include <type_traits>
 
@@ -51,7 +54,7 @@ struct StageRec32 {
 };
 
 // Per-lane, per-stage state record (16 B): { base_lo, base_hi, root key, heap_row | nq << 16 }
-template <int VMAX, int CMAX>
+template <int VMAX, int CMAX, int WARPS>
 struct SmemLayout32 {
   static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
   static constexpr uint32_t kStageRecBytes = StageRec32<VMAX>::kWords * 16;
@@ -61,8 +64,8 @@ struct SmemLayout32 {
   static constexpr uint32_t l32 = cnt + 8 * 4;
   static constexpr uint32_t inc = l32 + 8 * 4;  // 8 x {lo, hi}
   static constexpr uint32_t wbuf = inc + 8 * 8;
-  static constexpr uint32_t state = wbuf + kWarpsPerCta * 32 * kStageRecBytes;  // [warp][stage][lane] x 16 B
-  static constexpr uint32_t heaps = state + kWarpsPerCta * VMAX * 512;
+  static constexpr uint32_t state = wbuf + WARPS * 32 * kStageRecBytes;  // [warp][stage][lane] x 16 B
+  static constexpr uint32_t heaps = state + WARPS * VMAX * 512;
   static constexpr uint32_t fixed_bytes = heaps;
 };
 
@@ -119,14 +122,12 @@ __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint
   return p == kInf32 ? kInf32 : v;
 }
 
-// T8: more than 4 request types (a second word of hit-counter byte fields)
-template <int VMAX, int CMAX, bool HAS_DELAY, bool T8>
-#ifndef CF_MINB32
-#define CF_MINB32 2
-#endif
-__global__ void __launch_bounds__(kThreads, CF_MINB32)
+// T8: more than 4 request types (a second word of hit-counter byte fields); WARPS per thread block
+// (16 warps per SM either way: 124-128 registers per thread)
+template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, 16 / WARPS)
 cf_sim32_kernel(const __grid_constant__ KParams prm) {
-  using SL = SmemLayout32<VMAX, CMAX>;
+  using SL = SmemLayout32<VMAX, CMAX, WARPS>;
   constexpr int kW = StageRec32<VMAX>::kWords;
   extern __shared__ __align__(16) uint8_t smem[];
   const uint32_t smem_sa = (uint32_t)__cvta_generic_to_shared(smem);
@@ -220,7 +221,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   // a warp whose lanes all skip (closed brackets) only helps producing the tiles
   const bool consume = __any_sync(kFull, wanted);
   __syncthreads();
-  produce_tile<CMAX>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
+  produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
   __syncthreads();
 
   // the origin moves forward by delta: every stage base goes to max(earliest free time, new origin)
@@ -250,7 +251,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
 
   for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
     if (tile_idx + 1 < n_tiles)
-      produce_tile<CMAX>(prm, cta.variant, trial, variant, tile_idx + 1, tiles, totals, cnt_s, tid, warp, lane);
+      produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, tile_idx + 1, tiles, totals, cnt_s, tid, warp, lane);
     if (consume) {
       const uint32_t buf = tile_idx & 1u;
       const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;

@@ -20,7 +20,6 @@ namespace {
 
 thread_local uint32_t g_launch_count = 0;
 thread_local uint32_t g_kernel_mode = 0;  // cf_debug_kernel_mode: 0 auto, 1 = 64-bit kernel only
-thread_local uint32_t g_rate_major = 0;   // bisection lane order (probe knob, see build_schedule)
 thread_local uint32_t g_spec_depth = 0;   // cf_debug_bisect_depth: 0 auto, 1..4 = bisection steps per pass
 
 constexpr size_t kAlign = 256;
@@ -166,7 +165,7 @@ int kernel_regs32(int vmax, int cmax);
 // the same warps and blocks with its own, larger heap offsets.
 int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
                        const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
-                       bool fast, bool rate_major, Schedule* out) {
+                       bool fast, Schedule* out) {
   const uint32_t P = pl->n_plans, MS = pl->max_stages;
   Schedule& sc = *out;
   sc.plan_c.assign((size_t)P * 8, 1);
@@ -268,16 +267,10 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
            plan_topo[order[j]] == plan_topo[order[i]])
       ++j;
     const size_t sim0 = sc.sims.size();
-    // plan-major: the R rates of a plan share replica counts (uniform heap depths in a warp);
-    // rate-major (bisection): the same tree node of many plans, so that the simulations that
-    // leave the fast window (the overloaded nodes) cluster in few warps
-    if (rate_major) {
-      for (uint32_t r = 0; r < R; ++r)
-        for (size_t q = i; q < j; ++q) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
-    } else {
-      for (size_t q = i; q < j; ++q)
-        for (uint32_t r = 0; r < R; ++r) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
-    }
+    // plan-major: the R rates of a plan share replica counts (uniform heap depths in a warp); the
+    // same tree node of many plans per warp (rate-major) measured 10 % slower on config 4
+    for (size_t q = i; q < j; ++q)
+      for (uint32_t r = 0; r < R; ++r) sc.sims.push_back(SimDesc{order[q], order[q] * R + r});
     const size_t n_group = sc.sims.size() - sim0;
     const TopoDesc& td = sc.topos[plan_topo[order[i]]];
     for (size_t w0 = 0; w0 < n_group; w0 += 32) {
@@ -862,7 +855,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   const bool fast = fast_path_ok(a.g);
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, false, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);  // status block
@@ -911,8 +904,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   depth = std::min(depth, std::max(1u, a.n_steps));
   const uint32_t R = (1u << depth) - 1u;
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast,
-                                  g_rate_major != 0, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);
@@ -1098,7 +1090,7 @@ int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint3
   if (int32_t rc = check_workspace(workspace, workspace_bytes, cf_workspace_bytes(g, pl, 1))) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   Schedule sc;
-  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, false, false, &sc)) return rc;
+  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, false, &sc)) return rc;
   // the single simulation reads rate slot `plan` (pr = plan*1 + 0): upload a full-length rate array
   Blob blob;
   blob.reserve(kAlign);
@@ -1151,10 +1143,6 @@ int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_
 }
 
 int32_t cf_debug_bisect_depth(uint32_t depth) {
-  if (depth >= 16) {  // 16/17: plan-major / rate-major lane order of the bisection passes
-    g_rate_major = depth & 1u;
-    return CF_OK;
-  }
   if (depth > kMaxSpecDepth) return CF_ERR_ARG;
   g_spec_depth = depth;
   return CF_OK;

@@ -1,0 +1,100 @@
+"""Seeded random graphs, plans, tables and rates (from sparse to overloaded) through both kernels,
+bit for bit against the CPU oracle: the cross-product of the fast kernel's paths (32-bit / 64-bit /
+sparse-arrival request bodies, tile rebases, heap depths 0..3, edge delay, 1..8 types and stages)
+that the hand-written cases do not enumerate."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2512_14098_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+NT = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def cf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2512_14098_b200 import binding
+    yield binding
+    binding.cf_debug_kernel_mode(0)
+    binding.cf_debug_bisect_depth(0)
+
+
+def random_case(seed):
+    rng = np.random.default_rng(seed)
+    C = int(rng.integers(1, 9))
+    T = int(rng.integers(1, 9))
+    N = int(rng.integers(1, 700))
+    K = int(rng.integers(1, 4))
+    scale = float(rng.choice([2_000.0, 50_000.0, 3_000_000.0]))  # service scale: ms .. seconds
+    tabs = []
+    for _ in range(C):
+        kind = rng.integers(0, 3)
+        m = scale * float(rng.uniform(0.2, 3.0))
+        tabs.append(W.lognormal_qtab(m, float(rng.uniform(0.2, 0.9))) if kind == 0 else
+                    W.exponential_qtab(m) if kind == 1 else W.constant_qtab(int(m)))
+    masks = [int(rng.integers(0, 1 << C)) for _ in range(T)]
+    if rng.random() < 0.8:
+        masks = [m | (1 << int(rng.integers(0, C))) for m in masks]  # mostly non-empty routes
+    frac = rng.dirichlet(np.ones(T))
+    svc_tab = np.repeat(np.arange(C, dtype=np.uint16), T)
+    arr = W.exponential_qtab(65536.0) if rng.random() < 0.6 else W.gamma_qtab(1.0 / 9.0, 65536.0)
+    edges = [[i, i + 1] for i in range(C - 1)]
+    delay = int(rng.choice([0, 0, 137, 10_000]))
+    g = W.Graph(C, T, N, K, masks, W.mix_thresholds(frac), svc_tab, tabs, arr, edges, edge_delay_us=delay)
+    plan_list = []
+    for _ in range(int(rng.integers(1, 24))):
+        n_cut = int(rng.integers(0, C))
+        cuts = sorted(rng.choice(np.arange(1, C), size=n_cut, replace=False).tolist()) if C > 1 else []
+        bounds = [0] + cuts + [C]
+        plan_list.append([(sum(1 << i for i in range(a, b)), int(rng.choice([1, 1, 2, 3, 5, 6, 9, 21, 22, 40])))
+                          for a, b in zip(bounds, bounds[1:])])
+    pl = W.make_plans(plan_list, max_stages=8)
+    R_p = np.maximum(W.flow_bound_mrps(g, pl), 8)
+    alphas = rng.choice([0.001, 0.02, 0.3, 0.7, 0.95, 1.1, 2.5], size=int(rng.integers(1, 5)), replace=False)
+    rates = np.maximum(W.rate_grid(R_p, list(alphas)), 1).astype(np.uint32)
+    if rng.random() < 0.3:
+        rates[0, 0] = 1  # one milli-request per second
+    L = (scale * rng.uniform(0.5, 30.0, T)).astype(np.int64)
+    slo = W.Slo(L, [9] * T, [10] * T)
+    return W.Workload(f"fuzz{seed}", g, pl, slo, seed=1000 + seed, rate_mrps=rates), R_p
+
+
+@pytest.mark.parametrize("seed", range(64))
+def test_random_eval(cf, orc, seed):
+    w, _ = random_case(seed)
+    assert orc.validate(w.graph, w.plans) == 0
+    want = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, 3, n_threads=NT)
+    for mode in (0, 1):
+        cf.cf_debug_kernel_mode(mode)
+        try:
+            got = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, 3)
+            status = cf.cf_workspace_status(got["workspace"])
+        finally:
+            cf.cf_debug_kernel_mode(0)
+        assert status == want["rc"]
+        np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+        np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+
+
+@pytest.mark.parametrize("seed", range(100, 116))
+def test_random_bisect(cf, orc, seed):
+    w, R_p = random_case(seed)
+    hi = np.minimum(np.ceil(1.5 * np.minimum(R_p, 1e9)), 1_000_000_000).astype(np.uint32)
+    steps = int(np.random.default_rng(seed).integers(1, 22))
+    bo = orc.goodput_bisect(w.graph, w.plans, hi, steps, w.slo, w.seed, n_threads=NT)
+    for depth in (0, 3):
+        cf.cf_debug_bisect_depth(depth)
+        try:
+            b = cf.cf_goodput_bisect(w.graph, w.plans, hi, steps, w.slo, w.seed)
+        finally:
+            cf.cf_debug_bisect_depth(0)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"]), bo["goodput_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])

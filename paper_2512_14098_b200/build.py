@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libcf_b200.so")
 SOURCES = ["cf_api.cu"]
-DEPS = ["cf_api.cu", "cf_device.cuh", os.path.join("..", "..", "include", "cf.h")]
+DEPS = ["cf_api.cu", "cf_device.cuh", "cf_rel32.cuh", "cf_scan.cuh", os.path.join("..", "..", "include", "cf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared"]
 

@@ -13,6 +13,7 @@
 
 #include "../../include/cf.h"
 #include "cf_rel32.cuh"
+#include "cf_scan.cuh"
 
 using namespace cfk;
 
@@ -121,6 +122,10 @@ struct Schedule {
   uint32_t smem_bytes32 = 0;     // ... of the 32-bit launch
   uint32_t ctas_per_sm = 1;
   int warps_per_cta = 8;         // 4 or 8 (template choice of both kernels)
+  // every stage of every plan has one replica: the call runs on the max-plus scan kernel (cf_scan.cuh)
+  bool all_c1 = false;
+  std::vector<uint32_t> plan_topo_v, plan_var_v;  // [P] topology id / stream variant of each plan
+  uint32_t R = 1;
 };
 
 template <int W>
@@ -194,6 +199,17 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
     }
   }
   sc.cmax = g->n_comp <= 6 ? 6 : 8;
+  sc.R = R;
+  sc.plan_topo_v = plan_topo;
+  sc.all_c1 = true;
+  for (uint32_t p = 0; p < P; ++p)
+    for (uint32_t st = 0; st < pl->n_stages[p]; ++st)
+      if (pl->stage_c[(size_t)p * MS + st] != 1) sc.all_c1 = false;
+  // The scan kernel spends a warp (and its own Philox draws) per simulation: 3.6x faster than a
+  // thread per simulation when the call has few simulations (config 0: 32 per call), 5.7x slower
+  // when there are enough to fill the GPU with threads (measured crossover near 9 000 simulations).
+  if ((uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
+  if (only_plan || g_kernel_mode == 1) sc.all_c1 = false;  // traces and the forced 64-bit mode keep the thread-per-simulation path
   sc.vmax = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 6 ? 6 : 8));
   sc.vmax32 = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 4 ? 4 : (maxV <= 6 ? 6 : 8)));
   // 8 warps per block amortise the tile over more simulations and win when a warp's lanes are
@@ -214,6 +230,8 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   };
   for (uint32_t p : order)
     if (variant_of(p) >= std::max(1u, n_variants)) return CF_ERR_ARG;
+  sc.plan_var_v.resize(P);
+  for (uint32_t p = 0; p < P; ++p) sc.plan_var_v[p] = only_plan ? 0u : variant_of(p);
   // (variant, topology, then similar heap depths) -> homogeneous warps. A warp executes every
   // replace-min to the depth of its deepest lane, so plans are ordered by the vector of their
   // stages' heap depths, the most visited stage first (mix-weighted), then by the replica counts.
@@ -427,7 +445,7 @@ size_t fill_graph_params(const cf_graph* g, const cf_slo* slo, uint64_t seed, Bl
   return blob->add(pool.data(), pool.size() * sizeof(int32_t));
 }
 
-struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c; };
+struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c, plan_topo, plan_var; };
 
 SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
   SchedOffsets o;
@@ -436,6 +454,8 @@ SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
   o.warps = blob->add(sc.warps.data(), sc.warps.size() * sizeof(WarpDesc));
   o.ctas = blob->add(sc.ctas.data(), sc.ctas.size() * sizeof(CtaDesc));
   o.plan_c = blob->add(sc.plan_c.data(), sc.plan_c.size() * sizeof(uint16_t));
+  o.plan_topo = blob->add(sc.plan_topo_v.data(), sc.plan_topo_v.size() * sizeof(uint32_t));
+  o.plan_var = blob->add(sc.plan_var_v.data(), sc.plan_var_v.size() * sizeof(uint32_t));
   return o;
 }
 
@@ -446,6 +466,8 @@ void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool
   kp->warps = reinterpret_cast<const WarpDesc*>(ws + o.warps);
   kp->ctas = reinterpret_cast<const CtaDesc*>(ws + o.ctas);
   kp->plan_c = reinterpret_cast<const uint16_t*>(ws + o.plan_c);
+  kp->plan_topo = reinterpret_cast<const uint32_t*>(ws + o.plan_topo);
+  kp->plan_var = reinterpret_cast<const uint32_t*>(ws + o.plan_var);
   kp->status = reinterpret_cast<int32_t*>(ws);
 }
 
@@ -576,7 +598,22 @@ bool fast_path_ok(const cf_graph* g) {
 
 // One pass over the schedule: the 32-bit kernel, then the 64-bit kernel over the simulations that
 // left the 32-bit window (normally none: its blocks exit at once) -- or the 64-bit kernel alone.
+cudaError_t launch_scan(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  kp.k_launch = n_trials;
+  const uint64_t n_sims = (uint64_t)sc.plan_topo_v.size() * sc.R * n_trials;
+  const uint64_t blocks = (n_sims + kScanWarps - 1) / kScanWarps;
+  if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+  const uint32_t* pv = kp.stream ? kp.plan_var : nullptr;
+  if (sc.cmax == 8)
+    cf_scan_kernel<8><<<(uint32_t)blocks, kScanWarps * 32, 0, st>>>(kp, kp.plan_topo, pv, sc.R, (uint32_t)n_sims);
+  else
+    cf_scan_kernel<6><<<(uint32_t)blocks, kScanWarps * 32, 0, st>>>(kp, kp.plan_topo, pv, sc.R, (uint32_t)n_sims);
+  ++g_launch_count;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_pass(KParams kp, const Schedule& sc, uint32_t n_trials, bool fast, cudaStream_t st) {
+  if (sc.all_c1) return launch_scan(kp, sc, n_trials, st);  // one replica everywhere: max-plus scan
   if (!fast) {
     kp.fixup = 0;
     return launch_sims(kp, sc, n_trials, st);
@@ -946,7 +983,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   for (uint32_t step = 0; step < a.n_steps; step += depth) {
     const uint32_t levels = std::min(depth, a.n_steps - step);
     const uint32_t next_levels = std::min(depth, a.n_steps - step - levels);
-    if (!fast) {
+    if (!fast || sc.all_c1) {
       if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, false, a.st))) return rc;
     } else {
       if (int32_t rc = cuda_rc(launch_sims32(kp, sc, K, a.st))) return rc;
@@ -986,7 +1023,7 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   const size_t max_warps = P * R / 32 + P + 1;
   n += align_up(max_warps * sizeof(WarpDesc));
   n += align_up(max_warps * sizeof(CtaDesc));
-  n += align_up(P * 8 * 2);
+  n += align_up(P * 8 * 2) + 2 * align_up(P * 4);
   n += 4 * kAlign + 3 * align_up(P * 4) + align_up(P * Rb * 4);  // bisection: att, lo/hi, probes, tree
   n += align_up(P * Rb * K * T * 2 * 4) + align_up(P * K * T * 2 * 4) + kAlign;  // probe + at_lo counts
   n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch

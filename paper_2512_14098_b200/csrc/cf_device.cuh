@@ -81,6 +81,8 @@ struct KParams {
   const SimDesc* sims;
   const TopoDesc* topos;
   const uint16_t* plan_c;  // [P*8]
+  const uint32_t* plan_topo;  // [P] topology of each plan   (scan kernel)
+  const uint32_t* plan_var;   // [P] stream variant of each plan
   const uint32_t* rates;   // [P*R]
   // outputs
   uint32_t* out_counts;    // [PR][K][T][2]

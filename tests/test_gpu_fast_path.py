@@ -157,3 +157,66 @@ def test_bisection_with_window_exits(cf, orc):
         np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
         np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"]), bo["goodput_mrps"])
         np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
+
+
+# ---------------------------------------------------------------------------------------------
+# calls whose plans have one replica at every stage run on the max-plus scan kernel (cf_scan.cuh)
+# ---------------------------------------------------------------------------------------------
+def all_c1(w):
+    w.plans = W.Plans(w.plans.n_stages, w.plans.stage_mask, np.ones_like(w.plans.stage_c))
+    return w
+
+
+@pytest.mark.parametrize("n_req", [1, 31, 32, 33, 500, 1025])
+def test_scan_kernel_multistage(cf, orc, n_req):
+    w = all_c1(W.config2_omni(n_req=n_req, n_trials=3, n_rates=4, vectors_per_pattern=1))  # 32 topologies
+    w.graph.edge_delay_us = 10_000
+    w.rate_mrps = np.maximum(W.rate_grid(W.flow_bound_mrps(w.graph, w.plans), [0.01, 0.6, 0.95, 1.4]), 1)
+    want = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, 2, n_threads=NT)
+    got = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, 2)
+    assert cf.cf_workspace_status(got["workspace"]) == want["rc"] == 0
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+    np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+    # the thread-per-simulation kernels give the same answer on the same call
+    cf.cf_debug_kernel_mode(1)
+    try:
+        ref = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, 2)
+    finally:
+        cf.cf_debug_kernel_mode(0)
+    np.testing.assert_array_equal(cf.to_numpy_u32(ref["counts"]), want["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u64(ref["dep_sum"]), want["dep_sum"])
+
+
+def test_scan_kernel_stream_bisect_and_ranges(cf, orc):
+    w = all_c1(W.config4_sweep(n_req=900, n_trials=2, n_steps=12, vectors_per_pattern=2, n_variants=3))
+    g, pl = w.graph, w.plans
+    w.plan_variant = ((np.arange(pl.n_plans) // 3) % 3).astype(np.uint32)
+    w.rate_hi_mrps = np.ceil(1.5 * W.flow_bound_mrps(g, pl)).astype(np.uint32)
+    rec = cf.cf_materialize_stream(g, w.seed, 0, w.n_variants)
+    rates = np.maximum(W.rate_grid(W.flow_bound_mrps(g, pl), [0.5, 1.2]), 1)
+    got = cf.cf_eval_plans(g, pl, rates, w.slo, w.seed, stream_records=rec, n_variants=w.n_variants,
+                           plan_variant=w.plan_variant)
+    b = cf.cf_goodput_bisect(g, pl, w.rate_hi_mrps, w.n_steps, w.slo, w.seed, stream_records=rec,
+                             n_variants=w.n_variants, plan_variant=w.plan_variant)
+    for v in range(w.n_variants):
+        idx = np.nonzero(w.plan_variant == v)[0]
+        o = orc.eval_plans(g, pl.subset(idx), rates[idx], w.slo, w.seed, v, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"])[idx], o["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"])[idx], o["dep_sum"])
+        np.testing.assert_array_equal(got["makespan"].cpu().numpy()[idx], o["makespan"])
+        bo = orc.goodput_bisect(g, pl.subset(idx), w.rate_hi_mrps[idx], w.n_steps, w.slo, w.seed, v, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"])[idx], bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"])[idx], bo["goodput_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"])[idx], bo["counts"])
+    # out-of-range rates and the R17 horizon on the scan path
+    w1 = one_stage(W.constant_qtab(5), W.constant_qtab(2**31 - 1), 1 << 12, (1,), (1, 1000, 1_000_000_000), n_trials=1)
+    want = orc.eval_plans(w1.graph, w1.plans, w1.rate_mrps, w1.slo, w1.seed, n_threads=NT)
+    got = cf.cf_eval_plans(w1.graph, w1.plans, w1.rate_mrps, w1.slo, w1.seed)
+    assert cf.cf_workspace_status(got["workspace"]) == want["rc"] == orc.ORC_ERR_RANGE
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    w1.rate_mrps[0, 1] = 0
+    want = orc.eval_plans(w1.graph, w1.plans, w1.rate_mrps, w1.slo, w1.seed, n_threads=NT)
+    got = cf.cf_eval_plans(w1.graph, w1.plans, w1.rate_mrps, w1.slo, w1.seed)
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])

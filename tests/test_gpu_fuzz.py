@@ -54,6 +54,8 @@ def random_case(seed):
         bounds = [0] + cuts + [C]
         plan_list.append([(sum(1 << i for i in range(a, b)), int(rng.choice([1, 1, 2, 3, 5, 6, 9, 21, 22, 40])))
                           for a, b in zip(bounds, bounds[1:])])
+    if rng.random() < 0.25:  # one replica everywhere: the call runs on the max-plus scan kernel
+        plan_list = [[(m, 1) for m, _ in stages] for stages in plan_list]
     pl = W.make_plans(plan_list, max_stages=8)
     R_p = np.maximum(W.flow_bound_mrps(g, pl), 8)
     alphas = rng.choice([0.001, 0.02, 0.3, 0.7, 0.95, 1.1, 2.5], size=int(rng.integers(1, 5)), replace=False)

@@ -225,6 +225,13 @@ def main():
             c["hi"] = c["hi_host"].to(dev)
             c["ws"] = cf.alloc_workspace(w.graph, w.plans, 1)
             c["stream_records"] = cf.cf_materialize_stream(w.graph, w.seed, variant * w.n_variants, w.n_variants)
+            # the a10 producer, timed once on its own (outside the step): records written per second
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            cf.cf_materialize_stream(w.graph, w.seed, variant * w.n_variants, w.n_variants, out=c["stream_records"])
+            e1.record(stream)
+            torch.cuda.synchronize()
+            c["materialize_ms"] = e0.elapsed_time(e1)
         calls.append(c)
 
     launches = [0]
@@ -396,6 +403,8 @@ def main():
                 "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
                 "config": {"workload": workload_name(args.config), "scale": args.scale,
                            "updates_per_step": total_updates, "l2": "flushed between timed steps (256 MiB fill)",
+                           "stream_materialise": next(({"ms": c["materialize_ms"], "GB/s": c["stream_records"].numel() / c["materialize_ms"] / 1e6}
+                                                       for c in calls if "materialize_ms" in c), None),
                            "wide_fixups": wide, "bisect_probes": sum(c.get("probes_total", 0) for c in calls),
                            "parallelism": f"replicas x{world} (one Philox variant per rank)"},
                 "clocks": clocks,

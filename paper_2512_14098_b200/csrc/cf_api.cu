@@ -776,44 +776,39 @@ __global__ void bisect_final_kernel(BisectState bs, uint32_t P, uint32_t K, uint
 }
 
 // ------------------------------------------------------------------------------------------------
-// stream materialisation (a10 producer): one warp per 32-request chunk, then a per-(variant,trial)
-// pass that turns chunk-relative cumulative gaps into absolute ones.
+// stream materialisation (a10 producer), HBM-bound: three launches, the records are written ONCE.
+//   1. one warp per 32-request chunk draws only the gaps (Philox block 0 + arrival table) and
+//      stores the chunk's total gap;
+//   2. one block per (variant, trial) turns the chunk totals into exclusive prefixes;
+//   3. one warp per chunk draws the full records (the producer code of the simulation kernels),
+//      adds the chunk's prefix to the cumulative gap and writes 1 KiB of records, fully coalesced.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
-materialize_chunks_kernel(const __grid_constant__ KParams prm, uint32_t variant_lo, uint4* out,
-                          uint64_t* chunk_totals, uint32_t chunks_per_sim) {
-  __shared__ uint32_t cnt_dummy[8];
+materialize_totals_kernel(const __grid_constant__ KParams prm, uint32_t variant_lo, uint64_t* chunk_totals,
+                          uint32_t chunks_per_sim) {
   const int lane = threadIdx.x & 31;
   const uint32_t chunk = blockIdx.x * 4 + (threadIdx.x >> 5);
   const uint32_t trial = blockIdx.y, vi = blockIdx.z;
   if (chunk >= chunks_per_sim) return;
-  const size_t sim = (size_t)vi * prm.K + trial;
-  // records of one request are 2 x uint4; lanes beyond N write nothing
-  uint4 tmp_base[1];
-  (void)tmp_base;
-  uint4* dst = out + (sim * prm.N + (size_t)chunk * 32) * 2;
-  // produce into registers via a small shared staging area to reuse the producer
-  __shared__ __align__(16) uint4 stage[4][32 * 2];
-  produce_chunk_philox<6>(prm, chunk * 32, trial, variant_lo + vi, stage[threadIdx.x >> 5],
-                          chunk_totals + sim * chunks_per_sim + chunk, cnt_dummy, lane);
-  __syncwarp();
-  if (chunk * 32 + lane < prm.N) {
-    dst[lane * 2 + 0] = stage[threadIdx.x >> 5][lane * 2 + 0];
-    dst[lane * 2 + 1] = stage[threadIdx.x >> 5][lane * 2 + 1];
+  const uint32_t n = chunk * 32 + lane;
+  uint64_t gap = 0;
+  if (n < prm.N) {
+    const uint4 b0 = philox4x32_10(n, trial, 0, variant_lo + vi, prm.seed_lo, prm.seed_hi);
+    gap = (uint32_t)qtab_sample(prm.qpool, prm.arr_tab, b0.x);
   }
+  const uint64_t tot = warp_inclusive_sum(gap, lane);
+  if (lane == 31) chunk_totals[((size_t)vi * prm.K + trial) * chunks_per_sim + chunk] = tot;
 }
 
-// one CTA per (variant, trial): exclusive scan of the chunk totals, then add to every record
+// one CTA per (variant, trial): in-place exclusive scan of the chunk totals
 __global__ void __launch_bounds__(256)
-materialize_fixup_kernel(uint4* out, uint64_t* chunk_totals, uint32_t N, uint32_t chunks_per_sim) {
-  const size_t sim = blockIdx.x;
-  uint64_t* tot = chunk_totals + sim * chunks_per_sim;
+materialize_scan_kernel(uint64_t* chunk_totals, uint32_t chunks_per_sim) {
+  uint64_t* tot = chunk_totals + (size_t)blockIdx.x * chunks_per_sim;
   __shared__ uint64_t carry;
   __shared__ uint64_t warp_sum[8];
   if (threadIdx.x == 0) carry = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  // pass 1: in-place exclusive prefix of chunk totals (blocks of 256 chunks)
   for (uint32_t base = 0; base < chunks_per_sim; base += 256) {
     const uint32_t c = base + threadIdx.x;
     const uint64_t v = c < chunks_per_sim ? tot[c] : 0;
@@ -827,16 +822,34 @@ materialize_fixup_kernel(uint4* out, uint64_t* chunk_totals, uint32_t N, uint32_
     if (threadIdx.x == 255) carry = off + inc;
     __syncthreads();
   }
-  // pass 2: add the chunk base to the cu field of every record head
-  uint4* rec = out + sim * (size_t)N * 2;
-  for (uint32_t n = threadIdx.x; n < N; n += 256) {
-    uint4 h = rec[(size_t)n * 2];
+}
+
+__global__ void __launch_bounds__(128)
+materialize_chunks_kernel(const __grid_constant__ KParams prm, uint32_t variant_lo, uint4* out,
+                          const uint64_t* chunk_base, uint32_t chunks_per_sim) {
+  __shared__ uint32_t cnt_dummy[8];
+  __shared__ uint64_t tot_dummy[4];
+  __shared__ __align__(16) uint4 stage[4][32 * 2];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t chunk = blockIdx.x * 4 + warp;
+  const uint32_t trial = blockIdx.y, vi = blockIdx.z;
+  if (chunk >= chunks_per_sim) return;
+  const size_t sim = (size_t)vi * prm.K + trial;
+  produce_chunk_philox<6>(prm, chunk * 32, trial, variant_lo + vi, stage[warp], &tot_dummy[warp], cnt_dummy, lane);
+  {  // chunk-relative cumulative gap -> absolute (the head word of this lane's own record)
+    uint4 h = stage[warp][lane * 2];
     const uint64_t t = h.y >> 24;
-    uint64_t cu = (((uint64_t)(h.y & 0x00ffffffu)) << 32 | h.x) + tot[n >> 5];
+    const uint64_t cu = (((uint64_t)(h.y & 0x00ffffffu)) << 32 | h.x) + chunk_base[sim * chunks_per_sim + chunk];
     h.x = (uint32_t)cu;
     h.y = (uint32_t)(cu >> 32) | (uint32_t)(t << 24);
-    rec[(size_t)n * 2] = h;
+    stage[warp][lane * 2] = h;
   }
+  __syncwarp();
+  // 64 x 16 B of the chunk, consecutive lanes write consecutive words; requests beyond N write nothing
+  uint4* dst = out + (sim * prm.N + (size_t)chunk * 32) * 2;
+  const uint32_t n_words = min(32u, prm.N - chunk * 32) * 2u;
+  if ((uint32_t)lane < n_words) dst[lane] = stage[warp][lane];
+  if ((uint32_t)lane + 32u < n_words) dst[lane + 32] = stage[warp][lane + 32];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1107,11 +1120,12 @@ int32_t cf_materialize_stream(const cf_graph* g, uint64_t seed, uint32_t variant
   kp.qpool = reinterpret_cast<const int32_t*>(ws + pool_off);
   kp.status = reinterpret_cast<int32_t*>(ws);
   uint64_t* totals = reinterpret_cast<uint64_t*>(ws + tot_off);
-  materialize_chunks_kernel<<<dim3((chunks + 3) / 4, g->n_trials, n_variants), 128, 0, st>>>(
-      kp, variant_lo, static_cast<uint4*>(out_stream), totals, chunks);
+  const dim3 grid((chunks + 3) / 4, g->n_trials, n_variants);
+  materialize_totals_kernel<<<grid, 128, 0, st>>>(kp, variant_lo, totals, chunks);
   ++g_launch_count;
-  materialize_fixup_kernel<<<n_variants * g->n_trials, 256, 0, st>>>(static_cast<uint4*>(out_stream), totals,
-                                                                      g->n_req, chunks);
+  materialize_scan_kernel<<<n_variants * g->n_trials, 256, 0, st>>>(totals, chunks);
+  ++g_launch_count;
+  materialize_chunks_kernel<<<grid, 128, 0, st>>>(kp, variant_lo, static_cast<uint4*>(out_stream), totals, chunks);
   ++g_launch_count;
   return cuda_rc(cudaGetLastError());
 }

@@ -117,3 +117,21 @@ def test_no_cpu_fallback(cf):
         cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, 0)
     # even through the raw ABI with valid arguments the call fails loudly instead of computing
     assert raw_eval(cf, w.graph, w.plans, w.slo, ws_bytes=1 << 30) == cf.CF_ERR_CUDA
+
+
+def test_update_and_heap_level_counts():
+    """bench.py's exact work counters: hand-computed on a two-plan example, and per-plan sums."""
+    import numpy as np
+    # 2 components, 2 types: type 0 visits {0}, type 1 visits {0, 1}
+    tab = W.constant_qtab(1000)
+    g = W.Graph(2, 2, 10, 1, [0b01, 0b11], W.mix_thresholds([0.5, 0.5]), [0, 0, 0, 0], [tab], tab, [[0, 1]])
+    pl = W.make_plans([[(0b11, 8)], [(0b01, 1), (0b10, 5)]])  # colocated c=8; disaggregated c=1, c=5
+    counts = np.zeros((2, 1, 1, 2, 2), dtype=np.uint32)
+    counts[..., 0, 0] = 6  # 6 requests of type 0
+    counts[..., 1, 0] = 4  # 4 of type 1
+    # plan 0: every request visits its single stage once; plan 1: type 0 one stage, type 1 two
+    assert W.count_updates(g, pl, counts) == (6 + 4) + (6 + 2 * 4)
+    # floor(log2 c): plan 0: 3 per update; plan 1: stage 0 -> 0, stage 1 (type 1 only) -> 2
+    assert W.count_heap_levels(g, pl, counts) == 3 * 10 + 2 * 4
+    np.testing.assert_array_equal(W.count_updates(g, pl, counts, per_plan=True), [10, 14])
+    np.testing.assert_array_equal(W.count_heap_levels(g, pl, counts, per_plan=True), [30, 8])

@@ -236,12 +236,13 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   // replace-min to the depth of its deepest lane, so plans are ordered by the vector of their
   // stages' heap depths, the most visited stage first (mix-weighted), then by the replica counts.
   std::vector<uint64_t> plan_key(P, 0);  // 8 stages x (2 bits depth class | 6 bits of c), most visited stage first
+  std::vector<std::vector<double>> topo_wgt(sc.topos.size());  // probability that a request visits stage s
   {
     std::vector<double> pi(g->n_types);
     for (uint32_t t = 0; t < g->n_types; ++t) {
       const double hi = t + 1 == g->n_types ? 4294967296.0 : (double)g->type_thresh[t];
       const double lo = t == 0 ? 0.0 : (double)g->type_thresh[t - 1];
-      pi[t] = std::max(0.0, hi - lo);
+      pi[t] = std::max(0.0, hi - lo) / 4294967296.0;
     }
     std::vector<std::vector<uint32_t>> topo_order(sc.topos.size());
     for (size_t ti = 0; ti < sc.topos.size(); ++ti) {
@@ -254,6 +255,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       std::iota(topo_order[ti].begin(), topo_order[ti].end(), 0u);
       std::stable_sort(topo_order[ti].begin(), topo_order[ti].end(),
                        [&](uint32_t x, uint32_t y) { return wgt[x] > wgt[y]; });
+      topo_wgt[ti] = wgt;
     }
     for (uint32_t p = 0; p < P; ++p) {
       uint64_t kd = 0, kc = 0;
@@ -297,19 +299,26 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       wi.wd.sim_begin = (uint32_t)(sim0 + w0);
       wi.wd.n_lanes = (uint32_t)std::min<size_t>(32, n_group - w0);
       wi.wd.topo = plan_topo[order[i]];
-      uint32_t pairs = 0, quads = 0, cost = 0;
+      uint32_t pairs = 0, quads = 0;
+      uint32_t lv_max[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // a warp sifts to the depth of its deepest lane
       for (uint32_t l = 0; l < wi.wd.n_lanes; ++l) {
         const uint32_t p = sc.sims[wi.wd.sim_begin + l].plan;
         pairs = std::max(pairs, plan_pairs[p]);
         quads = std::max(quads, plan_quads[p]);
-        uint32_t cp = 0;  // rough time of one request: 2 units per stage + 3 per heap level
         for (uint32_t s = 0; s < td.n_stages; ++s) {
           uint32_t c = sc.plan_c[(size_t)p * 8 + s], lv = 0;
-          while (c > 1) { ++lv; c >>= 1; }
-          cp += 2 + 3 * lv;
+          if (fast) lv = c <= 1 ? 0 : (c <= 5 ? 1 : (c <= 21 ? 2 : 3));
+          else while (c > 1) { ++lv; c >>= 1; }
+          lv_max[s] = std::max(lv_max[s], lv);
         }
-        cost = std::max(cost, cp);
       }
+      // expected warp instructions per request (ncu source page of the fast kernel: 45 per request,
+      // 25 per visited stage, 17 per heap level), in 1/1000: the warps of a block meet at a barrier
+      // after every tile, so a block is cut from warps of equal expected cost
+      double cost_d = 45.0;
+      for (uint32_t s = 0; s < td.n_stages; ++s)
+        cost_d += topo_wgt[wi.wd.topo][s] * (25.0 + 17.0 * lv_max[s]);
+      const uint32_t cost = (uint32_t)(cost_d * 1000.0 + 0.5);
       wi.heap_w = pairs * 512u;
       wi.heap_f = quads * 512u;
       wi.wd.heap_rows32 = quads;
@@ -321,11 +330,11 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
     }
     i = j;
   }
-  // slow (deep-heap) warps together: a block advances tile by tile at the pace of its slowest warp
+  // warps of equal expected cost together: a block advances tile by tile at the pace of its slowest warp
   std::stable_sort(winfo.begin(), winfo.end(), [](const WarpInfo& a, const WarpInfo& b) {
     if (a.variant != b.variant) return a.variant < b.variant;
-    if (a.heap_bytes != b.heap_bytes) return a.heap_bytes > b.heap_bytes;
-    return a.cost > b.cost;
+    if (a.cost != b.cost) return a.cost > b.cost;
+    return a.heap_bytes > b.heap_bytes;
   });
   uint32_t max_heap = 0;
   for (const WarpInfo& wi : winfo) max_heap = std::max(max_heap, wi.heap_bytes);

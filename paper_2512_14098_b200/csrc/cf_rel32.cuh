@@ -53,7 +53,10 @@ struct StageRec32 {
   static constexpr int kWords = VMAX <= 2 ? 2 : (VMAX <= 6 ? 3 : 4);
 };
 
-// Per-lane, per-stage state record (16 B): { base_lo, base_hi, root key, heap_row | nq << 16 }
+// Per-lane, per-stage state record (16 B): { base_lo, base_hi, root key, hb | nq << 18 }: hb = shared
+// address of the lane's top heap quad (18 bits; the record's own address when nq == 0, so that the
+// request loop can load "the top quad" unconditionally), nq = number of quads
+constexpr uint32_t kHbMask = 0x3ffffu;
 template <int VMAX, int CMAX, int WARPS>
 struct SmemLayout32 {
   static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
@@ -79,6 +82,12 @@ __device__ __forceinline__ uint64_t mad_wide_u32(uint32_t a, uint32_t b, uint64_
 __device__ __forceinline__ uint4 lds128(uint32_t a) {
   uint4 v;
   asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+  return v;
+}
+// volatile: ptxas keeps the load where it is written (ahead of the arithmetic that hides its latency)
+__device__ __forceinline__ uint4 lds128v(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
   return v;
 }
 __device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
@@ -202,7 +211,8 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           sts128(heap_sa + (row + j) * 512u, make_uint4(v[0], v[1], v[2], v[3]));
         }
       }
-      sts128(st_sa + s * 512u, make_uint4(0u, 0u, 0u, row | (nq << 16)));
+      const uint32_t hb = nq ? heap_sa + row * 512u : st_sa + s * 512u;
+      sts128(st_sa + s * 512u, make_uint4(0u, 0u, 0u, hb | (nq << 18)));
       row += nq;
     }
   }
@@ -237,7 +247,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
       const uint64_t nbr = nb - delta;                  // ... relative to the new origin
       sts128(sa, make_uint4((uint32_t)nbr, (uint32_t)(nbr >> 32), 0u, st.w));
       const uint32_t sh4 = shift >= (1ull << 30) ? 0xfffffffcu : ((uint32_t)shift << 2);
-      const uint32_t nq = st.w >> 16, ha = heap_sa + (st.w & 0xffffu) * 512u;
+      const uint32_t nq = st.w >> 18, ha = st.w & kHbMask;
       if (sh4 != 0u)
         for (uint32_t j = 0; j < nq; ++j) {
           uint4 q = lds128(ha + j * 512u);
@@ -334,7 +344,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           constexpr bool NARROW = MODE == 0;
           using X = typename std::conditional<NARROW, uint32_t, uint64_t>::type;
           uint32_t sid = w1.x & 0xffu;
-          uint4 st = make_uint4(0, 0, 0, 0);
+          uint4 st;
           if (sid != 0xffu) st = lds128(st_sa + sid * 512u);
           {  // next record (the buffer has 32 records; reading one past the chunk's last is harmless)
             const uint32_t na = wb_sa + (uint32_t)min(r + 1, 31) * (kW * 16u);
@@ -367,12 +377,13 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
                              : j == 4 ? w2.z : j == 5 ? w2.w : j == 6 ? w3.x : w3.y;
             const uint32_t sa = st_sa + sid * 512u;
             const uint4 cur = st;
-            const uint32_t nq = cur.w >> 16, hb = heap_sa + (cur.w & 0xffffu) * 512u;
-            uint4 q = make_uint4(0, 0, 0, 0);
-            if (nq) q = lds128(hb);  // top quad of this stage's heap
-            if (j + 1 < VMAX) {      // state record of the next visit
+            const uint32_t nq512 = (cur.w >> 9) & ~0x1ffu, hb = cur.w & kHbMask;  // nq * 512
+            const uint4 q = lds128v(hb);  // top quad of this stage's heap (the state record if nq == 0)
+            if (j + 1 < VMAX) {          // state record of the next visit
               sid = ((j + 1 < 4 ? w1.x : w1.y) >> (8 * ((j + 1) & 3))) & 0xffu;
-              if (sid != 0xffu) st = lds128(st_sa + sid * 512u);
+              uint4 nxt;  // left undefined after the last visit: no copy of the old record is kept
+              if (sid != 0xffu) nxt = lds128(st_sa + sid * 512u);
+              st = nxt;
             } else {
               sid = 0xffu;
             }
@@ -392,7 +403,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
               if (key64 >= (uint64_t)kKeyLimit) flagged = true;
               key = (uint32_t)key64;
             }
-            if (nq) key = heap4_replace_min(hb, nq << 9, key, q);
+            if (nq512) key = heap4_replace_min(hb, nq512, key, q);
             sts32(sa + 8u, key);
           }
           // a8

@@ -103,23 +103,30 @@ __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
 // each stored as (key << 2) | slot; nodes >= c hold +inf. nq = heap_quads(c) >= 1.
 // Returns the new root key.
 // ------------------------------------------------------------------------------------------------
+// slot bits of a packed key; opaque to the compiler, which otherwise derives the hole address and the
+// child offset from the packed word by separate shift/mask chains (8 instructions per level instead of 4)
+__device__ __forceinline__ uint32_t slot_of(uint32_t m) {
+  uint32_t k;
+  asm("and.b32 %0, %1, 3;" : "=r"(k) : "r"(m));
+  return k;
+}
 __device__ __forceinline__ uint32_t heap4_replace_min(uint32_t hb, uint32_t nq512, uint32_t key, uint4 q) {
   const uint32_t xk = key << 2;  // q = the top quad (at hb), loaded by the caller ahead of time
   uint32_t m = min(min(q.x, q.y), min(q.z, q.w));
   if (xk <= m) return key;  // x <= every child
   const uint32_t new_root = m >> 2;
-  uint32_t k = m & 3u;
+  uint32_t k = slot_of(m);
   uint32_t hole = hb + 4u * k;       // byte address of the hole; its slot is k
-  uint32_t rel = (k + 1u) << 9;      // 512 * node index of the hole = byte offset of its children quad
+  uint32_t rel = k * 512u + 512u;    // 512 * node index of the hole = byte offset of its children quad
   while (rel < nq512) {
     const uint32_t qa = hb + rel;
     q = lds128(qa);
     m = min(min(q.x, q.y), min(q.z, q.w));
     if (xk <= m) break;
     sts32(hole, (m & ~3u) | k);      // the smallest child moves up into the hole (slot k)
-    k = m & 3u;
+    k = slot_of(m);
     hole = qa + 4u * k;
-    rel = 4u * rel + ((k + 1u) << 9);
+    rel = 4u * rel + (k * 512u + 512u);
   }
   sts32(hole, xk | k);
   return new_root;

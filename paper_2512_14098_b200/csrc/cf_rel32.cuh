@@ -387,7 +387,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
             const uint32_t nq512 = (cur.w >> 9) & ~0x1ffu, hb = cur.w & kHbMask;  // nq * 512
             const uint4 q = lds128v(hb);  // top quad of this stage's heap (the state record if nq == 0)
             if (j + 1 < VMAX) {          // state record of the next visit
-              sid = ((j + 1 < 4 ? w1.x : w1.y) >> (8 * ((j + 1) & 3))) & 0xffu;
+              sid = __byte_perm(j + 1 < 4 ? w1.x : w1.y, 0u, 0x4440u + ((j + 1) & 3));  // one PRMT
               uint4 nxt;  // left undefined after the last visit: no copy of the old record is kept
               if (sid != 0xffu) nxt = lds128(st_sa + sid * 512u);
               st = nxt;

@@ -285,6 +285,14 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         origin = o_new;
       }
       uint32_t hlo = 0, hhi = 0;
+      auto flush_hits = [&]() {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          hits[t] += (hlo >> (8 * t)) & 0xffu;
+          if (T8) hits[T8 ? t + 4 : t] += (hhi >> (8 * t)) & 0xffu;
+        }
+        hlo = 0; hhi = 0;
+      };
       uint64_t dep = 0, mk = 0;
 #pragma unroll 1
       for (int ch = 0; ch < kChunks; ++ch) {
@@ -467,6 +475,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         }
         __syncwarp();
         cu_base += totals[buf * kChunks + ch];
+        if ((ch & 3) == 3) flush_hits();  // a byte field holds at most 128 hits
       }
       // ---- tile epilogue: absolute outputs, window checks
       const uint32_t idx_end = min(n0 + (uint32_t)kTile, prm.N);
@@ -474,11 +483,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
       flush_idx = idx_end;
       makespan = max(makespan, origin + mk);
       tile_base = last_cu;
-#pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        hits[t] += (hlo >> (8 * t)) & 0xffu;
-        if (T8) hits[T8 ? t + 4 : t] += (hhi >> (8 * t)) & 0xffu;
-      }
+      flush_hits();
     }
     __syncthreads();
   }

@@ -38,10 +38,11 @@ OPS_PER_UPDATE = 7
 OPS_PER_HEAP_LEVEL = 11
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the simulation kernel, per launch at full size,
-# from the ncu captures in profiles/r01_ncu_full_final_cfg2s_cfg1.txt (config 1) and
-# profiles/r01_ncu_full_cfg1_cfg2_fullsize_fast_kernel.txt (config 2) (the outputs
-# stay in the 126 MB L2 past the end of the launch, so almost nothing is written back in time)
-NCU_TRAFFIC_BYTES = {1: 193_280, 2: 1_176_576}
+# from the ncu captures in profiles/r01_ncu_full_s31_cfg2s_cfg1.txt (config 1) and
+# profiles/r01_ncu_metrics_cfg2_fullsize_s31.csv (config 2) (the outputs stay in the 126 MB L2
+# past the end of the launch, so almost nothing is written back in time; what is read is the
+# schedule, the tables and cold-cache instruction fetch, and varies by a few hundred KB per capture)
+NCU_TRAFFIC_BYTES = {1: 657_152, 2: 1_164_032}
 
 
 def make_workload(cfg: int, scale: float = 1.0):

@@ -21,7 +21,7 @@
  *    without synchronising (host-side scheduling happens before the first launch). Scratch comes
  *    from the caller's `workspace` (dev, >= cf_workspace_bytes(), 256-byte aligned); it must stay
  *    untouched until the stream work has finished. Distinct streams + distinct workspaces are
- *    thread-safe; there is no global state.
+ *    thread-safe; no call reads or writes library-wide state.
  *  - Return value: CF_OK or a negative cf_status. Argument errors are detected on the host before
  *    anything is enqueued. Conditions that depend on device data (a rate outside [1, 1e9] mrps, or
  *    arrivals that would exceed 2^62 us, R17) are detected on the device: that
@@ -156,37 +156,18 @@ int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint3
  * and returns it (CF_OK, CF_ERR_RANGE, or CF_ERR_CUDA). */
 int32_t cf_workspace_status(const void* workspace, void* stream);
 
-/* Number of kernels the last call on this workspace's host thread enqueued (bench bookkeeping). */
-uint32_t cf_last_launch_count(void);
-
 /* The simulation runs on a 32-bit fast kernel (times as uint32 offsets from a per-tile origin,
  * DESIGN.md 5.2) followed by the 64-bit kernel over exactly those simulations that left the 32-bit
  * window; results are bit-identical either way. cf_workspace_wide_count synchronises `stream` and
  * returns how many simulations of the last call on `workspace` were redone by the 64-bit kernel
- * (>= 0), or a negative cf_status. cf_debug_kernel_mode (tests): 0 = automatic (default),
- * 1 = 64-bit kernel only; applies to later calls made by the calling host thread. */
+ * (>= 0), or a negative cf_status. (Test and tuning hooks that force one path or the other live in
+ * cf_debug.h; they are per-call arguments, not library state.) */
 int64_t cf_workspace_wide_count(const void* workspace, void* stream);
-int32_t cf_debug_kernel_mode(uint32_t mode);
-
-/* cf_goodput_bisect[_stream] simulate, in one pass, the complete decision tree of the next `depth`
- * bisection steps of every plan (2^depth - 1 candidate rates) and then walk the path the sequential
- * algorithm takes: identical results, `depth` times fewer passes, more simulations in flight.
- * depth = 0 (default): chosen from P*K so that a pass fills the GPU; 1..4: fixed (tests, tuning).
- * Applies to later calls made by the calling host thread. */
-int32_t cf_debug_bisect_depth(uint32_t depth);
 
 /* Bench bookkeeping: synchronises `stream` and copies to out_probes (host, [n_plans]) how many
  * probes (simulated rates) lay on the bisection path of each plan in the last cf_goodput_bisect*
  * call on `workspace` (steps whose bracket had already closed are no-ops and do not count). */
 int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_probes, void* stream);
-
-/* Micro-benchmark used by bench.py for the ALU roofline denominator: runs `iters` rounds of an
- * unrolled, independent 32-bit integer instruction mix on every SM and writes the number of
- * lane-operations executed to *out_ops (host). mix: 0 = IADD3/LOP3 only (ALU pipe), 1 = IMAD only
- * (FMA pipe), 2 = alternating. Returns the elapsed milliseconds * 1000 (microseconds) in
- * *out_usec (host), measured with CUDA events on `stream`. Synchronises. */
-int32_t cf_bench_int32_peak(uint32_t mix, uint32_t iters, uint64_t* out_ops, uint64_t* out_usec,
-                            void* stream);
 
 const char* cf_strerror(int32_t status);
 

@@ -19,11 +19,15 @@ LIB_PATH = os.path.join(_HERE, "libcf_b200.so")
 CF_OK, CF_ERR_ARG, CF_ERR_RANGE, CF_ERR_PLAN, CF_ERR_TABLE, CF_ERR_CUDA, CF_ERR_WORKSPACE = \
     0, -1, -2, -3, -4, -5, -6
 
+# include/cf.h (the product ABI) and include/cf_debug.h (test / tuning / bench hooks)
 EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_stream_bytes",
            "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
-           "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status",
-           "cf_last_launch_count", "cf_bench_int32_peak", "cf_strerror", "cf_workspace_wide_count",
-           "cf_debug_kernel_mode", "cf_debug_bisect_depth", "cf_bisect_probes"]
+           "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_strerror",
+           "cf_workspace_wide_count", "cf_bisect_probes"]
+DEBUG_EXPORTS = ["cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
+                 "cf_goodput_bisect_stream_opt", "cf_trace_sim_opt", "cf_last_launch_count",
+                 "cf_bench_int32_peak"]
+CF_KERNEL_AUTO, CF_KERNEL_WIDE64, CF_KERNEL_FAST32, CF_KERNEL_SCAN = 0, 1, 2, 3
 
 
 class CfError(RuntimeError):
@@ -51,6 +55,11 @@ class cf_plans(C.Structure):
                 ("stage_c", C.POINTER(C.c_uint16))]
 
 
+class cf_options(C.Structure):
+    _fields_ = [("kernel_mode", C.c_uint32), ("bisect_depth", C.c_uint32), ("bisect_predict", C.c_uint32),
+                ("reserved", C.c_uint32 * 5)]
+
+
 class cf_slo(C.Structure):
     _fields_ = [("L_us", C.POINTER(C.c_int64)), ("att_num", C.POINTER(C.c_uint32)),
                 ("att_den", C.POINTER(C.c_uint32))]
@@ -66,12 +75,21 @@ _lib.cf_materialize_workspace_bytes.restype = C.c_size_t
 _lib.cf_strerror.restype = C.c_char_p
 _lib.cf_last_launch_count.restype = C.c_uint32
 _lib.cf_workspace_wide_count.restype = C.c_int64
-_lib.cf_debug_kernel_mode.restype = C.c_int32
-_lib.cf_debug_bisect_depth.restype = C.c_int32
 _lib.cf_bisect_probes.restype = C.c_int32
 for _n in ("cf_eval_plans", "cf_goodput_bisect", "cf_materialize_stream", "cf_eval_plans_stream",
-           "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak"):
+           "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak",
+           "cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
+           "cf_goodput_bisect_stream_opt", "cf_trace_sim_opt"):
     getattr(_lib, _n).restype = C.c_int32
+
+# Test / tuning options (include/cf_debug.h). The library itself has no knobs: this module-level
+# record belongs to the Python binding; while it holds defaults, calls go through the product entry
+# points of cf.h, otherwise through their *_opt twins with the record as the per-call argument.
+_OPT = cf_options()
+
+
+def _opt_active() -> bool:
+    return bool(_OPT.kernel_mode or _OPT.bisect_depth or _OPT.bisect_predict)
 
 
 def strerror(status: int) -> str:
@@ -159,10 +177,12 @@ def cf_workspace_wide_count(workspace: torch.Tensor, stream=None) -> int:
 
 
 def cf_debug_kernel_mode(mode: int) -> None:
-    """0 = automatic (32-bit fast kernel + 64-bit fixup), 1 = 64-bit kernel only (tests)."""
-    rc = int(_lib.cf_debug_kernel_mode(C.c_uint32(mode)))
-    if rc != CF_OK:
-        raise CfError(rc, "cf_debug_kernel_mode")
+    """Kernel choice of later calls made through this binding (cf_debug.h CF_KERNEL_*): 0 = automatic
+    (32-bit fast kernel + 64-bit fixup, or the scan kernel), 1 = 64-bit kernel only, 2 = fast kernel
+    (never the scan kernel; traces run on it), 3 = max-plus scan kernel."""
+    if not 0 <= mode <= 3:
+        raise CfError(CF_ERR_ARG, "cf_debug_kernel_mode")
+    _OPT.kernel_mode = mode
 
 
 def cf_bisect_probes(workspace: torch.Tensor, n_plans: int, stream=None) -> np.ndarray:
@@ -175,10 +195,17 @@ def cf_bisect_probes(workspace: torch.Tensor, n_plans: int, stream=None) -> np.n
 
 
 def cf_debug_bisect_depth(depth: int) -> None:
-    """Bisection steps simulated per pass: 0 = automatic, 1..4 = fixed (tests, tuning)."""
-    rc = int(_lib.cf_debug_bisect_depth(C.c_uint32(depth)))
-    if rc != CF_OK:
-        raise CfError(rc, "cf_debug_bisect_depth")
+    """Bisection steps simulated per pass by later calls: 0 = automatic, 1..4 = fixed (tests, tuning)."""
+    if not 0 <= depth <= 4:
+        raise CfError(CF_ERR_ARG, "cf_debug_bisect_depth")
+    _OPT.bisect_depth = depth
+
+
+def cf_debug_bisect_predict(mode: int) -> None:
+    """0 = default, 1 = always the full decision tree, 2 = always node + predicted child (cf_debug.h)."""
+    if not 0 <= mode <= 2:
+        raise CfError(CF_ERR_ARG, "cf_debug_bisect_predict")
+    _OPT.bisect_predict = mode
 
 
 def cf_last_launch_count() -> int:
@@ -205,18 +232,19 @@ def cf_eval_plans(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, 
         out_makespan = torch.empty((P, R, K), dtype=torch.int64, device=dev)
     if workspace is None:
         workspace = alloc_workspace(graph, plans, R)
+    opt = (C.byref(_OPT),) if _opt_active() else ()
     if stream_records is None:
-        rc = _lib.cf_eval_plans(C.byref(m.g), C.byref(m.pl), _dp(rates), C.c_uint32(R), C.byref(m.slo),
-                                C.c_uint64(seed), C.c_uint32(variant), _dp(out_counts),
-                                _dp(out_dep_sum), _dp(out_makespan), _dp(workspace),
-                                C.c_size_t(workspace.numel()), _stream_ptr(stream))
+        fn = _lib.cf_eval_plans_opt if opt else _lib.cf_eval_plans
+        rc = fn(*opt, C.byref(m.g), C.byref(m.pl), _dp(rates), C.c_uint32(R), C.byref(m.slo),
+                C.c_uint64(seed), C.c_uint32(variant), _dp(out_counts), _dp(out_dep_sum),
+                _dp(out_makespan), _dp(workspace), C.c_size_t(workspace.numel()), _stream_ptr(stream))
     else:
         pv = None if plan_variant is None else np.ascontiguousarray(plan_variant, dtype=np.uint32)
-        rc = _lib.cf_eval_plans_stream(C.byref(m.g), C.byref(m.pl), _dp(rates), C.c_uint32(R),
-                                       C.byref(m.slo), _dp(stream_records), C.c_uint32(n_variants),
-                                       _hp(pv, C.c_uint32), _dp(out_counts), _dp(out_dep_sum),
-                                       _dp(out_makespan), _dp(workspace),
-                                       C.c_size_t(workspace.numel()), _stream_ptr(stream))
+        fn = _lib.cf_eval_plans_stream_opt if opt else _lib.cf_eval_plans_stream
+        rc = fn(*opt, C.byref(m.g), C.byref(m.pl), _dp(rates), C.c_uint32(R), C.byref(m.slo),
+                _dp(stream_records), C.c_uint32(n_variants), _hp(pv, C.c_uint32), _dp(out_counts),
+                _dp(out_dep_sum), _dp(out_makespan), _dp(workspace), C.c_size_t(workspace.numel()),
+                _stream_ptr(stream))
     if check and rc != CF_OK:
         raise CfError(rc, "cf_eval_plans")
     return dict(counts=out_counts, dep_sum=out_dep_sum, makespan=out_makespan, workspace=workspace,
@@ -239,18 +267,18 @@ def cf_goodput_bisect(graph, plans, rate_hi_mrps, n_steps: int, slo, seed: int, 
     counts = torch.empty((P, K, T, 2), dtype=torch.int32, device=dev) if want_counts else None
     if workspace is None:
         workspace = alloc_workspace(graph, plans, 1)
+    opt = (C.byref(_OPT),) if _opt_active() else ()
     if stream_records is None:
-        rc = _lib.cf_goodput_bisect(C.byref(m.g), C.byref(m.pl), _dp(hi), C.c_uint32(n_steps),
-                                    C.byref(m.slo), C.c_uint64(seed), C.c_uint32(variant), _dp(rate),
-                                    _dp(good), _dp(counts), _dp(workspace),
-                                    C.c_size_t(workspace.numel()), _stream_ptr(stream))
+        fn = _lib.cf_goodput_bisect_opt if opt else _lib.cf_goodput_bisect
+        rc = fn(*opt, C.byref(m.g), C.byref(m.pl), _dp(hi), C.c_uint32(n_steps), C.byref(m.slo),
+                C.c_uint64(seed), C.c_uint32(variant), _dp(rate), _dp(good), _dp(counts), _dp(workspace),
+                C.c_size_t(workspace.numel()), _stream_ptr(stream))
     else:
         pv = None if plan_variant is None else np.ascontiguousarray(plan_variant, dtype=np.uint32)
-        rc = _lib.cf_goodput_bisect_stream(C.byref(m.g), C.byref(m.pl), _dp(hi), C.c_uint32(n_steps),
-                                           C.byref(m.slo), _dp(stream_records), C.c_uint32(n_variants),
-                                           _hp(pv, C.c_uint32), _dp(rate), _dp(good), _dp(counts),
-                                           _dp(workspace), C.c_size_t(workspace.numel()),
-                                           _stream_ptr(stream))
+        fn = _lib.cf_goodput_bisect_stream_opt if opt else _lib.cf_goodput_bisect_stream
+        rc = fn(*opt, C.byref(m.g), C.byref(m.pl), _dp(hi), C.c_uint32(n_steps), C.byref(m.slo),
+                _dp(stream_records), C.c_uint32(n_variants), _hp(pv, C.c_uint32), _dp(rate), _dp(good),
+                _dp(counts), _dp(workspace), C.c_size_t(workspace.numel()), _stream_ptr(stream))
     if check and rc != CF_OK:
         raise CfError(rc, "cf_goodput_bisect")
     return dict(rate_mrps=rate, goodput_mrps=good, counts=counts, workspace=workspace, rc=int(rc))
@@ -288,13 +316,16 @@ def cf_trace_sim(graph, plans, plan: int, rate_mrps: int, trial: int, seed: int,
     dep = torch.empty(N, dtype=torch.int64, device="cuda")
     typ = torch.empty(N, dtype=torch.uint8, device="cuda")
     ws = alloc_workspace(graph, plans, 1)
-    rc = _lib.cf_trace_sim(C.byref(m.g), C.byref(m.pl), C.c_uint32(plan), C.c_uint32(rate_mrps),
-                           C.c_uint32(trial), C.c_uint64(seed), C.c_uint32(variant), _dp(arr), _dp(dep),
-                           _dp(typ), _dp(ws), C.c_size_t(ws.numel()), _stream_ptr(stream))
+    opt = (C.byref(_OPT),) if _opt_active() else ()
+    fn = _lib.cf_trace_sim_opt if opt else _lib.cf_trace_sim
+    rc = fn(*opt, C.byref(m.g), C.byref(m.pl), C.c_uint32(plan), C.c_uint32(rate_mrps),
+            C.c_uint32(trial), C.c_uint64(seed), C.c_uint32(variant), _dp(arr), _dp(dep),
+            _dp(typ), _dp(ws), C.c_size_t(ws.numel()), _stream_ptr(stream))
     if check and rc != CF_OK:
         raise CfError(rc, "cf_trace_sim")
     status = cf_workspace_status(ws, stream)
-    return dict(arrival=arr, departure=dep, type=typ, rc=int(rc), status=status)
+    wide = cf_workspace_wide_count(ws, stream) if rc == CF_OK else -1
+    return dict(arrival=arr, departure=dep, type=typ, rc=int(rc), status=status, wide=wide)
 
 
 def cf_bench_int32_peak(mix: int, iters: int = 2000, stream=None):

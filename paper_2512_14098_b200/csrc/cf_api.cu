@@ -12,18 +12,20 @@
 #include <vector>
 
 #include "../../include/cf.h"
-#include "cf_rel32.cuh"
-#include "cf_scan.cuh"
+#include "../../include/cf_debug.h"
+#include "cf_launch.h"
+#include "cf_rel32.cuh"  // layout constants only: the kernels are instantiated in cf_k32.cu
+#include "cf_scan.cuh"   // kScanWarps
 
 using namespace cfk;
 
 namespace {
 
+// statistics only (cf_debug.h cf_last_launch_count): nothing in the library reads it
 thread_local uint32_t g_launch_count = 0;
-thread_local uint32_t g_kernel_mode = 0;  // cf_debug_kernel_mode: 0 auto, 1 = 64-bit kernel only
-thread_local uint32_t g_spec_depth = 0;   // cf_debug_bisect_depth: 0 auto, 1..4 = bisection steps per pass
 
 constexpr size_t kAlign = 256;
+constexpr uint32_t kMaxSpecDepth = 4;  // bisection steps simulated per pass (speculative decision tree)
 constexpr uint32_t kMaxSmem = 227u * 1024u;
 size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
@@ -170,7 +172,7 @@ int kernel_regs32(int vmax, int cmax);
 // the same warps and blocks with its own, larger heap offsets.
 int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
                        const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
-                       bool fast, Schedule* out) {
+                       bool fast, uint32_t kernel_mode, Schedule* out) {
   const uint32_t P = pl->n_plans, MS = pl->max_stages;
   Schedule& sc = *out;
   sc.plan_c.assign((size_t)P * 8, 1);
@@ -202,14 +204,17 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   sc.R = R;
   sc.plan_topo_v = plan_topo;
   sc.all_c1 = true;
-  for (uint32_t p = 0; p < P; ++p)
+  for (uint32_t p = only_plan ? *only_plan : 0; p < (only_plan ? *only_plan + 1 : P); ++p)
     for (uint32_t st = 0; st < pl->n_stages[p]; ++st)
       if (pl->stage_c[(size_t)p * MS + st] != 1) sc.all_c1 = false;
   // The scan kernel spends a warp (and its own Philox draws) per simulation: 3.6x faster than a
   // thread per simulation when the call has few simulations (config 0: 32 per call), 5.7x slower
   // when there are enough to fill the GPU with threads (measured crossover near 9 000 simulations).
-  if ((uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
-  if (only_plan || g_kernel_mode == 1) sc.all_c1 = false;  // traces and the forced 64-bit mode keep the thread-per-simulation path
+  if (!only_plan && (uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
+  if (kernel_mode == CF_KERNEL_SCAN && !sc.all_c1) return CF_ERR_ARG;  // one replica everywhere, <= 8192 simulations
+  // the forced thread-per-simulation modes (cf_debug.h) keep that path; so do traces unless asked otherwise
+  if (kernel_mode == CF_KERNEL_WIDE64 || kernel_mode == CF_KERNEL_FAST32) sc.all_c1 = false;
+  if (only_plan && kernel_mode != CF_KERNEL_SCAN) sc.all_c1 = false;
   sc.vmax = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 6 ? 6 : 8));
   sc.vmax32 = sc.cmax == 8 ? 8 : (maxV <= 2 ? 2 : (maxV <= 4 ? 4 : (maxV <= 6 ? 6 : 8)));
   // 8 warps per block amortise the tile over more simulations and win when a warp's lanes are
@@ -483,115 +488,51 @@ void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool
 // ------------------------------------------------------------------------------------------------
 // launches
 // ------------------------------------------------------------------------------------------------
-template <int VMAX, int CMAX, bool HAS_DELAY, int W>
-cudaError_t launch_one(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY, W>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
-  if (e != cudaSuccess) return e;
-  kp.k_launch = n_trials;
+LaunchCfg launch_cfg(const Schedule& sc, uint32_t n_trials, bool fast, cudaError_t* err) {
   // 1-D grid, block b = (CTA b / n_trials, trial b % n_trials): <= 2^31-1 blocks
   const uint64_t blocks = (uint64_t)sc.ctas.size() * n_trials;
-  if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-  kern<<<(uint32_t)blocks, W * 32, sc.smem_bytes, st>>>(kp, 0u);
-  ++g_launch_count;
-  return cudaGetLastError();
+  *err = blocks > 0x7fffffffull ? cudaErrorInvalidConfiguration : cudaSuccess;
+  return LaunchCfg{(uint32_t)blocks, fast ? sc.smem_bytes32 : sc.smem_bytes, sc.warps_per_cta};
 }
 
-template <int VMAX, int CMAX>
-int regs_of() {
-  static int regs = [] {
-    cudaFuncAttributes a;
-    if (cudaFuncGetAttributes(&a, cf_sim_kernel<VMAX, CMAX, false, 8>) != cudaSuccess) {
-      cudaGetLastError();
-      return VMAX <= 2 ? 64 : 128;  // ptxas figures of this build; used when no device is present
-    }
-    return a.numRegs;
-  }();
-  return regs;
-}
-
-template <int VMAX, int CMAX>
-cudaError_t launch_v(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  const bool d = kp.edge_delay != 0;
-  if (sc.warps_per_cta == 4)
-    return d ? launch_one<VMAX, CMAX, true, 4>(kp, sc, n_trials, st) : launch_one<VMAX, CMAX, false, 4>(kp, sc, n_trials, st);
-  return d ? launch_one<VMAX, CMAX, true, 8>(kp, sc, n_trials, st) : launch_one<VMAX, CMAX, false, 8>(kp, sc, n_trials, st);
-}
-
-cudaError_t launch_sims(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  if (sc.cmax == 8) return launch_v<8, 8>(kp, sc, n_trials, st);
-  if (sc.vmax == 2) return launch_v<2, 6>(kp, sc, n_trials, st);
-  if (sc.vmax == 6) return launch_v<6, 6>(kp, sc, n_trials, st);
-  return launch_v<8, 6>(kp, sc, n_trials, st);
-}
-
-int kernel_regs(int vmax, int cmax) {
-  if (cmax == 8) return regs_of<8, 8>();
-  if (vmax == 2) return regs_of<2, 6>();
-  if (vmax == 6) return regs_of<6, 6>();
-  return regs_of<8, 6>();
-}
-
-// ---- the 32-bit fast kernel (cf_rel32.cuh) ---------------------------------------------------------
-template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int W>
-cudaError_t launch_one32(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  auto kern = cf_sim32_kernel<VMAX, CMAX, HAS_DELAY, T8, W>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+cudaError_t launch_sims(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  cudaError_t e;
+  const LaunchCfg lc = launch_cfg(sc, n_trials, false, &e);
   if (e != cudaSuccess) return e;
   kp.k_launch = n_trials;
-  const uint64_t blocks = (uint64_t)sc.ctas.size() * n_trials;
-  if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-  kern<<<(uint32_t)blocks, W * 32, sc.smem_bytes32, st>>>(kp);
   ++g_launch_count;
-  return cudaGetLastError();
+  return launch_k64(sc.vmax, sc.cmax, kp, lc, st);
 }
 
-template <int VMAX, int CMAX>
-int regs_of32() {
-  static int regs = [] {
-    cudaFuncAttributes a;
-    if (cudaFuncGetAttributes(&a, cf_sim32_kernel<VMAX, CMAX, false, true, 8>) != cudaSuccess) {
-      cudaGetLastError();
-      return 128;  // __launch_bounds__ cap of this build; used when no device is present
-    }
-    return a.numRegs;
-  }();
-  return regs;
-}
+int kernel_regs(int vmax, int cmax) { return regs_k64(vmax, cmax); }
 
+// ---- the 32-bit fast kernel (cf_rel32.cuh, instantiated per (VMAX, CMAX) in cf_k32.cu) ------------
 int kernel_regs32(int vmax, int cmax) {
-  if (cmax == 8) return regs_of32<8, 8>();
-  if (vmax == 2) return regs_of32<2, 6>();
-  if (vmax == 4) return regs_of32<4, 6>();
-  if (vmax == 6) return regs_of32<6, 6>();
-  return regs_of32<8, 6>();
+  if (cmax == 8) return regs_k32_v8c8();
+  if (vmax == 2) return regs_k32_v2c6();
+  if (vmax == 4) return regs_k32_v4c6();
+  if (vmax == 6) return regs_k32_v6c6();
+  return regs_k32_v8c6();
 }
 
-template <int VMAX, int CMAX, int W>
-cudaError_t launch_w32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  const bool d = kp.edge_delay != 0, t8 = kp.T > 4;
-  if (d) return t8 ? launch_one32<VMAX, CMAX, true, true, W>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, true, false, W>(kp, sc, n_trials, st);
-  return t8 ? launch_one32<VMAX, CMAX, false, true, W>(kp, sc, n_trials, st) : launch_one32<VMAX, CMAX, false, false, W>(kp, sc, n_trials, st);
-}
-
-template <int VMAX, int CMAX>
-cudaError_t launch_v32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  return sc.warps_per_cta == 4 ? launch_w32<VMAX, CMAX, 4>(kp, sc, n_trials, st) : launch_w32<VMAX, CMAX, 8>(kp, sc, n_trials, st);
-}
-
-cudaError_t launch_sims32(const KParams& kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
-  if (sc.cmax == 8) return launch_v32<8, 8>(kp, sc, n_trials, st);
-  if (sc.vmax32 == 2) return launch_v32<2, 6>(kp, sc, n_trials, st);
-  if (sc.vmax32 == 4) return launch_v32<4, 6>(kp, sc, n_trials, st);
-  if (sc.vmax32 == 6) return launch_v32<6, 6>(kp, sc, n_trials, st);
-  return launch_v32<8, 6>(kp, sc, n_trials, st);
+cudaError_t launch_sims32(KParams kp, const Schedule& sc, uint32_t n_trials, cudaStream_t st) {
+  cudaError_t e;
+  const LaunchCfg lc = launch_cfg(sc, n_trials, true, &e);
+  if (e != cudaSuccess) return e;
+  kp.k_launch = n_trials;
+  ++g_launch_count;
+  if (sc.cmax == 8) return launch_k32_v8c8(kp, lc, st);
+  if (sc.vmax32 == 2) return launch_k32_v2c6(kp, lc, st);
+  if (sc.vmax32 == 4) return launch_k32_v4c6(kp, lc, st);
+  if (sc.vmax32 == 6) return launch_k32_v6c6(kp, lc, st);
+  return launch_k32_v8c6(kp, lc, st);
 }
 
 // The 32-bit kernel needs max(A, F) + S + delay to stay below 2^32 whenever its inputs are inside the
 // 2^31 window: the worst-case service of a request over all its stages plus all its hops is capped
 // at 2^30. Anything else runs on the 64-bit kernel alone.
-bool fast_path_ok(const cf_graph* g) {
-  if (g_kernel_mode == 1) return false;
+bool fast_path_ok(const cf_graph* g, uint32_t kernel_mode) {
+  if (kernel_mode == CF_KERNEL_WIDE64) return false;
   int64_t worst = 0;
   for (uint32_t i = 0; i < g->n_comp; ++i) {
     int64_t mx = 0;
@@ -612,13 +553,8 @@ cudaError_t launch_scan(KParams kp, const Schedule& sc, uint32_t n_trials, cudaS
   const uint64_t n_sims = (uint64_t)sc.plan_topo_v.size() * sc.R * n_trials;
   const uint64_t blocks = (n_sims + kScanWarps - 1) / kScanWarps;
   if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-  const uint32_t* pv = kp.stream ? kp.plan_var : nullptr;
-  if (sc.cmax == 8)
-    cf_scan_kernel<8><<<(uint32_t)blocks, kScanWarps * 32, 0, st>>>(kp, kp.plan_topo, pv, sc.R, (uint32_t)n_sims);
-  else
-    cf_scan_kernel<6><<<(uint32_t)blocks, kScanWarps * 32, 0, st>>>(kp, kp.plan_topo, pv, sc.R, (uint32_t)n_sims);
   ++g_launch_count;
-  return cudaGetLastError();
+  return launch_scan_k(sc.cmax, kp, (uint32_t)blocks, sc.R, (uint32_t)n_sims, st);
 }
 
 cudaError_t launch_pass(KParams kp, const Schedule& sc, uint32_t n_trials, bool fast, cudaStream_t st) {
@@ -646,7 +582,6 @@ int32_t check_workspace(void* ws, size_t have, size_t need) {
 // infeasible: hi = rate_i] and 2i+1 [feasible: lo = rate_i]); the update kernel then walks the path
 // the sequential algorithm would have taken. Every probe on that path is exactly the probe of the
 // sequential bisection, so results are identical; the other nodes only buy parallelism.
-constexpr uint32_t kMaxSpecDepth = 4;
 constexpr uint32_t kMaxSpecNodes = (1u << kMaxSpecDepth) - 1u;
 
 struct BisectState {
@@ -902,19 +837,30 @@ struct EvalArgs {
   const cf_graph* g; const cf_plans* pl; const uint32_t* rates_dev; uint32_t R; const cf_slo* slo;
   uint64_t seed; uint32_t variant; const void* stream_records; uint32_t n_variants;
   const uint32_t* plan_variant; uint32_t* out_counts; uint64_t* out_dep_sum; int64_t* out_makespan;
-  void* ws; size_t ws_bytes; cudaStream_t st;
+  void* ws; size_t ws_bytes; cudaStream_t st; cf_options opt;
 };
+
+cf_options options_of(const cf_options* o) {
+  cf_options d;
+  std::memset(&d, 0, sizeof(d));
+  return o ? *o : d;
+}
+int32_t check_options(const cf_options& o) {
+  return (o.kernel_mode > CF_KERNEL_SCAN || o.bisect_depth > kMaxSpecDepth) ? CF_ERR_ARG : CF_OK;
+}
 
 int32_t eval_impl(const EvalArgs& a) {
   g_launch_count = 0;
+  if (int32_t rc = check_options(a.opt)) return rc;
   if (int32_t rc = check_graph(a.g)) return rc;
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
   if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
-  const bool fast = fast_path_ok(a.g);
+  const bool fast = fast_path_ok(a.g, a.opt.kernel_mode);
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast,
+                                  a.opt.kernel_mode, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);  // status block
@@ -941,11 +887,12 @@ struct BisectArgs {
   const cf_graph* g; const cf_plans* pl; const uint32_t* rate_hi_dev; uint32_t n_steps; const cf_slo* slo;
   uint64_t seed; uint32_t variant; const void* stream_records; uint32_t n_variants;
   const uint32_t* plan_variant; uint32_t* out_rate; uint32_t* out_goodput; uint32_t* out_counts;
-  void* ws; size_t ws_bytes; cudaStream_t st;
+  void* ws; size_t ws_bytes; cudaStream_t st; cf_options opt;
 };
 
 int32_t bisect_impl(const BisectArgs& a) {
   g_launch_count = 0;
+  if (int32_t rc = check_options(a.opt)) return rc;
   if (int32_t rc = check_graph(a.g)) return rc;
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rate_hi_dev || !a.slo || !a.slo->L_us || !a.slo->att_num || !a.slo->att_den || !a.out_rate || !a.out_goodput)
@@ -953,9 +900,9 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
-  const bool fast = fast_path_ok(a.g);
+  const bool fast = fast_path_ok(a.g, a.opt.kernel_mode);
   // speculation depth: enough simulations per pass to fill the GPU (one thread each), no more
-  uint32_t depth = g_spec_depth;
+  uint32_t depth = a.opt.bisect_depth;
   if (depth == 0) {
     depth = 1;
     while (depth < kMaxSpecDepth && (uint64_t)P * K * ((1u << depth) - 1u) < 90000ull) ++depth;
@@ -963,7 +910,8 @@ int32_t bisect_impl(const BisectArgs& a) {
   depth = std::min(depth, std::max(1u, a.n_steps));
   const uint32_t R = (1u << depth) - 1u;
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast, &sc))
+  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast,
+                                  a.opt.kernel_mode, &sc))
     return rc;
   Blob blob;
   blob.reserve(kAlign);
@@ -1055,12 +1003,33 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   return n + 4 * kAlign;
 }
 
+int32_t cf_eval_plans_opt(const cf_options* opt, const cf_graph* g, const cf_plans* pl,
+                          const uint32_t* rate_mrps, uint32_t R, const cf_slo* slo, uint64_t seed,
+                          uint32_t variant, uint32_t* out_counts, uint64_t* out_dep_sum,
+                          int64_t* out_makespan, void* workspace, size_t workspace_bytes, void* stream) {
+  EvalArgs a{g, pl, rate_mrps, R, slo, seed, variant, nullptr, 1, nullptr, out_counts, out_dep_sum,
+             out_makespan, workspace, workspace_bytes, static_cast<cudaStream_t>(stream), options_of(opt)};
+  return eval_impl(a);
+}
+
 int32_t cf_eval_plans(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps, uint32_t R,
                       const cf_slo* slo, uint64_t seed, uint32_t variant, uint32_t* out_counts,
                       uint64_t* out_dep_sum, int64_t* out_makespan, void* workspace,
                       size_t workspace_bytes, void* stream) {
-  EvalArgs a{g, pl, rate_mrps, R, slo, seed, variant, nullptr, 1, nullptr, out_counts, out_dep_sum,
-             out_makespan, workspace, workspace_bytes, static_cast<cudaStream_t>(stream)};
+  return cf_eval_plans_opt(nullptr, g, pl, rate_mrps, R, slo, seed, variant, out_counts, out_dep_sum,
+                           out_makespan, workspace, workspace_bytes, stream);
+}
+
+int32_t cf_eval_plans_stream_opt(const cf_options* opt, const cf_graph* g, const cf_plans* pl,
+                                 const uint32_t* rate_mrps, uint32_t R, const cf_slo* slo,
+                                 const void* stream_records, uint32_t n_variants,
+                                 const uint32_t* plan_variant, uint32_t* out_counts,
+                                 uint64_t* out_dep_sum, int64_t* out_makespan, void* workspace,
+                                 size_t workspace_bytes, void* stream) {
+  if (!stream_records) return CF_ERR_ARG;
+  EvalArgs a{g, pl, rate_mrps, R, slo, 0, 0, stream_records, n_variants, plan_variant, out_counts,
+             out_dep_sum, out_makespan, workspace, workspace_bytes, static_cast<cudaStream_t>(stream),
+             options_of(opt)};
   return eval_impl(a);
 }
 
@@ -1069,18 +1038,40 @@ int32_t cf_eval_plans_stream(const cf_graph* g, const cf_plans* pl, const uint32
                              uint32_t n_variants, const uint32_t* plan_variant,
                              uint32_t* out_counts, uint64_t* out_dep_sum, int64_t* out_makespan,
                              void* workspace, size_t workspace_bytes, void* stream) {
-  if (!stream_records) return CF_ERR_ARG;
-  EvalArgs a{g, pl, rate_mrps, R, slo, 0, 0, stream_records, n_variants, plan_variant, out_counts,
-             out_dep_sum, out_makespan, workspace, workspace_bytes, static_cast<cudaStream_t>(stream)};
-  return eval_impl(a);
+  return cf_eval_plans_stream_opt(nullptr, g, pl, rate_mrps, R, slo, stream_records, n_variants,
+                                  plan_variant, out_counts, out_dep_sum, out_makespan, workspace,
+                                  workspace_bytes, stream);
+}
+
+int32_t cf_goodput_bisect_opt(const cf_options* opt, const cf_graph* g, const cf_plans* pl,
+                              const uint32_t* rate_hi_mrps, uint32_t n_steps, const cf_slo* slo,
+                              uint64_t seed, uint32_t variant, uint32_t* out_rate_mrps,
+                              uint32_t* out_goodput_mrps, uint32_t* out_counts, void* workspace,
+                              size_t workspace_bytes, void* stream) {
+  BisectArgs a{g, pl, rate_hi_mrps, n_steps, slo, seed, variant, nullptr, 1, nullptr, out_rate_mrps,
+               out_goodput_mrps, out_counts, workspace, workspace_bytes, static_cast<cudaStream_t>(stream),
+               options_of(opt)};
+  return bisect_impl(a);
 }
 
 int32_t cf_goodput_bisect(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_hi_mrps,
                           uint32_t n_steps, const cf_slo* slo, uint64_t seed, uint32_t variant,
                           uint32_t* out_rate_mrps, uint32_t* out_goodput_mrps, uint32_t* out_counts,
                           void* workspace, size_t workspace_bytes, void* stream) {
-  BisectArgs a{g, pl, rate_hi_mrps, n_steps, slo, seed, variant, nullptr, 1, nullptr, out_rate_mrps,
-               out_goodput_mrps, out_counts, workspace, workspace_bytes, static_cast<cudaStream_t>(stream)};
+  return cf_goodput_bisect_opt(nullptr, g, pl, rate_hi_mrps, n_steps, slo, seed, variant, out_rate_mrps,
+                               out_goodput_mrps, out_counts, workspace, workspace_bytes, stream);
+}
+
+int32_t cf_goodput_bisect_stream_opt(const cf_options* opt, const cf_graph* g, const cf_plans* pl,
+                                     const uint32_t* rate_hi_mrps, uint32_t n_steps, const cf_slo* slo,
+                                     const void* stream_records, uint32_t n_variants,
+                                     const uint32_t* plan_variant, uint32_t* out_rate_mrps,
+                                     uint32_t* out_goodput_mrps, uint32_t* out_counts,
+                                     void* workspace, size_t workspace_bytes, void* stream) {
+  if (!stream_records) return CF_ERR_ARG;
+  BisectArgs a{g, pl, rate_hi_mrps, n_steps, slo, 0, 0, stream_records, n_variants, plan_variant,
+               out_rate_mrps, out_goodput_mrps, out_counts, workspace, workspace_bytes,
+               static_cast<cudaStream_t>(stream), options_of(opt)};
   return bisect_impl(a);
 }
 
@@ -1090,11 +1081,9 @@ int32_t cf_goodput_bisect_stream(const cf_graph* g, const cf_plans* pl,
                                  const uint32_t* plan_variant, uint32_t* out_rate_mrps,
                                  uint32_t* out_goodput_mrps, uint32_t* out_counts, void* workspace,
                                  size_t workspace_bytes, void* stream) {
-  if (!stream_records) return CF_ERR_ARG;
-  BisectArgs a{g, pl, rate_hi_mrps, n_steps, slo, 0, 0, stream_records, n_variants, plan_variant,
-               out_rate_mrps, out_goodput_mrps, out_counts, workspace, workspace_bytes,
-               static_cast<cudaStream_t>(stream)};
-  return bisect_impl(a);
+  return cf_goodput_bisect_stream_opt(nullptr, g, pl, rate_hi_mrps, n_steps, slo, stream_records,
+                                      n_variants, plan_variant, out_rate_mrps, out_goodput_mrps,
+                                      out_counts, workspace, workspace_bytes, stream);
 }
 
 size_t cf_stream_bytes(const cf_graph* g, uint32_t n_variants) {
@@ -1139,18 +1128,24 @@ int32_t cf_materialize_stream(const cf_graph* g, uint64_t seed, uint32_t variant
   return cuda_rc(cudaGetLastError());
 }
 
-int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint32_t rate_mrps,
-                     uint32_t trial, uint64_t seed, uint32_t variant, int64_t* out_arrival,
-                     int64_t* out_departure, uint8_t* out_type, void* workspace,
-                     size_t workspace_bytes, void* stream) {
+int32_t cf_trace_sim_opt(const cf_options* opt_in, const cf_graph* g, const cf_plans* pl, uint32_t plan,
+                         uint32_t rate_mrps, uint32_t trial, uint64_t seed, uint32_t variant,
+                         int64_t* out_arrival, int64_t* out_departure, uint8_t* out_type,
+                         void* workspace, size_t workspace_bytes, void* stream) {
   g_launch_count = 0;
+  const cf_options opt = options_of(opt_in);
+  if (int32_t rc = check_options(opt)) return rc;
   if (int32_t rc = check_graph(g)) return rc;
   if (int32_t rc = check_plans(g, pl)) return rc;
   if (plan >= pl->n_plans || trial >= g->n_trials) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(workspace, workspace_bytes, cf_workspace_bytes(g, pl, 1))) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  // default: the 64-bit kernel; CF_KERNEL_FAST32 / CF_KERNEL_SCAN trace the kernels that do the
+  // benchmarked work (the fast kernel followed by its fixup pass, or the max-plus scan kernel)
+  const bool fast = opt.kernel_mode == CF_KERNEL_FAST32;
+  if (fast && !fast_path_ok(g, opt.kernel_mode)) return CF_ERR_ARG;
   Schedule sc;
-  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, false, &sc)) return rc;
+  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, fast, opt.kernel_mode, &sc)) return rc;
   // the single simulation reads rate slot `plan` (pr = plan*1 + 0): upload a full-length rate array
   Blob blob;
   blob.reserve(kAlign);
@@ -1162,6 +1157,7 @@ int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint3
   std::vector<uint32_t> rates(pl->n_plans, rate_mrps);
   const size_t rate_off = blob.add(rates.data(), rates.size() * 4);
   const size_t scratch_off = blob.reserve((size_t)pl->n_plans * g->n_trials * g->n_types * 2 * 4);
+  const size_t flags_off = blob.reserve((size_t)pl->n_plans * g->n_trials);
   if (blob.bytes.size() > workspace_bytes) return CF_ERR_WORKSPACE;
   uint8_t* ws = static_cast<uint8_t*>(workspace);
   if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st)))
@@ -1170,11 +1166,26 @@ int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint3
   kp.variant_lo = variant;
   kp.rates = reinterpret_cast<const uint32_t*>(ws + rate_off);
   kp.out_counts = reinterpret_cast<uint32_t*>(ws + scratch_off);
+  kp.flags = ws + flags_off;
   kp.tr_arrival = out_arrival;
   kp.tr_departure = out_departure;
   kp.tr_type = out_type;
+  kp.tr_plan = plan;
   kp.trial_base = trial;
+  if (sc.all_c1) return cuda_rc(launch_scan(kp, sc, 1, st));
+  if (fast) {
+    if (int32_t rc = cuda_rc(launch_sims32(kp, sc, 1, st))) return rc;
+    kp.fixup = 1;
+  }
   return cuda_rc(launch_sims(kp, sc, 1, st));
+}
+
+int32_t cf_trace_sim(const cf_graph* g, const cf_plans* pl, uint32_t plan, uint32_t rate_mrps,
+                     uint32_t trial, uint64_t seed, uint32_t variant, int64_t* out_arrival,
+                     int64_t* out_departure, uint8_t* out_type, void* workspace,
+                     size_t workspace_bytes, void* stream) {
+  return cf_trace_sim_opt(nullptr, g, pl, plan, rate_mrps, trial, seed, variant, out_arrival,
+                          out_departure, out_type, workspace, workspace_bytes, stream);
 }
 
 int32_t cf_workspace_status(const void* workspace, void* stream) {
@@ -1188,24 +1199,12 @@ int32_t cf_workspace_status(const void* workspace, void* stream) {
 
 uint32_t cf_last_launch_count(void) { return g_launch_count; }
 
-int32_t cf_debug_kernel_mode(uint32_t mode) {
-  if (mode > 1) return CF_ERR_ARG;
-  g_kernel_mode = mode;
-  return CF_OK;
-}
-
 int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_probes, void* stream) {
   if (!workspace || !out_probes) return CF_ERR_ARG;
   cudaError_t e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
   if (e == cudaSuccess)
     e = cudaMemcpy(out_probes, static_cast<const uint8_t*>(workspace) + kAlign, (size_t)n_plans * 4, cudaMemcpyDeviceToHost);
   return e == cudaSuccess ? CF_OK : cuda_rc(e);
-}
-
-int32_t cf_debug_bisect_depth(uint32_t depth) {
-  if (depth > kMaxSpecDepth) return CF_ERR_ARG;
-  g_spec_depth = depth;
-  return CF_OK;
 }
 
 int64_t cf_workspace_wide_count(const void* workspace, void* stream) {

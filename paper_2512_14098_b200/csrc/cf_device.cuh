@@ -96,6 +96,7 @@ struct KParams {
   int64_t* tr_arrival;     // trace (single simulation) or null
   int64_t* tr_departure;
   uint8_t* tr_type;
+  uint32_t tr_plan;        // the traced plan (scan kernel: the warp whose simulation is written out)
 };
 
 // ------------------------------------------------------------------------------------------------

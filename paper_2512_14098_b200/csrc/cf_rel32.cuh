@@ -16,8 +16,9 @@
 //     minimum of the four packed words is the minimum key AND names its slot: no index arithmetic;
 //   * the per-request record lists only the stages the request visits (stage ids + services), so a
 //     stage that is not visited costs nothing; per-lane stage state lives in shared memory;
-//   * a8: hit <=> x <= (A_n - O) + min(L_t, 2^31-1); per-type hit counters are byte fields of two
-//     32-bit words flushed once per tile.
+//   * a8: hit <=> x - (A_n - O) <= min(L_t, 2^32-1) (a sojourn of 2^32 us or more under a clamped
+//     target leaves the fast path); per-type hit counters are byte fields of two 32-bit words
+//     flushed every 4 chunks.
 //
 // At every tile boundary the origin moves forward and every stage base moves to
 // max(earliest free time of the stage, new origin); keys below the new base are clamped to it.
@@ -44,7 +45,7 @@ constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kKeyLimit = (1u << 30) - 4u;  // keys must stay below this
 
 // Stage-level record of the fast kernel (a warp builds 32 of them per chunk for its topology):
-//   w0 = { d (tile-relative cumulative gap, Q16), min(L_t, 2^31-1), hit increment for types 0..3,
+//   w0 = { d (tile-relative cumulative gap, Q16), min(L_t, 2^32-1), hit increment for types 0..3,
 //          hit increment for types 4..7 }   (one byte field per type; 0 if L_t < 0)
 //   w1 = { stage ids of visits 0..3 (one byte each, 0xff = end), of visits 4..7, S_0, S_1 }
 //   w2 = { S_2 .. S_5 },  w3 = { S_6, S_7, -, - }        (S_j = service of the j-th visit)
@@ -140,7 +141,9 @@ __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint
 
 // T8: more than 4 request types (a second word of hit-counter byte fields); WARPS per thread block
 // (16 warps per SM either way: 124-128 registers per thread)
-template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int WARPS>
+// TRACE (cf_trace_sim through this kernel): the call holds one simulation, lane 0 of warp 0; it
+// writes every request's system arrival and final departure, the warp's lanes the request types
+template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int WARPS, bool TRACE = false>
 __global__ void __launch_bounds__(WARPS * 32, 16 / WARPS)
 cf_sim32_kernel(const __grid_constant__ KParams prm) {
   using SL = SmemLayout32<VMAX, CMAX, WARPS>;
@@ -164,7 +167,9 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   if (tid < 8) {
     cnt_s[tid] = 0;
     const int64_t L = prm.L_us[tid];
-    l32_s[tid] = (uint32_t)(L < 0 ? 0 : (L > 0x7fffffffll ? 0x7fffffffll : L));
+    // L >= 2^32-1 is held as 2^32-1: exact while the sojourn fits 32 bits; a longer sojourn that
+    // misses this bound sends the lane to the 64-bit kernel (see the a8 test below)
+    l32_s[tid] = (uint32_t)(L < 0 ? 0 : (L > 0xffffffffll ? 0xffffffffll : L));
     const uint32_t one = (L < 0) ? 0u : (1u << (8 * (tid & 3)));  // L < 0: never a hit
     inc_s[tid] = make_uint2(tid < 4 ? one : 0u, tid < 4 ? 0u : one);
   }
@@ -311,6 +316,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           svc[6] = 0; svc[7] = 0;
           if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
           const uint32_t t = w0.y >> 24;
+          if (TRACE && warp == 0 && lane < n_here && prm.tr_type) prm.tr_type[nc0 + lane] = (uint8_t)t;
           const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;  // absolute
           const uint64_t d64 = cu - tile_base;
           if (__any_sync(kFull, lane < n_here && (d64 >> 32) != 0)) flagged = true;  // tile too long
@@ -421,13 +427,20 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
             if (nq512) key = heap4_replace_min(hb, nq512, key, q);
             sts32(sa + 8u, key);
           }
+          if (TRACE && tid == 0) {  // lane 0 of warp 0 is the traced simulation
+            const uint32_t n = nc0 + (uint32_t)r;
+            if (prm.tr_arrival) prm.tr_arrival[n] = (int64_t)(origin + a);
+            if (prm.tr_departure) prm.tr_departure[n] = (int64_t)(origin + (uint64_t)x);
+          }
           // a8
           if (NARROW) {
-            if ((uint32_t)x <= a + w0.y) { hlo += w0.z; if (T8) hhi += w0.w; }
+            if ((uint32_t)x - a <= w0.y) { hlo += w0.z; if (T8) hhi += w0.w; }  // sojourn < 2^32 here
             dep = mad_wide_u32((uint32_t)x, 1u, dep);
             mk32 = max(mk32, (uint32_t)x);
           } else {
-            if ((uint64_t)x <= (uint64_t)a + w0.y) { hlo += w0.z; if (T8) hhi += w0.w; }
+            const uint64_t soj = (uint64_t)x - a;
+            if (soj <= (uint64_t)w0.y) { hlo += w0.z; if (T8) hhi += w0.w; }
+            else if (w0.y == 0xffffffffu) flagged = true;  // L_t >= 2^32-1 was clamped: the 64-bit kernel decides
             dep += (uint64_t)x;
             mk = (uint64_t)x > mk ? (uint64_t)x : mk;
           }

@@ -112,6 +112,11 @@ cf_scan_kernel(const __grid_constant__ KParams prm, const uint32_t* __restrict__
           carry[s] = __shfl_sync(0xffffffffu, D, 31);
         }
       }
+      if (valid && plan == prm.tr_plan && sim % prm.k_launch == 0) {  // cf_trace_sim through this kernel (R = 1)
+        if (prm.tr_arrival) prm.tr_arrival[n0 + lane] = A;
+        if (prm.tr_departure) prm.tr_departure[n0 + lane] = x;
+        if (prm.tr_type) prm.tr_type[n0 + lane] = (uint8_t)t;
+      }
       // a8
       const bool hit = valid && (x - A) <= prm.L_us[t];
       for (uint32_t tt = 0; tt < prm.T; ++tt) {

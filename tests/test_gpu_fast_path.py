@@ -117,6 +117,25 @@ def test_negative_and_huge_latency_targets(cf, orc):
     eval_both_modes(cf, orc, w)
 
 
+def test_latency_targets_beyond_32_bits_with_long_sojourns(cf, orc):
+    # 3x overload, 20 000 requests of 1 s: sojourns grow past 2^31 and 2^32 us. Targets
+    # between 2^31 and 2^32 must be exact inside the fast kernel; targets of 2^32 or more ("no
+    # target") are held clamped there and the lanes whose sojourn passes the clamp are redone by
+    # the 64-bit kernel. Hits must match the oracle either way.
+    for L, expect_fixups in ((3_000_000_000, False), ((1 << 32) - 1, None), (1 << 40, True), (2**63 - 1, True)):
+        w = one_stage(W.lognormal_qtab(1_000_000.0, 0.3), W.exponential_qtab(65536.0), 20_000, (1, 2, 5),
+                      (3000, 6000, 15_000), L=(L,), n_trials=1)
+        wide = eval_both_modes(cf, orc, w)
+        want = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, n_threads=NT)
+        hits = want["counts"][..., 0, 1]
+        if L >= 1 << 40:
+            np.testing.assert_array_equal(hits, want["counts"][..., 0, 0])  # every request is a hit
+        else:
+            assert (hits < want["counts"][..., 0, 0]).any() and (hits > 0).all()
+        if expect_fixups is not None:
+            assert (wide > 0) == expect_fixups
+
+
 def test_speculative_bisection_depths(cf, orc):
     w = W.config2_omni(n_req=600, n_trials=2, n_rates=2, vectors_per_pattern=2, n_patterns=16)
     R_p = W.flow_bound_mrps(w.graph, w.plans)

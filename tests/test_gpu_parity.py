@@ -107,17 +107,100 @@ def test_cfg4_reduced_stream_and_bisect(cf, orc):
 # ---------------------------------------------------------------------------------------------
 # traces, edge cases
 # ---------------------------------------------------------------------------------------------
+def check_trace(cf, orc, g, pl, p, rate, k, seed, variant, modes):
+    o = orc.trace_sim(g, pl, p, rate, k, seed, variant=variant)
+    for mode in modes:
+        cf.cf_debug_kernel_mode(mode)
+        try:
+            t = cf.cf_trace_sim(g, pl, p, rate, k, seed, variant=variant)
+        finally:
+            cf.cf_debug_kernel_mode(0)
+        assert t["status"] == o["rc"] == 0
+        np.testing.assert_array_equal(t["arrival"].cpu().numpy(), o["arrival"], err_msg=f"mode {mode}")
+        np.testing.assert_array_equal(t["departure"].cpu().numpy(), o["departure"], err_msg=f"mode {mode}")
+        np.testing.assert_array_equal(t["type"].cpu().numpy(), o["type"], err_msg=f"mode {mode}")
+        if mode == cf.CF_KERNEL_FAST32:
+            assert t["wide"] == 0  # the departures came from the fast kernel, not from its fixup pass
+    return o
+
+
 def test_trace_matches_oracle(cf, orc):
+    """Per-request arrivals, departures and types of the 64-bit kernel, the fast kernel (the one
+    that does the benchmarked work) and -- for one-replica plans -- the max-plus scan kernel."""
     w = W.config2_omni(n_req=777, n_trials=3, n_rates=2, vectors_per_pattern=2, n_patterns=8)
     w.graph.edge_delay_us = 10_000
+    both = (cf.CF_KERNEL_AUTO, cf.CF_KERNEL_WIDE64, cf.CF_KERNEL_FAST32)
     for p in (0, 3, 7, 15):
         for k in (0, 2):
-            rate = int(w.rate_mrps[p, 1])
-            t = cf.cf_trace_sim(w.graph, w.plans, p, rate, k, w.seed, variant=5)
-            o = orc.trace_sim(w.graph, w.plans, p, rate, k, w.seed, variant=5)
-            np.testing.assert_array_equal(t["arrival"].cpu().numpy(), o["arrival"])
-            np.testing.assert_array_equal(t["departure"].cpu().numpy(), o["departure"])
-            np.testing.assert_array_equal(t["type"].cpu().numpy(), o["type"])
+            check_trace(cf, orc, w.graph, w.plans, p, int(w.rate_mrps[p, 1]), k, w.seed, 5, both)
+    # overloaded (waits grow without bound: the 64-bit request body and mid-chunk mode changes) and
+    # sparse arrivals (1 and 40 mrps: hours between requests, per-request origin moves)
+    w = W.config3_multireplica(n_req=2500, n_trials=2, n_rates=2, plans_per_topology=6)
+    R_p = W.flow_bound_mrps(w.graph, w.plans)
+    for p in (1, 8, 13, 22):
+        o = check_trace(cf, orc, w.graph, w.plans, p, int(3.0 * R_p[p]), 1, w.seed, 0, both)
+        assert (o["departure"] - o["arrival"]).max() > 10 * (o["departure"] - o["arrival"])[:20].max()
+        for rate in (1, 40):
+            check_trace(cf, orc, w.graph, w.plans, p, rate, 0, w.seed, 2, both)
+    # long overload: departures beyond 2^32 us while the keys stay in the window
+    g = W.Graph(1, 1, 9000, 1, [1], W.mix_thresholds([1.0]), [0], [W.lognormal_qtab(1_000_000.0, 0.3)],
+                W.exponential_qtab(65536.0), np.zeros((0, 2)))
+    o = check_trace(cf, orc, g, W.make_plans([[(1, 2)], [(1, 1)]]), 0, 6000, 0, 11, 0, both)
+    assert o["departure"].max() > 1 << 32
+    # one replica at every stage: all four paths, the scan kernel included
+    w = W.config2_omni(n_req=1000, n_trials=2, n_rates=2, vectors_per_pattern=1, n_patterns=32)
+    w.plans = W.Plans(w.plans.n_stages, w.plans.stage_mask, np.ones_like(w.plans.stage_c))
+    w.graph.edge_delay_us = 333
+    R_p = W.flow_bound_mrps(w.graph, w.plans)
+    for p in (0, 9, 31):
+        for rate in (1, int(0.8 * R_p[p]), int(2.5 * R_p[p])):
+            check_trace(cf, orc, w.graph, w.plans, p, max(rate, 1), 1, w.seed, 7, both + (cf.CF_KERNEL_SCAN,))
+    # the scan kernel refuses a plan with more than one replica
+    w2 = W.config1_mllm(n_req=100, n_trials=1, n_rates=1, llm_max=4, e_steps=2)
+    cf.cf_debug_kernel_mode(cf.CF_KERNEL_SCAN)
+    try:
+        assert cf.cf_trace_sim(w2.graph, w2.plans, 3, 1000, 0, 1, check=False)["rc"] == cf.CF_ERR_ARG
+    finally:
+        cf.cf_debug_kernel_mode(0)
+
+
+@pytest.mark.parametrize("L,B", [(1, 10), (1, 0), (4, 3), (32, 2), (8, 16), (20, 0), (16, 6)])
+def test_quantile_table_shapes(cf, orc, L, B):
+    """The device table lookup at every (levels, log2_cells) shape the oracle's geometric pin covers
+    (tests/test_oracle_draws.py), through cf_eval_plans (both kernels), the materialised stream and
+    the max-plus scan kernel: service AND arrival tables of that shape, random monotone entries."""
+    rng = np.random.default_rng(L * 100 + B)
+    n = (L << B) + 1
+    tabs = [W.QTab(L, B, np.sort(rng.integers(0, 40_000, n)).astype(np.int32)),
+            W.QTab(L, B, np.sort(rng.integers(0, 300_000, n)).astype(np.int32))]
+    arr = W.QTab(L, B, np.sort(rng.integers(0, 4 * 65536, n)).astype(np.int32))
+    g = W.Graph(2, 2, 1100, 2, [0b10, 0b11], W.mix_thresholds([0.6, 0.4]), [0, 0, 1, 1], tabs, arr, [[0, 1]],
+                edge_delay_us=77)
+    pl = W.make_plans([[(0b11, 3)], [(0b01, 1), (0b10, 2)], [(0b01, 2), (0b10, 7)], [(0b11, 1)]], max_stages=2)
+    rates = np.maximum(W.rate_grid(W.flow_bound_mrps(g, pl), [0.5, 0.9, 1.3]), 1)
+    w = W.Workload("shapes", g, pl, W.Slo([400_000, 600_000], [9, 9], [10, 10]), seed=L * 1000 + B, rate_mrps=rates)
+    want = orc.eval_plans(g, pl, rates, w.slo, w.seed, 4, n_threads=NT)
+    for mode in (0, 1):
+        cf.cf_debug_kernel_mode(mode)
+        try:
+            got = cf.cf_eval_plans(g, pl, rates, w.slo, w.seed, 4)
+        finally:
+            cf.cf_debug_kernel_mode(0)
+        np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+        np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+    rec = cf.cf_materialize_stream(g, w.seed, 4, 2)
+    np.testing.assert_array_equal(rec.cpu().numpy().reshape(-1),
+                                  orc.materialize_stream(g, w.seed, 4, 2).view(np.uint8).reshape(-1))
+    got = cf.cf_eval_plans(g, pl, rates, w.slo, w.seed, stream_records=rec, n_variants=2,
+                           plan_variant=np.zeros(4, np.uint32))
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    # one replica everywhere: the scan kernel draws with the same lookup
+    pl1 = W.Plans(pl.n_stages, pl.stage_mask, np.ones_like(pl.stage_c))
+    want1 = orc.eval_plans(g, pl1, rates, w.slo, w.seed, 4, n_threads=NT)
+    got1 = cf.cf_eval_plans(g, pl1, rates, w.slo, w.seed, 4)
+    np.testing.assert_array_equal(cf.to_numpy_u32(got1["counts"]), want1["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u64(got1["dep_sum"]), want1["dep_sum"])
 
 
 def test_edge_delay_and_variant(cf, orc):
@@ -206,6 +289,24 @@ def test_bisect_parity_and_degenerate_brackets(cf, orc):
         np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
 
 
+def test_bisect_out_of_range_probe_is_infeasible_r18(cf, orc):
+    # the hand-worked R18 case of tests/test_oracle_invariants.py, on the device
+    from test_oracle_invariants import R18_HI, R18_RATE, r18_case
+    g, pl1, slo = r18_case()
+    pl2 = W.make_plans([[(1, 2)]] * 4)  # two replicas: the thread-per-simulation kernels + fixup pass
+    for pl, depth in ((pl1, 0), (pl1, 1), (pl1, 3), (pl2, 0), (pl2, 2)):
+        cf.cf_debug_bisect_depth(depth)
+        try:
+            b = cf.cf_goodput_bisect(g, pl, R18_HI, 20, slo, 0)
+        finally:
+            cf.cf_debug_bisect_depth(0)
+        assert cf.cf_workspace_status(b["workspace"]) == cf.CF_ERR_RANGE
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), R18_RATE)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["goodput_mrps"])[:, 0], R18_RATE)
+        c = cf.to_numpy_u32(b["counts"])
+        assert (c[:2] == 0).all() and (c[2:] == 1 << 12).all()
+
+
 def test_host_errors_on_gpu(cf):
     w = W.config1_mllm(n_req=100, n_trials=1, n_rates=1, llm_max=2, e_steps=1)
     bad = W.make_plans([[(0b10, 1), (0b01, 1)]])
@@ -243,7 +344,7 @@ def sampled_full_size(cf, orc, w, n_samples, seed):
 
 def test_cfg1_full_size_sampled(cf, orc):
     w = W.config1_mllm()
-    counts = sampled_full_size(cf, orc, w, 12, 1)
+    counts = sampled_full_size(cf, orc, w, 64, 1)
     # R16: colocated plans with equal l+e are duplicates and must agree exactly (same rates)
     pl = w.plans
     seen = {}
@@ -255,11 +356,11 @@ def test_cfg1_full_size_sampled(cf, orc):
 
 
 def test_cfg2_full_size_sampled(cf, orc):
-    sampled_full_size(cf, orc, W.config2_omni(), 6, 2)
+    sampled_full_size(cf, orc, W.config2_omni(), 64, 2)
 
 
 def test_cfg3_full_size_sampled(cf, orc):
-    sampled_full_size(cf, orc, W.config3_multireplica(), 8, 3)
+    sampled_full_size(cf, orc, W.config3_multireplica(), 64, 3)
 
 
 def test_cfg4_full_size_sampled(cf, orc):
@@ -275,7 +376,7 @@ def test_cfg4_full_size_sampled(cf, orc):
     counts = cf.to_numpy_u32(b["counts"])
     probes = cf.cf_bisect_probes(b["workspace"], w.plans.n_plans)
     rng = np.random.default_rng(4)
-    for p in rng.integers(0, w.plans.n_plans, 4):
+    for p in rng.integers(0, w.plans.n_plans, 16):
         idx = np.array([p])
         bo = orc.goodput_bisect(w.graph, w.plans.subset(idx), w.rate_hi_mrps[idx], w.n_steps, w.slo, w.seed,
                                 int(w.plan_variant[p]), n_threads=NT)

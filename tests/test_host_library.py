@@ -23,13 +23,16 @@ def cf():
 
 
 def test_exports_every_declared_symbol(cf):
-    hdr = open(os.path.join(ROOT, "include", "cf.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(cf_[a-z0-9_]+)\s*\(", hdr))
-    assert declared == set(cf.EXPORTS), declared ^ set(cf.EXPORTS)
     lib = C.CDLL(cf.LIB_PATH)
-    for name in declared:
-        assert hasattr(lib, name), name
+    for header, exports in (("cf.h", cf.EXPORTS), ("cf_debug.h", cf.DEBUG_EXPORTS)):
+        hdr = open(os.path.join(ROOT, "include", header)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        declared = set(re.findall(r"\b(cf_[a-z0-9_]+)\s*\(", hdr))
+        assert declared == set(exports), (header, declared ^ set(exports))
+        for name in declared:
+            assert hasattr(lib, name), name
+    # the product header declares no test knob
+    assert not [n for n in cf.EXPORTS if "debug" in n or "bench" in n or n.endswith("_opt")]
 
 
 def test_strerror(cf):

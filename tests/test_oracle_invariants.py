@@ -175,6 +175,40 @@ def test_bisect_zero_and_closed_bracket(orc):
     assert int(b["rate_mrps"][0]) == 0
 
 
+def r18_case():
+    """Constant gaps of 2^31-1 Q16 units, N = 2^12: CU_N = 2^43 - 2^12, so the R17 horizon
+    CU_N * period + 2^15 < 2^62 holds iff period <= 524288, i.e. iff rate >= 1908 mrps
+    (round(1e9/1908) = 524109, round(1e9/1907) = 524384). Service 5 us <= L = 10 us and hours
+    between arrivals: every in-range probe is feasible with every request a hit."""
+    g = W.Graph(1, 1, 1 << 12, 2, [1], W.mix_thresholds([1.0]), [0], [W.constant_qtab(5)],
+                W.constant_qtab(2**31 - 1), np.zeros((0, 2)))
+    return g, W.make_plans([[(1, 1)]] * 4), W.Slo([10], [9], [10])
+
+
+# bracket hi -> rate* worked by hand from the rule "an out-of-range probe is infeasible" (R18):
+#  3000: mids 1500, 750, ... all out of range                      -> 0
+#  3814: mid 1907 out of range -> hi = 1907, then as above          -> 0
+#  3816: mid 1908 in range, feasible -> lo = 1908; 2862, 3339, ... -> 3815
+#  4000: mid 2000 feasible; 3000, 3500, ...                         -> 3999
+R18_HI = np.array([3000, 3814, 3816, 4000], dtype=np.uint32)
+R18_RATE = np.array([0, 0, 3815, 3999], dtype=np.uint32)
+
+
+def test_bisect_out_of_range_probe_is_infeasible_r18(orc):
+    g, pl, slo = r18_case()
+    assert (10**9 + 1908 // 2) // 1908 == 524109 and (10**9 + 1907 // 2) // 1907 == 524384
+    cu_n = (1 << 12) * (2**31 - 1)
+    assert cu_n * 524288 + 32768 < 1 << 62 <= cu_n * 524289 + 32768
+    b = orc.goodput_bisect(g, pl, R18_HI, 20, slo, seed=0)
+    assert b["rc"] == orc.ORC_ERR_RANGE                       # the sticky status is still raised
+    np.testing.assert_array_equal(b["rate_mrps"], R18_RATE)
+    np.testing.assert_array_equal(b["goodput_mrps"][:, 0], R18_RATE)  # every request a hit: rate* x 1
+    assert (b["counts"][:2] == 0).all() and (b["counts"][2:] == 1 << 12).all()
+    # a bracket that never probes out of range raises nothing
+    b = orc.goodput_bisect(g, pl.subset([3]), R18_HI[3:], 20, slo, seed=0)
+    assert b["rc"] == 0 and int(b["rate_mrps"][0]) == 3999
+
+
 @pytest.mark.parametrize("s_ms,lam", [(5.0, 176.97), (20.0, 26.97)])
 def test_bisect_mm1_closed_form(orc, s_ms, lam):
     # lambda* = 1/s - ln(10)/L (SURVEY.md 8(c)); statistical, a few percent

@@ -143,18 +143,19 @@ uint32_t fixed_smem(int vmax, int cmax, int warps) {
   return warps == 4 ? fixed_smem_w<4>(vmax, cmax) : fixed_smem_w<8>(vmax, cmax);
 }
 
-template <int W>
+template <int W, bool PW>
 uint32_t fixed_smem32_w(int vmax, int cmax) {
   if (cmax <= 6) {
-    if (vmax <= 2) return SmemLayout32<2, 6, W>::fixed_bytes;
-    if (vmax <= 4) return SmemLayout32<4, 6, W>::fixed_bytes;
-    if (vmax <= 6) return SmemLayout32<6, 6, W>::fixed_bytes;
-    return SmemLayout32<8, 6, W>::fixed_bytes;
+    if (vmax <= 2) return SmemLayout32<2, 6, W, PW>::fixed_bytes;
+    if (vmax <= 4) return SmemLayout32<4, 6, W, PW>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout32<6, 6, W, PW>::fixed_bytes;
+    return SmemLayout32<8, 6, W, PW>::fixed_bytes;
   }
-  return SmemLayout32<8, 8, W>::fixed_bytes;
+  return SmemLayout32<8, 8, W, false>::fixed_bytes;
 }
-uint32_t fixed_smem32(int vmax, int cmax, int warps) {
-  return warps == 4 ? fixed_smem32_w<4>(vmax, cmax) : fixed_smem32_w<8>(vmax, cmax);
+uint32_t fixed_smem32(int vmax, int cmax, int warps, bool pw) {
+  if (pw) return fixed_smem32_w<4, true>(vmax, cmax);  // materialised stream: blocks of 4 warps
+  return warps == 4 ? fixed_smem32_w<4, false>(vmax, cmax) : fixed_smem32_w<8, false>(vmax, cmax);
 }
 
 // registers per thread of the kernel variant the schedule selects (occupancy model of the packing)
@@ -171,8 +172,8 @@ int kernel_regs32(int vmax, int cmax);
 // fast: pack for the 32-bit kernel (its heap rows set the occupancy); the 64-bit kernel then reuses
 // the same warps and blocks with its own, larger heap offsets.
 int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
-                       const uint32_t* plan_variant, uint32_t n_variants, const uint32_t* only_plan,
-                       bool fast, uint32_t kernel_mode, Schedule* out) {
+                       const uint32_t* plan_variant, uint32_t n_variants, bool streamed,
+                       const uint32_t* only_plan, bool fast, uint32_t kernel_mode, Schedule* out) {
   const uint32_t P = pl->n_plans, MS = pl->max_stages;
   Schedule& sc = *out;
   sc.plan_c.assign((size_t)P * 8, 1);
@@ -220,10 +221,13 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   // 8 warps per block amortise the tile over more simulations and win when a warp's lanes are
   // alike (>= 8 rates per plan); with many different plans per warp (bisection passes, few rates)
   // warps of a block drift apart between the per-tile barriers and 4 per block are faster (measured)
-  sc.warps_per_cta = R >= 8 ? 8 : 4;
+  // materialised stream (n_variants >= 1 records passed): every warp reads its own chunks, a block
+  // has no barrier and may mix stream variants; blocks of 4 warps
+  const bool pw = streamed;
+  sc.warps_per_cta = (R >= 8 && !pw) ? 8 : 4;
   const uint32_t kWarpsPerCta = (uint32_t)sc.warps_per_cta;
   const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax, sc.warps_per_cta),
-                 fixed_f = fixed_smem32(sc.vmax32, sc.cmax, sc.warps_per_cta);
+                 fixed_f = fixed_smem32(sc.vmax32, sc.cmax, sc.warps_per_cta, pw);
   const uint32_t fixed = fast ? fixed_f : fixed_w;  // the layout that is packed for occupancy
 
   std::vector<uint32_t> order;
@@ -330,14 +334,15 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       wi.heap_bytes = fast ? wi.heap_f : wi.heap_w;
       wi.cost = cost;
       wi.variant = variant_of(order[i]);
+      wi.wd.variant = wi.variant;
       if (fixed_w + wi.heap_w > kMaxSmem) return CF_ERR_RANGE;  // replica counts too large for one SM
       winfo.push_back(wi);
     }
     i = j;
   }
   // warps of equal expected cost together: a block advances tile by tile at the pace of its slowest warp
-  std::stable_sort(winfo.begin(), winfo.end(), [](const WarpInfo& a, const WarpInfo& b) {
-    if (a.variant != b.variant) return a.variant < b.variant;
+  std::stable_sort(winfo.begin(), winfo.end(), [pw](const WarpInfo& a, const WarpInfo& b) {
+    if (!pw && a.variant != b.variant) return a.variant < b.variant;
     if (a.cost != b.cost) return a.cost > b.cost;
     return a.heap_bytes > b.heap_bytes;
   });
@@ -354,7 +359,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
     while (w < winfo.size()) {
       CtaDesc cd{(uint32_t)w, 0, winfo[w].variant, 0, 0};
       uint32_t packed = 0;  // heap bytes of the layout being packed
-      while (w < winfo.size() && cd.n_warps < kWarpsPerCta && winfo[w].variant == cd.variant &&
+      while (w < winfo.size() && cd.n_warps < kWarpsPerCta && (pw || winfo[w].variant == cd.variant) &&
              (cd.n_warps == 0 || (fixed + packed + winfo[w].heap_bytes <= budget &&
                                   fixed_w + cd.heap_bytes + winfo[w].heap_w <= kMaxSmem))) {
         if (assign) {
@@ -859,7 +864,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   const bool fast = fast_path_ok(a.g, a.opt.kernel_mode);
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast,
+  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, a.stream_records != nullptr, nullptr, fast,
                                   a.opt.kernel_mode, &sc))
     return rc;
   Blob blob;
@@ -910,7 +915,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   depth = std::min(depth, std::max(1u, a.n_steps));
   const uint32_t R = (1u << depth) - 1u;
   Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, nullptr, fast,
+  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, a.stream_records != nullptr, nullptr, fast,
                                   a.opt.kernel_mode, &sc))
     return rc;
   Blob blob;
@@ -1145,7 +1150,7 @@ int32_t cf_trace_sim_opt(const cf_options* opt_in, const cf_graph* g, const cf_p
   const bool fast = opt.kernel_mode == CF_KERNEL_FAST32;
   if (fast && !fast_path_ok(g, opt.kernel_mode)) return CF_ERR_ARG;
   Schedule sc;
-  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, &plan, fast, opt.kernel_mode, &sc)) return rc;
+  if (int32_t rc = build_schedule(g, pl, 1, nullptr, 1, false, &plan, fast, opt.kernel_mode, &sc)) return rc;
   // the single simulation reads rate slot `plan` (pr = plan*1 + 0): upload a full-length rate array
   Blob blob;
   blob.reserve(kAlign);

@@ -42,6 +42,7 @@ struct SimDesc {
 
 struct WarpDesc {
   uint32_t sim_begin, n_lanes, topo;
+  uint32_t variant;     // stream variant of this warp's simulations (materialised stream: a block may mix variants)
   uint32_t heap_off;    // byte offset of this warp's heap region in the CTA heap arena (64-bit kernel)
   uint32_t heap_off32;  // same for the 32-bit kernel (4-ary heap of uint32 quads)
   uint32_t heap_rows32; // 512-byte rows of that region
@@ -308,6 +309,10 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
     cnt_s[tid] = 0;
     L_s[tid] = prm.L_us[tid];
   }
+  // a10: with a materialised stream every warp reads the records of its own (variant, trial) straight
+  // from HBM, one request per lane (two 128-bit loads); no shared tile
+  const bool streamed = prm.stream != nullptr;
+  uint32_t my_cnt = 0;  // streamed: lane t counts the requests of type t
 
   // ---- per-lane simulation state -------------------------------------------------------------
   const bool warp_active = warp < (int)cta.n_warps;
@@ -375,14 +380,15 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   };
 
   __syncthreads();
-  produce(0);
+  if (!streamed) produce(0);
   __syncthreads();
+  const uint4* wsrc = streamed && warp_active ? prm.stream + (size_t)(wd.variant * prm.K + trial) * prm.N * 2 : nullptr;
 
   // a warp none of whose lanes has work (closed brackets; fixup pass: no flagged lane) only helps
   // producing the tiles
   const bool consume = __any_sync(0xffffffffu, wanted);
   for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
-    if (tile_idx + 1 < n_tiles) produce(tile_idx + 1);
+    if (!streamed && tile_idx + 1 < n_tiles) produce(tile_idx + 1);
     if (consume) {
       const uint32_t buf = tile_idx & 1u;
       const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
@@ -391,16 +397,28 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
       for (int ch = 0; ch < kChunks; ++ch) {
         const uint32_t nc0 = n0 + ch * 32;
         if (nc0 >= prm.N) break;
+        const int n_here = (int)min(32u, prm.N - nc0);
         // ---- a4: component-level -> stage-level records for this warp's topology -------------
         {
           const uint4* src = tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
-          const uint4 w0 = src[0], w1 = src[1];
+          uint4 w0 = make_uint4(0u, 0u, 0u, 0u), w1 = w0;
+          if (!streamed) {
+            w0 = src[0]; w1 = src[1];
+          } else if (lane < n_here) {
+            w0 = __ldg(wsrc + (size_t)(nc0 + lane) * 2);
+            w1 = __ldg(wsrc + (size_t)(nc0 + lane) * 2 + 1);
+          }
           int32_t svc[8];
           svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x;
           svc[3] = (int32_t)w1.y; svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w;
           svc[6] = 0; svc[7] = 0;
           if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
           const uint32_t t = w0.y >> 24;
+          if (streamed)
+            for (uint32_t tt = 0; tt < prm.T; ++tt) {
+              const uint32_t b = __ballot_sync(0xffffffffu, lane < n_here && t == tt);
+              if ((uint32_t)lane == tt) my_cnt += __popc(b);
+            }
           const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;
           const uint32_t tm = prm.type_mask[t];
           int32_t S[VMAX];
@@ -425,7 +443,6 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
         }
         __syncwarp();
         // ---- the per-request loop: every lane runs its own simulation over the same 32 requests
-        const int n_here = (int)min(32u, prm.N - nc0);
         uint64_t hp = 0;  // per-type hit counters of this chunk, one byte each
 #pragma unroll 1
         for (int r = 0; r < n_here; ++r) {
@@ -477,13 +494,16 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
 #pragma unroll
         for (int t = 0; t < 8; ++t) hits[t] += (uint32_t)(hp >> (8 * t)) & 0xffu;
         __syncwarp();
-        cu_base += totals[buf * kChunks + ch];
+        if (!streamed) cu_base += totals[buf * kChunks + ch];
       }
     }
     __syncthreads();
   }
 
   // ---- outputs ---------------------------------------------------------------------------------
+  uint32_t cnt_out[8];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) cnt_out[t] = streamed ? __shfl_sync(0xffffffffu, my_cnt, t) : cnt_s[t];
   if (write_out) {
     // DESIGN.md R17: the arrival horizon CU_N * period + 2^15 must stay below 2^62
     bool bad = rate_bad;
@@ -497,7 +517,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
     const size_t slot = (size_t)pr * prm.K + trial;
     uint32_t* oc = prm.out_counts + slot * prm.T * 2;
     for (uint32_t t = 0; t < prm.T; ++t) {
-      oc[2 * t + 0] = zero ? 0u : cnt_s[t];
+      oc[2 * t + 0] = zero ? 0u : cnt_out[t];
       oc[2 * t + 1] = zero ? 0u : hits[t];
     }
     if (prm.out_dep_sum) prm.out_dep_sum[slot] = zero ? 0ull : dep_sum;

@@ -35,6 +35,18 @@ cudaError_t launch_trace(const KParams& kp, const LaunchCfg& lc, cudaStream_t st
   return cudaGetLastError();
 }
 
+// materialised stream: per-warp chunk rings, blocks of 4 warps
+#if CF_CMAX <= 6
+template <bool HAS_DELAY, bool T8>
+cudaError_t launch_pw(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) {
+  auto kern = cf_sim32_kernel<CF_VMAX, CF_CMAX, HAS_DELAY, T8, 4, false, true>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+  if (e != cudaSuccess) return e;
+  kern<<<lc.blocks, 4 * 32, lc.smem_bytes, st>>>(kp);
+  return cudaGetLastError();
+}
+#endif
+
 template <int W>
 cudaError_t launch_w(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) {
   const bool d = kp.edge_delay != 0, t8 = kp.T > 4;
@@ -46,6 +58,16 @@ cudaError_t launch_w(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) {
 
 cudaError_t CF_K32_LAUNCH(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) {
   if (kp.tr_arrival || kp.tr_departure || kp.tr_type) return lc.warps_per_cta == 4 ? launch_trace(kp, lc, st) : cudaErrorInvalidConfiguration;
+  if (kp.stream) {
+#if CF_CMAX <= 6
+    if (lc.warps_per_cta != 4) return cudaErrorInvalidConfiguration;
+    const bool d = kp.edge_delay != 0, t8 = kp.T > 4;
+    if (d) return t8 ? launch_pw<true, true>(kp, lc, st) : launch_pw<true, false>(kp, lc, st);
+    return t8 ? launch_pw<false, true>(kp, lc, st) : launch_pw<false, false>(kp, lc, st);
+#else
+    return cudaErrorInvalidConfiguration;
+#endif
+  }
   return lc.warps_per_cta == 4 ? launch_w<4>(kp, lc, st) : launch_w<8>(kp, lc, st);
 }
 

@@ -58,14 +58,16 @@ struct StageRec32 {
 // address of the lane's top heap quad (18 bits; the record's own address when nq == 0, so that the
 // request loop can load "the top quad" unconditionally), nq = number of quads
 constexpr uint32_t kHbMask = 0x3ffffu;
-template <int VMAX, int CMAX, int WARPS>
+// PW (materialised stream, a10): no block-shared tile; every warp owns a ring of two 32-record
+// chunks (32-byte records) filled by cp.async.bulk behind two mbarriers, and its own type counts
+template <int VMAX, int CMAX, int WARPS, bool PW = false>
 struct SmemLayout32 {
   static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
   static constexpr uint32_t kStageRecBytes = StageRec32<VMAX>::kWords * 16;
-  static constexpr uint32_t tiles = 0;
-  static constexpr uint32_t totals = tiles + 2 * kTile * kCompRecBytes;
-  static constexpr uint32_t cnt = totals + 2 * kChunks * 8;
-  static constexpr uint32_t l32 = cnt + 8 * 4;
+  static constexpr uint32_t tiles = 0;   // PW: [warp][2][32] x 32 B
+  static constexpr uint32_t totals = tiles + (PW ? WARPS * 2 * 32 * 32 : 2 * kTile * kCompRecBytes);  // PW: [warp][2] mbarriers
+  static constexpr uint32_t cnt = totals + (PW ? WARPS * 2 * 8 : 2 * kChunks * 8);                      // PW: [warp][8]
+  static constexpr uint32_t l32 = cnt + (PW ? WARPS * 8 * 4 : 8 * 4);
   static constexpr uint32_t inc = l32 + 8 * 4;  // 8 x {lo, hi}
   static constexpr uint32_t wbuf = inc + 8 * 8;
   static constexpr uint32_t state = wbuf + WARPS * 32 * kStageRecBytes;  // [warp][stage][lane] x 16 B
@@ -133,6 +135,29 @@ __device__ __forceinline__ uint32_t heap4_replace_min(uint32_t hb, uint32_t nq51
   return new_root;
 }
 
+// ---- per-warp bulk copies of stream chunks (sm_90+ bulk async copy: one instruction per chunk) -----
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "CF_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra CF_DONE_%=;\n"
+      "bra CF_WAIT_%=;\n"
+      "CF_DONE_%=:\n"
+      "}" ::"r"(bar), "r"(parity) : "memory");
+}
+
 // packed key p of slot k -> rebased by sh4 = shift << 2 (clamped at 0); +inf stays +inf
 __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint32_t k) {
   const uint32_t v = (max(p, sh4) - sh4) | k;
@@ -143,10 +168,11 @@ __device__ __forceinline__ uint32_t rebase_packed(uint32_t p, uint32_t sh4, uint
 // (16 warps per SM either way: 124-128 registers per thread)
 // TRACE (cf_trace_sim through this kernel): the call holds one simulation, lane 0 of warp 0; it
 // writes every request's system arrival and final departure, the warp's lanes the request types
-template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int WARPS, bool TRACE = false>
+template <int VMAX, int CMAX, bool HAS_DELAY, bool T8, int WARPS, bool TRACE = false, bool PW = false>
 __global__ void __launch_bounds__(WARPS * 32, 16 / WARPS)
 cf_sim32_kernel(const __grid_constant__ KParams prm) {
-  using SL = SmemLayout32<VMAX, CMAX, WARPS>;
+  static_assert(!PW || CMAX <= 6, "the materialised stream holds 32-byte records (C <= 6)");
+  using SL = SmemLayout32<VMAX, CMAX, WARPS, PW>;
   constexpr int kW = StageRec32<VMAX>::kWords;
   extern __shared__ __align__(16) uint8_t smem[];
   const uint32_t smem_sa = (uint32_t)__cvta_generic_to_shared(smem);
@@ -157,15 +183,15 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
 
   uint4* tiles = reinterpret_cast<uint4*>(smem + SL::tiles);
   uint64_t* totals = reinterpret_cast<uint64_t*>(smem + SL::totals);
-  uint32_t* cnt_s = reinterpret_cast<uint32_t*>(smem + SL::cnt);
+  uint32_t* cnt_s = reinterpret_cast<uint32_t*>(smem + SL::cnt) + (PW ? warp * 8 : 0);
   uint32_t* l32_s = reinterpret_cast<uint32_t*>(smem + SL::l32);
   uint2* inc_s = reinterpret_cast<uint2*>(smem + SL::inc);
   uint4* wbuf = reinterpret_cast<uint4*>(smem + SL::wbuf) + warp * 32 * kW;
   // shared addresses of this lane's state records (stage s at + s*512) and of its heap column
   const uint32_t st_sa = smem_sa + SL::state + (uint32_t)warp * VMAX * 512u + (uint32_t)lane * 16u;
 
+  if (PW ? lane < 8 : tid < 8) cnt_s[PW ? lane : tid] = 0;
   if (tid < 8) {
-    cnt_s[tid] = 0;
     const int64_t L = prm.L_us[tid];
     // L >= 2^32-1 is held as 2^32-1: exact while the sojourn fits 32 bits; a longer sojourn that
     // misses this bound sends the lane to the 64-bit kernel (see the a8 test below)
@@ -243,8 +269,32 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   // a warp whose lanes all skip (closed brackets) only helps producing the tiles
   const bool consume = __any_sync(kFull, wanted);
   __syncthreads();
-  produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
-  __syncthreads();
+  if (!PW) produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, 0, tiles, totals, cnt_s, tid, warp, lane);
+  if (!PW) __syncthreads();
+  // PW: this warp's records [n] of (its variant, the block's trial), its ring and the two barriers
+  const uint4* wsrc = nullptr;
+  const uint32_t ring_sa = smem_sa + SL::tiles + (uint32_t)warp * 2048u;
+  const uint32_t bar_sa = smem_sa + SL::totals + (uint32_t)warp * 16u;
+  const uint32_t n_chunks = (prm.N + 31u) / 32u;
+  uint32_t my_cnt = 0;  // PW: lane t counts the requests of type t
+  auto fetch = [&](uint32_t g) {  // lane 0: chunk g -> ring slot g & 1
+    const uint32_t bytes = min(32u, prm.N - g * 32u) * 32u;
+    mbar_expect_tx(bar_sa + (g & 1u) * 8u, bytes);
+    bulk_load(ring_sa + (g & 1u) * 1024u, wsrc + (size_t)g * 64u, bytes, bar_sa + (g & 1u) * 8u);
+  };
+  if (PW) {
+    if (!consume) return;  // nothing below synchronises the block
+    wsrc = prm.stream + (size_t)(wd.variant * prm.K + trial) * prm.N * 2;
+    if (lane == 0) {
+      mbar_init(bar_sa, 1u);
+      mbar_init(bar_sa + 8u, 1u);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      fetch(0u);
+      if (n_chunks > 1u) fetch(1u);
+    }
+    __syncwarp();
+  }
 
   // the origin moves forward by delta: every stage base goes to max(earliest free time, new origin)
   // and the stage's heap is re-keyed (keys below the new base are clamped to it: DESIGN.md 5.2)
@@ -272,7 +322,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
   uint32_t flush_idx = 0;  // requests [flush_idx, current) are accumulated in dep relative to origin
 
   for (uint32_t tile_idx = 0; tile_idx < n_tiles; ++tile_idx) {
-    if (tile_idx + 1 < n_tiles)
+    if (!PW && tile_idx + 1 < n_tiles)
       produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, tile_idx + 1, tiles, totals, cnt_s, tid, warp, lane);
     if (consume) {
       const uint32_t buf = tile_idx & 1u;
@@ -308,14 +358,26 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
         uint64_t chunk_work = 0;
         // ---- a4: component-level record -> list of visited stages for this warp's topology ----
         {
-          const uint4* src = tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
-          const uint4 w0 = src[0], w1 = src[1];
+          const uint32_t g = tile_idx * kChunks + (uint32_t)ch;  // chunk index
+          if (PW) mbar_wait(bar_sa + (g & 1u) * 8u, (g >> 1) & 1u);  // the chunk's bytes have landed
+          const uint4* src = PW ? tiles + warp * 128 + (g & 1u) * 64 + lane * 2
+                                : tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
+          uint4 w0 = src[0], w1 = src[1];
+          if (PW && lane >= n_here) w0 = w1 = make_uint4(0u, 0u, 0u, 0u);  // beyond N: the slot holds stale bytes
           int32_t svc[8];
           svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x;
           svc[3] = (int32_t)w1.y; svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w;
           svc[6] = 0; svc[7] = 0;
           if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
           const uint32_t t = w0.y >> 24;
+          if (PW) {
+            for (uint32_t tt = 0; tt < prm.T; ++tt) {
+              const uint32_t b = __ballot_sync(kFull, lane < n_here && t == tt);
+              if ((uint32_t)lane == tt) my_cnt += __popc(b);
+            }
+            __syncwarp();  // every lane has read its record: the slot may be refilled
+            if (lane == 0 && g + 2u < n_chunks) fetch(g + 2u);
+          }
           if (TRACE && warp == 0 && lane < n_here && prm.tr_type) prm.tr_type[nc0 + lane] = (uint8_t)t;
           const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;  // absolute
           const uint64_t d64 = cu - tile_base;
@@ -487,7 +549,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           if (r < n_here) request(tag, a0, a1, a2, a3, b0, b1, b2, b3, r);
         }
         __syncwarp();
-        cu_base += totals[buf * kChunks + ch];
+        if (!PW) cu_base += totals[buf * kChunks + ch];
         if ((ch & 3) == 3) flush_hits();  // a byte field holds at most 128 hits
       }
       // ---- tile epilogue: absolute outputs, window checks
@@ -498,7 +560,11 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
       tile_base = last_cu;
       flush_hits();
     }
-    __syncthreads();
+    if (!PW) __syncthreads();
+  }
+  if (PW) {  // the warp's type counts -> its row of cnt_s
+    if (lane < 8) cnt_s[lane] = my_cnt;
+    __syncwarp();
   }
 
   // ---- outputs ---------------------------------------------------------------------------------

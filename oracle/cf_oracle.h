@@ -13,7 +13,9 @@
  *
  * Parity status: every function below is pinned by tests/test_oracle_*.py (Random123 known-answer
  * vectors, queueing closed forms, exact D/D/c cases, brute-force event simulators on tiny inputs,
- * invariants). Nothing here is "parity unpinned"; the modelling choices R2/R6/R7 are pinned to
+ * invariants; the phase-1/2/selection functions by hand-worked examples, closed forms, brute force
+ * and the identity "Monte Carlo = simulation with unlimited replicas": tests/test_oracle_phases.py).
+ * Nothing here is "parity unpinned"; the modelling choices R2/R6/R7 are pinned to
  * independent brute-force simulators of the same discipline.
  *
  * All pointers are HOST pointers. All functions are deterministic and thread-safe.
@@ -111,6 +113,30 @@ int32_t orc_trace_sim(const orc_graph* g, const orc_plans* pl, uint32_t plan, ui
  * visits i, else 0. out has n_variants*K*N records. */
 int32_t orc_materialize_stream(const orc_graph* g, uint64_t seed, uint32_t variant_lo,
                                uint32_t n_variants, void* out);
+
+/* ---- the cheap phases around the simulation (cf_oracle_phases.cpp; SURVEY.md 8(f) NEXT-1..3) ---- */
+
+/* Mean of the distribution a quantile table induces, Q16 (R21). */
+uint64_t orc_qtab_mean_q16(const orc_qtab* tab);
+
+/* Phase 1, flow-based throughput estimation (Algorithm 2 l.1-5).
+ * out_rate_mrps[P] = min(floor(R_d * alpha_num / alpha_den), 1e9); optional out_bound_mrps[P] = R_d
+ * (capped at 1e9), out_bottleneck[P] (stage index, 0xff: no demand anywhere), out_redundant[P]. */
+int32_t orc_flow_bound(const orc_graph* g, const orc_plans* pl, uint32_t alpha_num,
+                       uint32_t alpha_den, uint32_t* out_rate_mrps, uint32_t* out_bound_mrps,
+                       uint8_t* out_bottleneck, uint8_t* out_redundant);
+
+/* Phase 2, latency estimation with Monte Carlo (Algorithm 2 l.6-11).
+ * rate_mrps[P] = the incoming rate alpha R_d of each plan. out_counts[P][K][T][2] (may be NULL),
+ * out_goodput_mrps[P][T]. */
+int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* rate_mrps,
+                       const orc_slo* slo, uint64_t seed, uint32_t variant, uint32_t* out_counts,
+                       uint32_t* out_goodput_mrps);
+
+/* Pareto pruning of goodput vectors and the default selection policy (Algorithm 2 l.12, 16-18,
+ * PAPER.md:251-259, 286-288). goodput[P][T], alive[P] or NULL; out_pruned[P]. */
+int32_t orc_pareto_select(const uint32_t* goodput, uint32_t P, uint32_t T, const uint8_t* alive,
+                          uint8_t* out_pruned, uint32_t* out_best, uint32_t* out_n_survivors);
 
 #ifdef __cplusplus
 }

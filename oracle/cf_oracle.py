@@ -16,6 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libcf_oracle.so")
 _SRC = os.path.join(_HERE, "cf_oracle.cpp")
+_SRC2 = os.path.join(_HERE, "cf_oracle_phases.cpp")
 _HDR = os.path.join(_HERE, "cf_oracle.h")
 
 ORC_OK, ORC_ERR_ARG, ORC_ERR_RANGE, ORC_ERR_PLAN, ORC_ERR_TABLE = 0, -1, -2, -3, -4
@@ -23,9 +24,9 @@ ORC_OK, ORC_ERR_ARG, ORC_ERR_RANGE, ORC_ERR_PLAN, ORC_ERR_TABLE = 0, -1, -2, -3,
 
 def build(force: bool = False) -> str:
     """Compile the oracle with g++ -O2 (plain, untuned)."""
-    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC2), os.path.getmtime(_HDR))
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
-        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-Wall", "-o", _SO, _SRC]
+        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-Wall", "-o", _SO, _SRC, _SRC2]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _SO
 
@@ -72,8 +73,9 @@ def lib():
         _lib.orc_qtab_sample.argtypes = [C.POINTER(_QTab), C.c_uint32]
         _lib.orc_philox4x32_10.restype = None
         for name in ("orc_validate", "orc_eval_plans", "orc_goodput_bisect", "orc_trace_sim",
-                     "orc_materialize_stream"):
+                     "orc_materialize_stream", "orc_flow_bound", "orc_mc_latency", "orc_pareto_select"):
             getattr(_lib, name).restype = C.c_int32
+        _lib.orc_qtab_mean_q16.restype = C.c_uint64
     return _lib
 
 
@@ -185,3 +187,49 @@ def materialize_stream(graph, seed: int, variant_lo: int, n_variants: int):
                                       C.c_uint32(n_variants), out.ctypes.data_as(C.c_void_p))
     assert rc == 0, rc
     return out
+
+
+# ---- the cheap phases around the simulation (cf_oracle_phases.cpp) ----------------------------------
+def qtab_mean_q16(tab) -> int:
+    t = _QTab(tab.levels, tab.log2_cells, _ptr(tab.q, C.c_int32))
+    return int(lib().orc_qtab_mean_q16(C.byref(t)))
+
+
+def flow_bound(graph, plans, alpha_num: int = 1, alpha_den: int = 1):
+    """Returns dict(rate_mrps [P] u32, bound_mrps [P] u32, bottleneck [P] u8, redundant [P] u8, rc)."""
+    m = _Marshalled(graph, plans)
+    P = plans.n_plans
+    rate = np.zeros(P, dtype=np.uint32)
+    bound = np.zeros(P, dtype=np.uint32)
+    bott = np.zeros(P, dtype=np.uint8)
+    red = np.zeros(P, dtype=np.uint8)
+    rc = lib().orc_flow_bound(C.byref(m.g), C.byref(m.pl), C.c_uint32(alpha_num), C.c_uint32(alpha_den),
+                              _ptr(rate, C.c_uint32), _ptr(bound, C.c_uint32), _ptr(bott, C.c_uint8),
+                              _ptr(red, C.c_uint8))
+    return dict(rate_mrps=rate, bound_mrps=bound, bottleneck=bott, redundant=red, rc=int(rc))
+
+
+def mc_latency(graph, plans, rate_mrps, slo, seed: int, variant: int = 0):
+    """Returns dict(counts [P,K,T,2] u32, goodput_mrps [P,T] u32, rc)."""
+    m = _Marshalled(graph, plans, slo)
+    P, K, T = plans.n_plans, graph.n_trials, graph.n_types
+    rates = np.ascontiguousarray(rate_mrps, dtype=np.uint32).reshape(-1)
+    assert rates.size == P
+    counts = np.zeros((P, K, T, 2), dtype=np.uint32)
+    good = np.zeros((P, T), dtype=np.uint32)
+    rc = lib().orc_mc_latency(C.byref(m.g), C.byref(m.pl), _ptr(rates, C.c_uint32), C.byref(m.slo),
+                              C.c_uint64(seed), C.c_uint32(variant), _ptr(counts, C.c_uint32),
+                              _ptr(good, C.c_uint32))
+    return dict(counts=counts, goodput_mrps=good, rc=int(rc))
+
+
+def pareto_select(goodput, alive=None):
+    """goodput [P,T] u32; alive [P] u8 or None. Returns dict(pruned [P] u8, best, n_survivors, rc)."""
+    gp = np.ascontiguousarray(goodput, dtype=np.uint32)
+    P, T = gp.shape
+    al = None if alive is None else np.ascontiguousarray(alive, dtype=np.uint8)
+    pruned = np.zeros(P, dtype=np.uint8)
+    best, ns = C.c_uint32(0), C.c_uint32(0)
+    rc = lib().orc_pareto_select(_ptr(gp, C.c_uint32), C.c_uint32(P), C.c_uint32(T), _ptr(al, C.c_uint8),
+                                 _ptr(pruned, C.c_uint8), C.byref(best), C.byref(ns))
+    return dict(pruned=pruned, best=int(best.value), n_survivors=int(ns.value), rc=int(rc))

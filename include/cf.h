@@ -169,6 +169,56 @@ int64_t cf_workspace_wide_count(const void* workspace, void* stream);
  * call on `workspace` (steps whose bracket had already closed are no-ops and do not count). */
 int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_probes, void* stream);
 
+/* ---- the cheap phases around the simulation (Algorithm 2 phases 1-2 and selection) --------------
+ * They run on the device so that alpha R_d, goodput vectors and survivor flags pass from phase to
+ * phase without leaving HBM. Integer definitions: DESIGN.md readings R20-R23. */
+
+/* Scratch of cf_flow_bound / cf_mc_latency for (graph, plans); of cf_pareto_select. */
+size_t cf_aux_workspace_bytes(const cf_graph* g, const cf_plans* pl);
+size_t cf_pareto_workspace_bytes(void);
+
+/* Phase 1, flow-based throughput estimation (Algorithm 2 l.1-5; sec. 4.3
+ * PAPER.md:274-276). A node's demand per arriving request is sum_t pi_t * (mean service of type t on
+ * the node's components), from the exact means of the quantile tables; "the node whose aggregate
+ * demand first reaches its capacity is the bottleneck, and the aggregate request rate R_d at which
+ * this occurs is plan d's maximum throughput"; "plans that configure a node with more capacity than
+ * the node's aggregate demand are redundant".
+ *   out_rate_mrps  dev [P]  min(floor(R_d * alpha_num / alpha_den), 1e9): the rate alpha R_d the later
+ *                           phases evaluate; usable as cf_goodput_bisect's rate_hi_mrps
+ *   out_bound_mrps dev [P]  R_d in milli-requests/s, capped at 1e9, or NULL
+ *   out_bottleneck dev [P]  index of the bottleneck stage (lowest on ties; 0xff: no stage has demand), or NULL
+ *   out_redundant  dev [P]  1 iff some stage with >= 2 replicas still sustains R_d with one fewer, or
+ *                           has no demand at all (R22), or NULL
+ * alpha_den >= 1. */
+int32_t cf_flow_bound(const cf_graph* g, const cf_plans* pl, uint32_t alpha_num, uint32_t alpha_den,
+                      uint32_t* out_rate_mrps, uint32_t* out_bound_mrps, uint8_t* out_bottleneck,
+                      uint8_t* out_redundant, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Phase 2, latency estimation with Monte Carlo (Algorithm 2 l.6-11; sec. 4.3
+ * PAPER.md:278): the K x N sampled requests of the simulation (same Philox counters, R4) are routed
+ * through every plan; a request's latency is the sum of its sampled processing latencies along its
+ * path plus edge_delay_us per hop; "queuing not modeled". F_{t,d}(L_t) = hits_t / cnt_t.
+ *   rate_mrps        dev [P]  incoming rate alpha R_d of each plan (e.g. cf_flow_bound's out_rate_mrps)
+ *   out_counts       dev [P][K][T][2] = {cnt_t, hits_t}, or NULL
+ *   out_goodput_mrps dev [P][T] floor(rate * hits_t / (N K)), hits pooled over trials
+ *                    (G_{t,d} = alpha R_d pi_t F_{t,d}(L_t), Algorithm 2 l.11, with the sampled mix) */
+int32_t cf_mc_latency(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps, const cf_slo* slo,
+                      uint64_t seed, uint32_t variant, uint32_t* out_counts, uint32_t* out_goodput_mrps,
+                      void* workspace, size_t workspace_bytes, void* stream);
+
+/* Pareto pruning of per-type goodput vectors and the default selection policy (Algorithm 2 l.12,
+ * 16-18; sec. 4.3). Plan p is pruned iff it is not live or some
+ * live plan q has G_q[t] >= G_p[t] for all t and G_q[t] > G_p[t] for one t (equal vectors do not
+ * prune each other, R23). The policy picks the live plan with the largest sum_t G[t] (lowest index
+ * on ties); it is never a pruned plan.
+ *   goodput_mrps dev [P][T] (e.g. cf_mc_latency's or cf_goodput_bisect's output), T <= 8
+ *   alive        dev [P] 0/1, or NULL (all live): chains the phases' survivor sets
+ *   out_pruned   dev [P]; out_best dev [1] (0xffffffff if no plan is live) or NULL;
+ *   out_n_survivors dev [1] or NULL */
+int32_t cf_pareto_select(const uint32_t* goodput_mrps, uint32_t n_plans, uint32_t n_types,
+                         const uint8_t* alive, uint8_t* out_pruned, uint32_t* out_best,
+                         uint32_t* out_n_survivors, void* workspace, size_t workspace_bytes, void* stream);
+
 const char* cf_strerror(int32_t status);
 
 #ifdef __cplusplus

@@ -23,7 +23,8 @@ CF_OK, CF_ERR_ARG, CF_ERR_RANGE, CF_ERR_PLAN, CF_ERR_TABLE, CF_ERR_CUDA, CF_ERR_
 EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_stream_bytes",
            "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_strerror",
-           "cf_workspace_wide_count", "cf_bisect_probes"]
+           "cf_workspace_wide_count", "cf_bisect_probes", "cf_aux_workspace_bytes",
+           "cf_pareto_workspace_bytes", "cf_flow_bound", "cf_mc_latency", "cf_pareto_select"]
 DEBUG_EXPORTS = ["cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
                  "cf_goodput_bisect_stream_opt", "cf_trace_sim_opt", "cf_last_launch_count",
                  "cf_bench_int32_peak"]
@@ -76,6 +77,10 @@ _lib.cf_strerror.restype = C.c_char_p
 _lib.cf_last_launch_count.restype = C.c_uint32
 _lib.cf_workspace_wide_count.restype = C.c_int64
 _lib.cf_bisect_probes.restype = C.c_int32
+_lib.cf_aux_workspace_bytes.restype = C.c_size_t
+_lib.cf_pareto_workspace_bytes.restype = C.c_size_t
+for _n in ("cf_flow_bound", "cf_mc_latency", "cf_pareto_select"):
+    getattr(_lib, _n).restype = C.c_int32
 for _n in ("cf_eval_plans", "cf_goodput_bisect", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak",
            "cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
@@ -326,6 +331,74 @@ def cf_trace_sim(graph, plans, plan: int, rate_mrps: int, trial: int, seed: int,
     status = cf_workspace_status(ws, stream)
     wide = cf_workspace_wide_count(ws, stream) if rc == CF_OK else -1
     return dict(arrival=arr, departure=dep, type=typ, rc=int(rc), status=status, wide=wide)
+
+
+def _aux_workspace(m, stream_dev="cuda") -> torch.Tensor:
+    n = int(_lib.cf_aux_workspace_bytes(C.byref(m.g), C.byref(m.pl) if m.pl is not None else None))
+    return torch.empty(n, dtype=torch.uint8, device=stream_dev)
+
+
+def cf_flow_bound(graph, plans, alpha_num: int = 1, alpha_den: int = 1, *, stream=None, check=True):
+    """Phase 1 on the device. Returns dict of CUDA tensors: rate_mrps int32 [P] (alpha R_d),
+    bound_mrps int32 [P] (R_d), bottleneck uint8 [P], redundant uint8 [P]."""
+    _require_cuda()
+    m = Marshalled(graph, plans)
+    P = plans.n_plans
+    rate = torch.empty(P, dtype=torch.int32, device="cuda")
+    bound = torch.empty(P, dtype=torch.int32, device="cuda")
+    bott = torch.empty(P, dtype=torch.uint8, device="cuda")
+    red = torch.empty(P, dtype=torch.uint8, device="cuda")
+    ws = _aux_workspace(m)
+    rc = _lib.cf_flow_bound(C.byref(m.g), C.byref(m.pl), C.c_uint32(alpha_num), C.c_uint32(alpha_den), _dp(rate),
+                            _dp(bound), _dp(bott), _dp(red), _dp(ws), C.c_size_t(ws.numel()), _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_flow_bound")
+    return dict(rate_mrps=rate, bound_mrps=bound, bottleneck=bott, redundant=red, workspace=ws, rc=int(rc))
+
+
+def cf_mc_latency(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, want_counts=True, stream=None,
+                  check=True):
+    """Phase 2 on the device. rate_mrps: [P] CUDA int32 tensor or array-like. Returns dict of CUDA
+    tensors: counts int32 [P,K,T,2] (or None), goodput_mrps int32 [P,T]."""
+    _require_cuda()
+    m = Marshalled(graph, plans, slo)
+    P, K, T = plans.n_plans, graph.n_trials, graph.n_types
+    rates = _as_dev_u32(rate_mrps, torch.device("cuda")).reshape(-1)
+    assert rates.numel() == P
+    counts = torch.empty((P, K, T, 2), dtype=torch.int32, device="cuda") if want_counts else None
+    good = torch.empty((P, T), dtype=torch.int32, device="cuda")
+    ws = _aux_workspace(m)
+    rc = _lib.cf_mc_latency(C.byref(m.g), C.byref(m.pl), _dp(rates), C.byref(m.slo), C.c_uint64(seed),
+                            C.c_uint32(variant), _dp(counts), _dp(good), _dp(ws), C.c_size_t(ws.numel()),
+                            _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_mc_latency")
+    return dict(counts=counts, goodput_mrps=good, workspace=ws, rc=int(rc))
+
+
+def cf_pareto_select(goodput_mrps, alive=None, *, stream=None, check=True):
+    """Pruning + policy on the device. goodput_mrps: [P,T] CUDA int32 tensor or array-like; alive: [P]
+    CUDA uint8 tensor, array-like or None. Returns dict of CUDA tensors: pruned uint8 [P], best int32
+    [1] (uint32 bit pattern), n_survivors int32 [1]."""
+    _require_cuda()
+    dev = torch.device("cuda")
+    gp = goodput_mrps if isinstance(goodput_mrps, torch.Tensor) else \
+        torch.from_numpy(np.ascontiguousarray(goodput_mrps, dtype=np.uint32).view(np.int32)).to(dev)
+    gp = gp.contiguous()
+    P, T = gp.shape
+    al = None
+    if alive is not None:
+        al = alive if isinstance(alive, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(alive, dtype=np.uint8)).to(dev)
+        al = al.contiguous()
+    pruned = torch.empty(P, dtype=torch.uint8, device=dev)
+    best = torch.empty(1, dtype=torch.int32, device=dev)
+    ns = torch.empty(1, dtype=torch.int32, device=dev)
+    ws = torch.empty(int(_lib.cf_pareto_workspace_bytes()), dtype=torch.uint8, device=dev)
+    rc = _lib.cf_pareto_select(_dp(gp), C.c_uint32(P), C.c_uint32(T), _dp(al), _dp(pruned), _dp(best), _dp(ns),
+                               _dp(ws), C.c_size_t(ws.numel()), _stream_ptr(stream))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_pareto_select")
+    return dict(pruned=pruned, best=best, n_survivors=ns, workspace=ws, rc=int(rc))
 
 
 def cf_bench_int32_peak(mix: int, iters: int = 2000, stream=None):

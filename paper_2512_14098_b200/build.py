@@ -18,7 +18,6 @@ HEADERS = ["cf_device.cuh", "cf_rel32.cuh", "cf_scan.cuh", "cf_launch.h", "cf_au
            os.path.join("..", "..", "include", "cf.h"), os.path.join("..", "..", "include", "cf_debug.h")]
 # (object name, source, extra defines)
 UNITS = [("cf_api", "cf_api.cu", []),
-         ("cf_aux", "cf_aux.cu", []),
          ("cf_k64", "cf_k64.cu", []),
          ("cf_scan", "cf_scan.cu", [])] + \
         [(f"cf_k32_v{v}c{c}", "cf_k32.cu", [f"-DCF_VMAX={v}", f"-DCF_CMAX={c}"])

@@ -16,6 +16,7 @@
 #include "cf_launch.h"
 #include "cf_rel32.cuh"  // layout constants only: the kernels are instantiated in cf_k32.cu
 #include "cf_scan.cuh"   // kScanWarps
+#include "cf_aux.cuh"    // phase-1 / phase-2 / selection kernels
 
 using namespace cfk;
 
@@ -1267,6 +1268,156 @@ const char* cf_strerror(int32_t status) {
     case CF_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     default: return "unknown status";
   }
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// phases 1, 2 and selection (cf_aux.cuh): shared host setup
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct AuxSetup {
+  AuxParams ap;
+  Blob blob;
+  size_t mean_off = 0, demand_off = 0, hist_off = 0, need = 0;
+};
+
+// uploads tables, table descriptors and (if pl) the plan arrays; lays out the scratch regions
+int32_t aux_setup(const cf_graph* g, const cf_plans* pl, const cf_slo* slo, uint64_t seed, uint32_t variant,
+                  void* ws, size_t ws_bytes, cudaStream_t st, AuxSetup* out) {
+  AuxSetup& a = *out;
+  AuxParams& ap = a.ap;
+  std::memset(&ap, 0, sizeof(ap));
+  a.blob.reserve(kAlign);  // status block
+  KParams kp;
+  const size_t pool_off = fill_graph_params(g, slo, seed, &a.blob, &kp);
+  ap.C = kp.C; ap.T = kp.T; ap.N = kp.N; ap.K = kp.K;
+  std::memcpy(ap.type_thresh, kp.type_thresh, sizeof(ap.type_thresh));
+  std::memcpy(ap.type_mask, kp.type_mask, sizeof(ap.type_mask));
+  std::memcpy(ap.svc_tab, kp.svc_tab, sizeof(ap.svc_tab));
+  std::memcpy(ap.L_us, kp.L_us, sizeof(ap.L_us));
+  ap.edge_delay = kp.edge_delay; ap.seed_lo = kp.seed_lo; ap.seed_hi = kp.seed_hi; ap.variant = variant;
+  // table descriptors in table-id order (fill_graph_params lays the pool out in that order)
+  std::vector<DevTab> tabs(g->n_tabs);
+  uint32_t off = 0;
+  for (uint32_t j = 0; j < g->n_tabs; ++j) {
+    tabs[j] = DevTab{off, g->tabs[j].levels, g->tabs[j].log2_cells, 0};
+    off += (uint32_t)tab_entries(g->tabs[j]);
+  }
+  for (uint32_t i = 0; i < g->n_comp; ++i)
+    for (uint32_t t = 0; t < g->n_types; ++t)
+      if ((g->type_mask[t] >> i) & 1) ap.tab_id[i * 8 + t] = g->svc_tab[i * g->n_types + t];
+  ap.n_tabs = g->n_tabs;
+  const size_t tabs_off = a.blob.add(tabs.data(), tabs.size() * sizeof(DevTab));
+  size_t ns_off = 0, sm_off = 0, sc_off = 0;
+  if (pl) {
+    ap.P = pl->n_plans; ap.MS = pl->max_stages;
+    ns_off = a.blob.add(pl->n_stages, (size_t)pl->n_plans);
+    sm_off = a.blob.add(pl->stage_mask, (size_t)pl->n_plans * pl->max_stages);
+    sc_off = a.blob.add(pl->stage_c, (size_t)pl->n_plans * pl->max_stages * sizeof(uint16_t));
+  }
+  a.mean_off = align_up(a.blob.bytes.size());
+  a.demand_off = align_up(a.mean_off + (size_t)g->n_tabs * 8);
+  a.hist_off = align_up(a.demand_off + 256 * 8);
+  a.need = align_up(a.hist_off + (size_t)g->n_trials * 72 * 4);
+  if (int32_t rc = check_workspace(ws, ws_bytes, a.need)) return rc;
+  uint8_t* w = static_cast<uint8_t*>(ws);
+  if (int32_t rc = cuda_rc(cudaMemcpyAsync(w, a.blob.bytes.data(), a.blob.bytes.size(), cudaMemcpyHostToDevice, st)))
+    return rc;
+  ap.qpool = reinterpret_cast<const int32_t*>(w + pool_off);
+  ap.tabs = reinterpret_cast<const DevTab*>(w + tabs_off);
+  if (pl) {
+    ap.n_stages = w + ns_off;
+    ap.stage_mask = w + sm_off;
+    ap.stage_c = reinterpret_cast<const uint16_t*>(w + sc_off);
+  }
+  ap.mean_q16 = reinterpret_cast<uint64_t*>(w + a.mean_off);
+  ap.demand_q16 = reinterpret_cast<uint64_t*>(w + a.demand_off);
+  ap.hist = reinterpret_cast<uint32_t*>(w + a.hist_off);
+  return CF_OK;
+}
+
+template <int T>
+void launch_pareto(const uint32_t* G, uint32_t P, const uint8_t* alive, uint8_t* out_pruned, uint32_t* out_best,
+                   uint32_t* out_n, unsigned long long* scratch, cudaStream_t st) {
+  const uint32_t nb = (P + 255) / 256;
+  pareto_dom_kernel<T><<<nb, 256, 0, st>>>(G, P, alive, out_pruned, out_n, scratch);
+  if (out_best) pareto_best_kernel<T><<<nb, 256, 0, st>>>(G, P, alive, scratch, out_best);
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t cf_aux_workspace_bytes(const cf_graph* g, const cf_plans* pl) {
+  if (!g || !g->tabs) return 0;
+  size_t n = 2 * kAlign + align_up(pool_entries(g) * 4) + align_up((size_t)g->n_tabs * sizeof(DevTab));
+  if (pl) n += 3 * kAlign + align_up((size_t)pl->n_plans) + align_up((size_t)pl->n_plans * pl->max_stages * 3);
+  n += align_up((size_t)g->n_tabs * 8) + align_up(256 * 8) + align_up((size_t)g->n_trials * 72 * 4);
+  return n + 4 * kAlign;
+}
+
+int32_t cf_flow_bound(const cf_graph* g, const cf_plans* pl, uint32_t alpha_num, uint32_t alpha_den,
+                      uint32_t* out_rate_mrps, uint32_t* out_bound_mrps, uint8_t* out_bottleneck,
+                      uint8_t* out_redundant, void* workspace, size_t workspace_bytes, void* stream) {
+  g_launch_count = 0;
+  if (int32_t rc = check_graph(g)) return rc;
+  if (int32_t rc = check_plans(g, pl)) return rc;
+  if (alpha_den == 0 || !out_rate_mrps) return CF_ERR_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  AuxSetup a;
+  if (int32_t rc = aux_setup(g, pl, nullptr, 0, 0, workspace, workspace_bytes, st, &a)) return rc;
+  a.ap.alpha_num = alpha_num;
+  a.ap.alpha_den = alpha_den;
+  flow_tabmean_kernel<<<g->n_tabs, 256, 0, st>>>(a.ap);
+  flow_demand_kernel<<<1, 256, 0, st>>>(a.ap);
+  flow_plan_kernel<<<(pl->n_plans + 127) / 128, 128, 0, st>>>(a.ap, out_rate_mrps, out_bound_mrps, out_bottleneck,
+                                                             out_redundant);
+  g_launch_count += 3;
+  return cuda_rc(cudaGetLastError());
+}
+
+int32_t cf_mc_latency(const cf_graph* g, const cf_plans* pl, const uint32_t* rate_mrps, const cf_slo* slo,
+                      uint64_t seed, uint32_t variant, uint32_t* out_counts, uint32_t* out_goodput_mrps,
+                      void* workspace, size_t workspace_bytes, void* stream) {
+  g_launch_count = 0;
+  if (int32_t rc = check_graph(g)) return rc;
+  if (int32_t rc = check_plans(g, pl)) return rc;
+  if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return CF_ERR_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  AuxSetup a;
+  if (int32_t rc = aux_setup(g, pl, slo, seed, variant, workspace, workspace_bytes, st, &a)) return rc;
+  if (int32_t rc = cuda_rc(cudaMemsetAsync(a.ap.hist, 0, (size_t)g->n_trials * 72 * 4, st))) return rc;
+  mc_hist_kernel<<<dim3((g->n_req + 255) / 256, g->n_trials), 256, 0, st>>>(a.ap);
+  mc_plan_kernel<<<(pl->n_plans + 127) / 128, 128, 0, st>>>(a.ap, rate_mrps, out_counts, out_goodput_mrps);
+  g_launch_count += 2;
+  return cuda_rc(cudaGetLastError());
+}
+
+size_t cf_pareto_workspace_bytes(void) { return kAlign; }
+
+int32_t cf_pareto_select(const uint32_t* goodput_mrps, uint32_t n_plans, uint32_t n_types, const uint8_t* alive,
+                         uint8_t* out_pruned, uint32_t* out_best, uint32_t* out_n_survivors, void* workspace,
+                         size_t workspace_bytes, void* stream) {
+  g_launch_count = 0;
+  if (!goodput_mrps || !out_pruned || n_plans < 1 || n_types < 1 || n_types > 8) return CF_ERR_ARG;
+  if (int32_t rc = check_workspace(workspace, workspace_bytes, kAlign)) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  unsigned long long* scratch = static_cast<unsigned long long*>(workspace);
+  pareto_init_kernel<<<1, 1, 0, st>>>(scratch, out_best, out_n_survivors);
+  switch (n_types) {
+    case 1: launch_pareto<1>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    case 2: launch_pareto<2>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    case 3: launch_pareto<3>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    case 4: launch_pareto<4>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    case 5: launch_pareto<5>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    case 6: launch_pareto<6>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    case 7: launch_pareto<7>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+    default: launch_pareto<8>(goodput_mrps, n_plans, alive, out_pruned, out_best, out_n_survivors, scratch, st); break;
+  }
+  g_launch_count += out_best ? 3 : 2;
+  return cuda_rc(cudaGetLastError());
 }
 
 }  // extern "C"

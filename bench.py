@@ -467,6 +467,40 @@ def measure(cfg, args, rank, world, dev, stream, torch, dist, cf, local_rank, wi
     return rec
 
 
+def measure_phases(torch, cf, stream, n_plans=1_000_000):
+    """Sub-record: the cheap phases of Algorithm 2 (flow bound -> Monte-Carlo latency -> Pareto prune
+    of the non-redundant plans) on a 10^6-plan candidate set, chained on the device; milliseconds per
+    call through the C ABI (host descriptors in, device arrays out), best of 3."""
+    w = W.config_phase_sweep(n_plans)
+    g, pl, slo = w.graph, w.plans, w.slo
+
+    def timed(fn):
+        best, out = None, None
+        for _ in range(3):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            out = fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        return out, best
+
+    f, ms_flow = timed(lambda: cf.cf_flow_bound(g, pl, 4, 5))
+    mc, ms_mc = timed(lambda: cf.cf_mc_latency(g, pl, f["rate_mrps"], slo, w.seed, want_counts=False))
+    alive = (1 - f["redundant"]).to(torch.uint8)
+    pr, ms_par = timed(lambda: cf.cf_pareto_select(mc["goodput_mrps"], alive))
+    P = pl.n_plans
+    return {"plans": P, "graph": "configs[2] Omni graph, 32 KEEP/MERGE patterns, sum c <= 64",
+            "flow_bound_ms": ms_flow, "mc_latency_ms": ms_mc, "pareto_select_ms": ms_par,
+            "mc_requests_sampled": g.n_req * g.n_trials, "non_redundant": int(alive.sum()),
+            "pareto_survivors": int(cf.to_numpy_u32(pr["n_survivors"])[0]),
+            "plans_per_s_flow_plus_mc": P / ((ms_flow + ms_mc) * 1e-3),
+            "paper_context": "Table 6 (PAPER.md:480-481): flow 3.48 s on 483.41 M plans, Monte Carlo 34.23 s on 1.95 M "
+                             "plans, planner host CPU not stated"}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -524,6 +558,11 @@ def main():
                   "l2": "flushed between timed steps (256 MiB fill)", "stream_materialise": head["stream_materialise"],
                   "wide_fixups": head["wide_fixups"], "bisect_probes": head["bisect_probes"],
                   "parallelism": f"replicas x{world} (one Philox variant per rank)"}
+        if args.config is None and world == 1:
+            try:
+                config["phases"] = measure_phases(torch, cf, stream)
+            except Exception as e:  # noqa: BLE001
+                config["phases"] = {"error": str(e)}
         if per:
             config["per_config"] = {f"cfg{c}": {k: v for k, v in r.items() if k != "stream_materialise"}
                                     for c, r in per.items()}

@@ -16,9 +16,16 @@
  *    rates uint32 milli-requests/s, gaps Q16 (65536 == one mean inter-arrival gap).
  *  - "host" pointers are read during the call only (descriptors, tables, plan lists: small).
  *    "dev" pointers are CUDA device pointers (e.g. torch.Tensor.data_ptr()); the caller owns all
- *    memory; nothing persistent is allocated by the library.
+ *    device memory. The only thing the library keeps between calls is a host-side cache (pinned
+ *    memory, at most 16 entries, LRU) of what cf_eval_plans* / cf_goodput_bisect* derive from their
+ *    host descriptors -- the launch schedule and the descriptor bytes they upload -- so that a call
+ *    repeated with byte-identical descriptors skips that work and its upload is a true asynchronous
+ *    copy. The cache never changes a result; cf_cache_clear() releases it.
  *  - Every compute call takes a cudaStream_t (as void*), enqueues its work on it and returns
- *    without synchronising (host-side scheduling happens before the first launch). Scratch comes
+ *    without synchronising (host-side scheduling happens before the first launch; the FIRST call
+ *    with given descriptors also allocates pinned memory, which may synchronise the device;
+ *    cf_trace_sim, cf_materialize_stream, cf_flow_bound and cf_mc_latency stage their small
+ *    descriptors through a pageable copy, which synchronises with the stream). Scratch comes
  *    from the caller's `workspace` (dev, >= cf_workspace_bytes(), 256-byte aligned); it must stay
  *    untouched until the stream work has finished. Distinct streams + distinct workspaces are
  *    thread-safe; no call reads or writes library-wide state.
@@ -218,6 +225,9 @@ int32_t cf_mc_latency(const cf_graph* g, const cf_plans* pl, const uint32_t* rat
 int32_t cf_pareto_select(const uint32_t* goodput_mrps, uint32_t n_plans, uint32_t n_types,
                          const uint8_t* alive, uint8_t* out_pruned, uint32_t* out_best,
                          uint32_t* out_n_survivors, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Releases the host-side cache of prepared calls (waits for uploads still in flight). */
+void cf_cache_clear(void);
 
 const char* cf_strerror(int32_t status);
 

@@ -7,6 +7,7 @@ import of this module raises, and without a CUDA device every compute call raise
 from __future__ import annotations
 
 import ctypes as C
+import functools
 import os
 from typing import Optional
 
@@ -24,7 +25,7 @@ EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_strea
            "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_strerror",
            "cf_workspace_wide_count", "cf_bisect_probes", "cf_aux_workspace_bytes",
-           "cf_pareto_workspace_bytes", "cf_flow_bound", "cf_mc_latency", "cf_pareto_select"]
+           "cf_pareto_workspace_bytes", "cf_flow_bound", "cf_mc_latency", "cf_pareto_select", "cf_cache_clear"]
 DEBUG_EXPORTS = ["cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
                  "cf_goodput_bisect_stream_opt", "cf_trace_sim_opt", "cf_last_launch_count",
                  "cf_bench_int32_peak"]
@@ -97,6 +98,13 @@ def _opt_active() -> bool:
     return bool(_OPT.kernel_mode or _OPT.bisect_depth or _OPT.bisect_predict)
 
 
+_lib.cf_cache_clear.restype = None
+
+
+def cf_cache_clear() -> None:
+    _lib.cf_cache_clear()
+
+
 def strerror(status: int) -> str:
     return _lib.cf_strerror(C.c_int32(status)).decode()
 
@@ -147,6 +155,21 @@ class Marshalled:
         if slo is not None:
             self.slo = cf_slo(_hp(slo.L_us, C.c_int64), _hp(slo.att_num, C.c_uint32),
                               _hp(slo.att_den, C.c_uint32))
+
+
+def _on_stream(fn):
+    """Runs the wrapped call with `stream` (keyword) as torch's current stream: the temporaries the
+    binding makes (rate arrays copied to the device, outputs, workspaces) are then allocated and
+    filled on the stream the library launches on, so there is no cross-stream race and the caching
+    allocator cannot hand them out again while the kernels still use them."""
+    @functools.wraps(fn)
+    def wrapped(*args, **kw):
+        stream = kw.get("stream")
+        if stream is None or not torch.cuda.is_available():
+            return fn(*args, **kw)
+        with torch.cuda.stream(stream):
+            return fn(*args, **kw)
+    return wrapped
 
 
 def _require_cuda():
@@ -217,6 +240,7 @@ def cf_last_launch_count() -> int:
     return int(_lib.cf_last_launch_count())
 
 
+@_on_stream
 def cf_eval_plans(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, out_counts=None,
                   out_dep_sum=None, out_makespan=None, workspace=None, stream=None, aux=True,
                   stream_records=None, n_variants: int = 1, plan_variant=None, check=True):
@@ -256,6 +280,7 @@ def cf_eval_plans(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, 
                 rc=int(rc))
 
 
+@_on_stream
 def cf_goodput_bisect(graph, plans, rate_hi_mrps, n_steps: int, slo, seed: int, variant: int = 0, *,
                       workspace=None, stream=None, stream_records=None, n_variants: int = 1,
                       plan_variant=None, want_counts=True, check=True):
@@ -294,6 +319,7 @@ def cf_stream_bytes(graph, n_variants: int) -> int:
     return int(_lib.cf_stream_bytes(C.byref(m.g), C.c_uint32(n_variants)))
 
 
+@_on_stream
 def cf_materialize_stream(graph, seed: int, variant_lo: int, n_variants: int, *, out=None,
                           stream=None, check=True):
     """Returns a CUDA uint8 tensor [n_variants, K, N, 32] of stream records."""
@@ -312,6 +338,7 @@ def cf_materialize_stream(graph, seed: int, variant_lo: int, n_variants: int, *,
     return out
 
 
+@_on_stream
 def cf_trace_sim(graph, plans, plan: int, rate_mrps: int, trial: int, seed: int, variant: int = 0, *,
                  stream=None, check=True):
     _require_cuda()
@@ -338,6 +365,7 @@ def _aux_workspace(m, stream_dev="cuda") -> torch.Tensor:
     return torch.empty(n, dtype=torch.uint8, device=stream_dev)
 
 
+@_on_stream
 def cf_flow_bound(graph, plans, alpha_num: int = 1, alpha_den: int = 1, *, stream=None, check=True):
     """Phase 1 on the device. Returns dict of CUDA tensors: rate_mrps int32 [P] (alpha R_d),
     bound_mrps int32 [P] (R_d), bottleneck uint8 [P], redundant uint8 [P]."""
@@ -356,6 +384,7 @@ def cf_flow_bound(graph, plans, alpha_num: int = 1, alpha_den: int = 1, *, strea
     return dict(rate_mrps=rate, bound_mrps=bound, bottleneck=bott, redundant=red, workspace=ws, rc=int(rc))
 
 
+@_on_stream
 def cf_mc_latency(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, want_counts=True, stream=None,
                   check=True):
     """Phase 2 on the device. rate_mrps: [P] CUDA int32 tensor or array-like. Returns dict of CUDA
@@ -376,6 +405,7 @@ def cf_mc_latency(graph, plans, rate_mrps, slo, seed: int, variant: int = 0, *, 
     return dict(counts=counts, goodput_mrps=good, workspace=ws, rc=int(rc))
 
 
+@_on_stream
 def cf_pareto_select(goodput_mrps, alive=None, *, stream=None, check=True):
     """Pruning + policy on the device. goodput_mrps: [P,T] CUDA int32 tensor or array-like; alive: [P]
     CUDA uint8 tensor, array-like or None. Returns dict of CUDA tensors: pruned uint8 [P], best int32

@@ -7,7 +7,10 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <list>
 #include <map>
+#include <memory>
+#include <mutex>
 #include <numeric>
 #include <vector>
 
@@ -838,6 +841,96 @@ int32_t cuda_rc(cudaError_t e) {
   return CF_ERR_CUDA;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Prepared calls. Everything a call derives from its host descriptors -- the schedule and the blob of
+// tables / schedule arrays it uploads -- is built once, kept in PINNED host memory and reused by later
+// calls with byte-identical descriptors (a planner evaluates the same candidate set at many seeds,
+// rates and brackets). The upload is then a true asynchronous copy and the call returns without
+// touching the stream's past work. At most kCacheEntries calls are remembered (LRU); cf_cache_clear()
+// releases them. The cache holds host memory only and never changes a result.
+// ------------------------------------------------------------------------------------------------
+constexpr size_t kCacheEntries = 16;
+
+struct Prepared {
+  Schedule sc;
+  KParams kp;  // graph part filled; pointers are set per call
+  size_t pool_off = 0, att_off = 0, den_off = 0, np_off = 0, blob_bytes = 0;
+  SchedOffsets so{};
+  uint32_t depth = 0;
+  bool fast = false;
+  uint8_t* pinned = nullptr;
+  std::mutex m;
+  std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;  // last upload per stream
+  bool many_streams = false;
+
+  cudaError_t upload(void* ws, cudaStream_t st) {
+    cudaError_t e = cudaMemcpyAsync(ws, pinned, blob_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lk(m);
+    for (auto& u : uses)
+      if (u.first == st) return cudaEventRecord(u.second, st);
+    if (uses.size() >= 8) { many_streams = true; return cudaSuccess; }
+    cudaEvent_t ev;
+    e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) return e;
+    uses.emplace_back(st, ev);
+    return cudaEventRecord(ev, st);
+  }
+  ~Prepared() {  // the pinned bytes may still be the source of a copy in flight
+    if (many_streams) cudaDeviceSynchronize();
+    for (auto& u : uses) { cudaEventSynchronize(u.second); cudaEventDestroy(u.second); }
+    if (pinned) cudaFreeHost(pinned);
+  }
+  int32_t adopt(const Blob& blob) {
+    blob_bytes = blob.bytes.size();
+    if (cudaHostAlloc(reinterpret_cast<void**>(&pinned), blob_bytes, cudaHostAllocDefault) != cudaSuccess) {
+      pinned = nullptr;
+      return cuda_rc(cudaGetLastError());
+    }
+    std::memcpy(pinned, blob.bytes.data(), blob_bytes);
+    return CF_OK;
+  }
+};
+
+struct KeyBuilder {
+  std::vector<uint8_t> b;
+  void put(const void* p, size_t n) { const uint8_t* q = static_cast<const uint8_t*>(p); b.insert(b.end(), q, q + n); }
+  template <class T> void val(const T& v) { put(&v, sizeof(T)); }
+  void tab(const cf_qtab& t) { val(t.levels); val(t.log2_cells); put(t.q, tab_entries(t) * 4); }
+  void graph(const cf_graph* g) {
+    val(g->n_comp); val(g->n_types); val(g->n_req); val(g->n_trials); val(g->n_tabs); val(g->n_edges); val(g->edge_delay_us);
+    put(g->type_mask, g->n_types); put(g->type_thresh, g->n_types * 4); put(g->svc_tab, (size_t)g->n_comp * g->n_types * 2);
+    for (uint32_t j = 0; j < g->n_tabs; ++j) tab(g->tabs[j]);
+    tab(g->arr_tab);
+    if (g->n_edges) put(g->edges, 2 * g->n_edges);
+  }
+  void plans(const cf_plans* pl) {
+    val(pl->n_plans); val(pl->max_stages);
+    put(pl->n_stages, pl->n_plans); put(pl->stage_mask, (size_t)pl->n_plans * pl->max_stages);
+    put(pl->stage_c, (size_t)pl->n_plans * pl->max_stages * 2);
+  }
+};
+
+std::mutex g_cache_mutex;
+std::list<std::pair<std::vector<uint8_t>, std::shared_ptr<Prepared>>> g_cache;  // most recent first
+
+std::shared_ptr<Prepared> cache_find(const std::vector<uint8_t>& key) {
+  std::lock_guard<std::mutex> lk(g_cache_mutex);
+  for (auto it = g_cache.begin(); it != g_cache.end(); ++it)
+    if (it->first.size() == key.size() && std::memcmp(it->first.data(), key.data(), key.size()) == 0) {
+      g_cache.splice(g_cache.begin(), g_cache, it);
+      return g_cache.front().second;
+    }
+  return nullptr;
+}
+
+void cache_insert(std::vector<uint8_t>&& key, const std::shared_ptr<Prepared>& p) {
+  std::list<std::pair<std::vector<uint8_t>, std::shared_ptr<Prepared>>> dropped;  // destroyed outside the lock
+  std::lock_guard<std::mutex> lk(g_cache_mutex);
+  g_cache.emplace_front(std::move(key), p);
+  while (g_cache.size() > kCacheEntries) dropped.splice(dropped.begin(), g_cache, std::prev(g_cache.end()));
+}
+
 // shared implementation of cf_eval_plans / cf_eval_plans_stream / cf_trace_sim
 struct EvalArgs {
   const cf_graph* g; const cf_plans* pl; const uint32_t* rates_dev; uint32_t R; const cf_slo* slo;
@@ -863,22 +956,32 @@ int32_t eval_impl(const EvalArgs& a) {
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
   if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
-  const bool fast = fast_path_ok(a.g, a.opt.kernel_mode);
-  Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1, a.stream_records != nullptr, nullptr, fast,
-                                  a.opt.kernel_mode, &sc))
-    return rc;
-  Blob blob;
-  blob.reserve(kAlign);  // status block
-  KParams kp;
-  const size_t pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &kp);
-  const SchedOffsets so = add_schedule(sc, &blob);
-  const size_t flags_off = align_up(blob.bytes.size());  // [P*R*K] bytes, written by the 32-bit kernel
+  KeyBuilder kb;
+  kb.val((uint32_t)1); kb.graph(a.g); kb.plans(a.pl); kb.val(a.R); kb.val(a.seed); kb.put(a.slo->L_us, a.g->n_types * 8);
+  kb.val(a.opt); kb.val((uint32_t)(a.stream_records != nullptr)); kb.val(a.n_variants);
+  if (a.stream_records && a.plan_variant) kb.put(a.plan_variant, (size_t)a.pl->n_plans * 4);
+  std::shared_ptr<Prepared> pp = cache_find(kb.b);
+  if (!pp) {
+    pp = std::make_shared<Prepared>();
+    Prepared& p = *pp;
+    p.fast = fast_path_ok(a.g, a.opt.kernel_mode);
+    if (int32_t rc = build_schedule(a.g, a.pl, a.R, a.plan_variant, a.stream_records ? a.n_variants : 1,
+                                    a.stream_records != nullptr, nullptr, p.fast, a.opt.kernel_mode, &p.sc))
+      return rc;
+    Blob blob;
+    blob.reserve(kAlign);  // status block
+    p.pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &p.kp);
+    p.so = add_schedule(p.sc, &blob);
+    if (int32_t rc = p.adopt(blob)) return rc;
+    cache_insert(std::move(kb.b), pp);
+  }
+  Prepared& p = *pp;
+  const size_t flags_off = align_up(p.blob_bytes);  // [P*R*K] bytes, written by the 32-bit kernel
   if (flags_off + (size_t)a.pl->n_plans * a.R * a.g->n_trials > a.ws_bytes) return CF_ERR_WORKSPACE;
   uint8_t* ws = static_cast<uint8_t*>(a.ws);
-  if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, a.st)))
-    return rc;
-  point_schedule(&kp, ws, so, pool_off);
+  if (int32_t rc = cuda_rc(p.upload(ws, a.st))) return rc;
+  KParams kp = p.kp;
+  point_schedule(&kp, ws, p.so, p.pool_off);
   kp.stream = static_cast<const uint4*>(a.stream_records);
   kp.variant_lo = a.stream_records ? 0 : a.variant;
   kp.rates = a.rates_dev;
@@ -886,7 +989,7 @@ int32_t eval_impl(const EvalArgs& a) {
   kp.out_dep_sum = a.out_dep_sum;
   kp.out_makespan = a.out_makespan;
   kp.flags = ws + flags_off;
-  return cuda_rc(launch_pass(kp, sc, a.g->n_trials, fast, a.st));
+  return cuda_rc(launch_pass(kp, p.sc, a.g->n_trials, p.fast, a.st));
 }
 
 struct BisectArgs {
@@ -906,29 +1009,43 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
-  const bool fast = fast_path_ok(a.g, a.opt.kernel_mode);
-  // speculation depth: enough simulations per pass to fill the GPU (one thread each), no more
-  uint32_t depth = a.opt.bisect_depth;
-  if (depth == 0) {
-    depth = 1;
-    while (depth < kMaxSpecDepth && (uint64_t)P * K * ((1u << depth) - 1u) < 90000ull) ++depth;
+  KeyBuilder kb;
+  kb.val((uint32_t)2); kb.graph(a.g); kb.plans(a.pl); kb.val(a.n_steps); kb.val(a.seed); kb.put(a.slo->L_us, T * 8);
+  kb.put(a.slo->att_num, T * 4); kb.put(a.slo->att_den, T * 4);
+  kb.val(a.opt); kb.val((uint32_t)(a.stream_records != nullptr)); kb.val(a.n_variants);
+  if (a.stream_records && a.plan_variant) kb.put(a.plan_variant, (size_t)P * 4);
+  std::shared_ptr<Prepared> pp = cache_find(kb.b);
+  if (!pp) {
+    pp = std::make_shared<Prepared>();
+    Prepared& p = *pp;
+    p.fast = fast_path_ok(a.g, a.opt.kernel_mode);
+    // speculation depth: enough simulations per pass to fill the GPU (one thread each), no more
+    uint32_t depth = a.opt.bisect_depth;
+    if (depth == 0) {
+      depth = 1;
+      while (depth < kMaxSpecDepth && (uint64_t)P * K * ((1u << depth) - 1u) < 90000ull) ++depth;
+    }
+    p.depth = std::min(depth, std::max(1u, a.n_steps));
+    if (int32_t rc = build_schedule(a.g, a.pl, (1u << p.depth) - 1u, a.plan_variant, a.stream_records ? a.n_variants : 1,
+                                    a.stream_records != nullptr, nullptr, p.fast, a.opt.kernel_mode, &p.sc))
+      return rc;
+    Blob blob;
+    blob.reserve(kAlign);
+    p.np_off = blob.reserve((size_t)P * 4);  // == kAlign: cf_bisect_probes reads it there
+    p.pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &p.kp);
+    p.so = add_schedule(p.sc, &blob);
+    p.att_off = blob.add(a.slo->att_num, T * 4);
+    p.den_off = blob.add(a.slo->att_den, T * 4);
+    if (int32_t rc = p.adopt(blob)) return rc;
+    cache_insert(std::move(kb.b), pp);
   }
-  depth = std::min(depth, std::max(1u, a.n_steps));
-  const uint32_t R = (1u << depth) - 1u;
-  Schedule sc;
-  if (int32_t rc = build_schedule(a.g, a.pl, R, a.plan_variant, a.stream_records ? a.n_variants : 1, a.stream_records != nullptr, nullptr, fast,
-                                  a.opt.kernel_mode, &sc))
-    return rc;
-  Blob blob;
-  blob.reserve(kAlign);
-  const size_t np_off = blob.reserve((size_t)P * 4);  // == kAlign: cf_bisect_probes reads it there
-  KParams kp;
-  const size_t pool_off = fill_graph_params(a.g, a.slo, a.seed, &blob, &kp);
-  const SchedOffsets so = add_schedule(sc, &blob);
-  const size_t att_off = blob.add(a.slo->att_num, T * 4);
-  const size_t den_off = blob.add(a.slo->att_den, T * 4);
+  Prepared& p = *pp;
+  const bool fast = p.fast;
+  const uint32_t depth = p.depth, R = (1u << depth) - 1u;
+  const Schedule& sc = p.sc;
+  const size_t np_off = p.np_off, att_off = p.att_off, den_off = p.den_off;
   const size_t per_plan = (size_t)K * T * 2;
-  const size_t blob_bytes = blob.bytes.size();
+  const size_t blob_bytes = p.blob_bytes;
   const size_t lo_off = align_up(blob_bytes), hi_off = align_up(lo_off + (size_t)P * 4);
   const size_t tree_off = align_up(hi_off + (size_t)P * 4);
   const size_t probe_off = align_up(tree_off + (size_t)P * R * 4);
@@ -936,9 +1053,9 @@ int32_t bisect_impl(const BisectArgs& a) {
   const size_t flags_off = align_up(at_lo_off + P * per_plan * 4);
   if (flags_off + (size_t)P * R * K > a.ws_bytes) return CF_ERR_WORKSPACE;
   uint8_t* ws = static_cast<uint8_t*>(a.ws);
-  if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob_bytes, cudaMemcpyHostToDevice, a.st)))
-    return rc;
-  point_schedule(&kp, ws, so, pool_off);
+  if (int32_t rc = cuda_rc(p.upload(ws, a.st))) return rc;
+  KParams kp = p.kp;
+  point_schedule(&kp, ws, p.so, p.pool_off);
   BisectState bs;
   bs.lo = reinterpret_cast<uint32_t*>(ws + lo_off);
   bs.hi = reinterpret_cast<uint32_t*>(ws + hi_off);
@@ -1204,6 +1321,12 @@ int32_t cf_workspace_status(const void* workspace, void* stream) {
 }
 
 uint32_t cf_last_launch_count(void) { return g_launch_count; }
+
+void cf_cache_clear(void) {
+  std::list<std::pair<std::vector<uint8_t>, std::shared_ptr<Prepared>>> dropped;  // destroyed outside the lock
+  std::lock_guard<std::mutex> lk(g_cache_mutex);
+  dropped.swap(g_cache);
+}
 
 int32_t cf_bisect_probes(const void* workspace, uint32_t n_plans, uint32_t* out_probes, void* stream) {
   if (!workspace || !out_probes) return CF_ERR_ARG;

@@ -442,6 +442,31 @@ def config4_sweep(n_req: int = 1 << 18, n_trials: int = 8, n_steps: int = 32,
                     n_variants=n_variants, plan_variant=pv)
 
 
+def config_phase_sweep(n_plans: int = 1_000_000, n_req: int = 1 << 17, n_trials: int = 8) -> Workload:
+    """A large candidate set for the cheap phases (flow bound, Monte-Carlo latency, Pareto pruning):
+    the Omni graph of configs[2], its 32 KEEP/MERGE patterns x n_plans/32 replica vectors with
+    sum c <= 64 drawn as in _replica_vectors but vectorised (numpy default_rng(6)). The paper's
+    funnel evaluates 1.95 M plans in its Monte-Carlo phase (Table 6)."""
+    g = _omni_graph4(n_req, n_trials, exponential_qtab(65536.0))
+    rng = np.random.default_rng(6)
+    pats = merge_patterns(6, OMNI_EDGES)[:32]
+    per = max(1, n_plans // len(pats))
+    ns, masks, cs = [], [], []
+    for stages in pats:
+        V = len(stages)
+        budget = rng.integers(V, 65, size=per)
+        wts = rng.dirichlet(np.ones(V), size=per)
+        c = 1 + np.floor(wts * (budget - V)[:, None]).astype(np.int64)
+        m = np.zeros((per, 6), dtype=np.uint8)
+        cc = np.zeros((per, 6), dtype=np.uint16)
+        m[:, :V] = np.asarray(stages, dtype=np.uint8)[None, :]
+        cc[:, :V] = c
+        ns.append(np.full(per, V, dtype=np.uint8)); masks.append(m); cs.append(cc)
+    plans = Plans(np.concatenate(ns), np.concatenate(masks), np.concatenate(cs))
+    slo = Slo([1_000_000, 10_000_000, 2_000_000, 10_000_000], [9] * 4, [10] * 4)
+    return Workload("phase_sweep", g, plans, slo, seed=6)
+
+
 def count_updates(graph: Graph, plans: Plans, counts: np.ndarray, per_plan: bool = False):
     """Exact number of request-stage updates from out_counts [P][R][K][T][2]: sum over sims and
     types of cnt_t * (number of stages of plan p that type t visits)."""

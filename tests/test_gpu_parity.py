@@ -392,3 +392,44 @@ def test_cfg4_full_size_sampled(cf, orc):
     assert (c[~feasible] == 0).all()
     att_ok = c[feasible][..., 1].sum(1) * 10 >= 9 * c[feasible][..., 0].sum(1)  # pooled 90 % per type
     assert att_ok.all()
+
+
+def test_prepared_call_cache_and_streams(cf, orc):
+    """Repeated calls reuse the pinned schedule / descriptor blob (cf.h "Conventions"); any change of a
+    descriptor byte must miss the cache. More distinct calls than the cache holds (eviction while
+    earlier uploads may be in flight), on a side stream, then cf_cache_clear."""
+    import torch
+    side = torch.cuda.Stream()
+    w = W.config1_mllm(n_req=400, n_trials=2, n_rates=2, llm_max=6, e_steps=2)
+    wants = {}
+    for rep in range(2):
+        for seed in range(20):  # 20 distinct descriptor sets > 16 cache entries
+            got = cf.cf_eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, seed, stream=side if seed % 2 else None)
+            if seed not in wants:
+                wants[seed] = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, seed, n_threads=NT)
+            (side if seed % 2 else torch.cuda.current_stream()).synchronize()
+            np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), wants[seed]["counts"])
+            np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), wants[seed]["dep_sum"])
+    # same descriptors, different device inputs (rates): a hit that must still see the new rates
+    r2 = (w.rate_mrps * 3 // 4).astype(np.uint32)
+    got = cf.cf_eval_plans(w.graph, w.plans, r2, w.slo, 19)
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]),
+                                  orc.eval_plans(w.graph, w.plans, r2, w.slo, 19, n_threads=NT)["counts"])
+    # one table entry, one replica count, one target changed: each a miss with the right answer
+    w2 = W.config1_mllm(n_req=400, n_trials=2, n_rates=2, llm_max=6, e_steps=2)
+    w2.graph.tabs[0].q[100] += 1
+    check_eval(cf, orc, w2)
+    w2.plans.stage_c[3, 0] += 1
+    check_eval(cf, orc, w2)
+    w2.slo = W.Slo([1_500_000, 3_000_000], [9, 9], [10, 10])
+    check_eval(cf, orc, w2)
+    hi = np.full(w.plans.n_plans, 30_000, np.uint32)
+    for steps, num in ((6, 9), (6, 8), (7, 9), (6, 9)):
+        slo = W.Slo(w.slo.L_us, [num, num], [10, 10])
+        b = cf.cf_goodput_bisect(w.graph, w.plans, hi, steps, slo, w.seed, stream=side)
+        side.synchronize()
+        bo = orc.goodput_bisect(w.graph, w.plans, hi, steps, slo, w.seed, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
+    cf.cf_cache_clear()
+    check_eval(cf, orc, w)

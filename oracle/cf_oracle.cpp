@@ -89,8 +89,12 @@ int32_t validate(const orc_graph* g, const orc_plans* pl) {
   for (uint32_t e = 0; e < g->n_edges; ++e)
     if (g->edges[2 * e] >= C || g->edges[2 * e + 1] >= C) return ORC_ERR_ARG;
   for (uint32_t i = 0; i < C; ++i)
-    for (uint32_t t = 0; t < T; ++t)
+    for (uint32_t t = 0; t < T; ++t) {
       if (((g->type_mask[t] >> i) & 1) && g->svc_tab[i * T + t] >= g->n_tabs) return ORC_ERR_ARG;
+      if (g->cpu_tab && ((g->type_mask[t] >> i) & 1) && g->cpu_tab[i * T + t] != 0xffff &&
+          g->cpu_tab[i * T + t] >= g->n_tabs)
+        return ORC_ERR_ARG;
+    }
   for (uint32_t j = 0; j < g->n_tabs; ++j)
     if (int32_t rc = check_qtab(g->tabs[j])) return rc;
   if (int32_t rc = check_qtab(g->arr_tab)) return rc;
@@ -102,7 +106,12 @@ int32_t validate(const orc_graph* g, const orc_plans* pl) {
     for (uint32_t t = 0; t < T; ++t)
       if ((g->type_mask[t] >> i) & 1) {
         const orc_qtab& tb = g->tabs[g->svc_tab[i * T + t]];
-        mx = std::max<int64_t>(mx, tb.q[qtab_entries(tb) - 1]);
+        int64_t both = tb.q[qtab_entries(tb) - 1];
+        if (g->cpu_tab && g->cpu_tab[i * T + t] != 0xffff) { /* R24: CPU + GPU time of an idle executor */
+          const orc_qtab& tc = g->tabs[g->cpu_tab[i * T + t]];
+          both += tc.q[qtab_entries(tc) - 1];
+        }
+        mx = std::max<int64_t>(mx, both);
       }
     worst += mx;
   }
@@ -180,24 +189,34 @@ void simulate(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate
       if (b0[1] < g->type_thresh[tt]) { t = tt; break; }
     const uint8_t tm = g->type_mask[t];
     int64_t svc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int64_t cpu[8] = {0, 0, 0, 0, 0, 0, 0, 0}; /* R24: CPU pre-processing time, paid only at an idle executor */
     for (uint32_t i = 0; i < C; ++i)
       if ((tm >> i) & 1) {
         uint32_t b[4];
         philox(n, k, 1 + i / 4, variant, k0, k1, b);
         svc[i] = qtab_sample(g->tabs[g->svc_tab[i * T + t]], b[i % 4]);
+        if (g->cpu_tab && g->cpu_tab[i * T + t] != 0xffff) {
+          philox(n, k, 3 + i / 4, variant, k0, k1, b);
+          cpu[i] = qtab_sample(g->tabs[g->cpu_tab[i * T + t]], b[i % 4]);
+        }
       }
     int64_t x = A;
     bool first = true;
     for (uint32_t s = 0; s < V; ++s) { /* stages in the plan's order */
       const uint8_t m = smask[s] & tm;
       if (m == 0) continue;
-      int64_t S = 0;
+      int64_t S = 0, S_cpu = 0;
       for (uint32_t i = 0; i < C; ++i)
-        if ((m >> i) & 1) S += svc[i];
+        if ((m >> i) & 1) { S += svc[i]; S_cpu += cpu[i]; }
       if (!first) x += g->edge_delay_us;
       first = false;
       const int64_t f = F[s][0]; /* earliest-free replica */
-      x = std::max(x, f) + S;
+      /* "When a request arrives at an idle multimodal encoder executor, it
+       * experiences the full CPU + GPU time. However, when the encoder is already busy, CPU
+       * preprocessing happens while the request is in the queue, and processing time reduces to
+       * GPU time alone" -- idle: the executor is free at the request's arrival (f <= x). */
+      if (f <= x) x = x + S_cpu + S;
+      else x = f + S;
       F[s][0] = x;
       std::sort(F[s].begin(), F[s].end());
     }
@@ -336,8 +355,8 @@ int32_t orc_trace_sim(const orc_graph* g, const orc_plans* pl, uint32_t plan, ui
 
 int32_t orc_materialize_stream(const orc_graph* g, uint64_t seed, uint32_t variant_lo,
                                uint32_t n_variants, void* out) {
-  if (!g || !out || g->n_comp < 1 || g->n_comp > 6 || g->n_types < 1 || g->n_types > 8)
-    return ORC_ERR_ARG;
+  if (!g || !out || g->n_comp < 1 || g->n_comp > 6 || g->n_types < 1 || g->n_types > 8 || g->cpu_tab)
+    return ORC_ERR_ARG; /* the 32-byte record has no room for CPU times (R24) */
   const uint32_t C = g->n_comp, T = g->n_types, N = g->n_req, K = g->n_trials;
   const uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
   uint8_t* dst = (uint8_t*)out;

@@ -56,6 +56,8 @@ typedef struct {
   const uint8_t* edges;        /* [2*n_edges] (u,v) pairs, component DAG                   */
   uint32_t n_edges;
   int64_t edge_delay_us;       /* PAPER.md:322; added between consecutive visited stages   */
+  const uint16_t* cpu_tab;     /* [C*T] table id of the CPU pre-processing time of (i, t), 0xffff = none;
+                                  NULL = no component has any (R24) */
 } orc_graph;
 
 /* P physical plans, each an ordered list of stages = (component bitmask, replica count). */

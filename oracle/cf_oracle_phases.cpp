@@ -139,6 +139,11 @@ int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* 
             uint32_t c2[4] = {n, k, 1 + i / 4, variant}, b[4];
             orc_philox4x32_10(c2, key, b);
             svc[i] = orc_qtab_sample(&g->tabs[g->svc_tab[i * T + t]], b[i % 4]);
+            if (g->cpu_tab && g->cpu_tab[i * T + t] != 0xffff) { /* R24: nobody queues, so every executor is idle */
+              uint32_t c3[4] = {n, k, 3 + i / 4, variant};
+              orc_philox4x32_10(c3, key, b);
+              svc[i] += orc_qtab_sample(&g->tabs[g->cpu_tab[i * T + t]], b[i % 4]);
+            }
           }
         int64_t lat = 0; /* accumulated latency along the path, no waiting */
         bool first = true;

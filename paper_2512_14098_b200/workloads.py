@@ -50,8 +50,11 @@ class Graph:
     comp_names: Tuple[str, ...] = ()
     type_names: Tuple[str, ...] = ()
     type_frac: Optional[np.ndarray] = None  # float64 [T], the mix the thresholds were built from
+    cpu_tab: Optional[np.ndarray] = None    # uint16 [C*T] CPU pre-processing table of (i, t), 0xffff = none (R24)
 
     def __post_init__(self):
+        if self.cpu_tab is not None:
+            self.cpu_tab = np.ascontiguousarray(self.cpu_tab, dtype=np.uint16)
         self.type_mask = np.ascontiguousarray(self.type_mask, dtype=np.uint8)
         self.type_thresh = np.ascontiguousarray(self.type_thresh, dtype=np.uint32)
         self.svc_tab = np.ascontiguousarray(self.svc_tab, dtype=np.uint16)

@@ -77,6 +77,11 @@ typedef struct {
   const uint8_t* edges;        /* [2*n_edges] (u,v): component u feeds component v (validation)    */
   uint32_t n_edges;
   int64_t edge_delay_us;       /* PAPER.md:322; added between consecutive visited stages; [0,2^31) */
+  const uint16_t* cpu_tab;     /* [C*T] id of the CPU pre-processing time table of (i, t), 0xffff = none; or
+                                  NULL. CPU-GPU overlap of PAPER.md:318-320 (R24): a request that
+                                  finds the stage's earliest-free replica idle pays CPU + GPU time (svc_tab is
+                                  the GPU time), a request that queued pays GPU time alone. Such graphs run on
+                                  the 64-bit kernel and cannot be materialised as a stream (CF_ERR_ARG).    */
 } cf_graph;
 
 /* P physical plans; plan p is an ORDERED list of n_stages[p] stages, stage s = (bitmask of the

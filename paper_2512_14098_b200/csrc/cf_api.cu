@@ -63,8 +63,12 @@ int32_t check_graph(const cf_graph* g) {
   for (uint32_t e = 0; e < 2 * g->n_edges; ++e)
     if (g->edges[e] >= C) return CF_ERR_ARG;
   for (uint32_t i = 0; i < C; ++i)
-    for (uint32_t t = 0; t < T; ++t)
+    for (uint32_t t = 0; t < T; ++t) {
       if (((g->type_mask[t] >> i) & 1) && g->svc_tab[i * T + t] >= g->n_tabs) return CF_ERR_ARG;
+      if (((g->type_mask[t] >> i) & 1) && g->cpu_tab && g->cpu_tab[i * T + t] != 0xffff &&
+          g->cpu_tab[i * T + t] >= g->n_tabs)
+        return CF_ERR_ARG;
+    }
   for (uint32_t j = 0; j < g->n_tabs; ++j)
     if (int32_t rc = check_tab(g->tabs[j])) return rc;
   if (int32_t rc = check_tab(g->arr_tab)) return rc;
@@ -76,12 +80,26 @@ int32_t check_graph(const cf_graph* g) {
     for (uint32_t t = 0; t < T; ++t)
       if ((g->type_mask[t] >> i) & 1) {
         const cf_qtab& tb = g->tabs[g->svc_tab[i * T + t]];
-        mx = std::max<int64_t>(mx, tb.q[tab_entries(tb) - 1]);
+        int64_t both = tb.q[tab_entries(tb) - 1];
+        if (g->cpu_tab && g->cpu_tab[i * T + t] != 0xffff) {  // an idle executor takes CPU + GPU time (R24)
+          const cf_qtab& tc = g->tabs[g->cpu_tab[i * T + t]];
+          both += tc.q[tab_entries(tc) - 1];
+        }
+        mx = std::max<int64_t>(mx, both);
       }
     worst += mx;
   }
   if (worst > INT32_MAX) return CF_ERR_RANGE;
   return CF_OK;
+}
+
+// R24: does any (component, type) the workload uses have a CPU pre-processing table?
+bool graph_has_cpu(const cf_graph* g) {
+  if (!g->cpu_tab) return false;
+  for (uint32_t i = 0; i < g->n_comp; ++i)
+    for (uint32_t t = 0; t < g->n_types; ++t)
+      if (((g->type_mask[t] >> i) & 1) && g->cpu_tab[i * g->n_types + t] != 0xffff) return true;
+  return false;
 }
 
 int32_t check_plans(const cf_graph* g, const cf_plans* pl) {
@@ -134,17 +152,18 @@ struct Schedule {
   uint32_t R = 1;
 };
 
-template <int W>
+template <int W, bool HAS_CPU>
 uint32_t fixed_smem_w(int vmax, int cmax) {
   if (cmax <= 6) {
-    if (vmax <= 2) return SmemLayout<2, 6, W>::fixed_bytes;
-    if (vmax <= 6) return SmemLayout<6, 6, W>::fixed_bytes;
-    return SmemLayout<8, 6, W>::fixed_bytes;
+    if (vmax <= 2) return SmemLayout<2, 6, W, HAS_CPU>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout<6, 6, W, HAS_CPU>::fixed_bytes;
+    return SmemLayout<8, 6, W, HAS_CPU>::fixed_bytes;
   }
-  return SmemLayout<8, 8, W>::fixed_bytes;
+  return SmemLayout<8, 8, W, HAS_CPU>::fixed_bytes;
 }
-uint32_t fixed_smem(int vmax, int cmax, int warps) {
-  return warps == 4 ? fixed_smem_w<4>(vmax, cmax) : fixed_smem_w<8>(vmax, cmax);
+uint32_t fixed_smem(int vmax, int cmax, int warps, bool has_cpu) {
+  if (has_cpu) return warps == 4 ? fixed_smem_w<4, true>(vmax, cmax) : fixed_smem_w<8, true>(vmax, cmax);
+  return warps == 4 ? fixed_smem_w<4, false>(vmax, cmax) : fixed_smem_w<8, false>(vmax, cmax);
 }
 
 template <int W, bool PW>
@@ -216,6 +235,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   // thread per simulation when the call has few simulations (config 0: 32 per call), 5.7x slower
   // when there are enough to fill the GPU with threads (measured crossover near 9 000 simulations).
   if (!only_plan && (uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
+  if (graph_has_cpu(g)) sc.all_c1 = false;  // the idle/busy rule (R24) is not max-plus linear
   if (kernel_mode == CF_KERNEL_SCAN && !sc.all_c1) return CF_ERR_ARG;  // one replica everywhere, <= 8192 simulations
   // the forced thread-per-simulation modes (cf_debug.h) keep that path; so do traces unless asked otherwise
   if (kernel_mode == CF_KERNEL_WIDE64 || kernel_mode == CF_KERNEL_FAST32) sc.all_c1 = false;
@@ -230,7 +250,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   const bool pw = streamed;
   sc.warps_per_cta = (R >= 8 && !pw) ? 8 : 4;
   const uint32_t kWarpsPerCta = (uint32_t)sc.warps_per_cta;
-  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax, sc.warps_per_cta),
+  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax, sc.warps_per_cta, graph_has_cpu(g)),
                  fixed_f = fixed_smem32(sc.vmax32, sc.cmax, sc.warps_per_cta, pw);
   const uint32_t fixed = fast ? fixed_f : fixed_w;  // the layout that is packed for occupancy
 
@@ -461,6 +481,11 @@ size_t fill_graph_params(const cf_graph* g, const cf_slo* slo, uint64_t seed, Bl
       if ((g->type_mask[t] >> i) & 1) {
         const uint32_t id = g->svc_tab[i * g->n_types + t];
         kp->svc_tab[i * 8 + t] = DevTab{tab_off[id], g->tabs[id].levels, g->tabs[id].log2_cells, 0};
+        if (g->cpu_tab && g->cpu_tab[i * g->n_types + t] != 0xffff) {
+          const uint32_t ic = g->cpu_tab[i * g->n_types + t];
+          kp->cpu_tab[i * 8 + t] = DevTab{tab_off[ic], g->tabs[ic].levels, g->tabs[ic].log2_cells, 0};
+          kp->has_cpu = 1;
+        }
       }
   kp->edge_delay = g->edge_delay_us;
   kp->seed_lo = (uint32_t)seed;
@@ -542,6 +567,7 @@ cudaError_t launch_sims32(KParams kp, const Schedule& sc, uint32_t n_trials, cud
 // at 2^30. Anything else runs on the 64-bit kernel alone.
 bool fast_path_ok(const cf_graph* g, uint32_t kernel_mode) {
   if (kernel_mode == CF_KERNEL_WIDE64) return false;
+  if (graph_has_cpu(g)) return false;  // CPU-GPU overlap (R24) runs on the 64-bit kernel
   int64_t worst = 0;
   for (uint32_t i = 0; i < g->n_comp; ++i) {
     int64_t mx = 0;
@@ -903,6 +929,8 @@ struct KeyBuilder {
     for (uint32_t j = 0; j < g->n_tabs; ++j) tab(g->tabs[j]);
     tab(g->arr_tab);
     if (g->n_edges) put(g->edges, 2 * g->n_edges);
+    val((uint32_t)(g->cpu_tab != nullptr));
+    if (g->cpu_tab) put(g->cpu_tab, (size_t)g->n_comp * g->n_types * 2);
   }
   void plans(const cf_plans* pl) {
     val(pl->n_plans); val(pl->max_stages);
@@ -954,7 +982,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_graph(a.g)) return rc;
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g))) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   KeyBuilder kb;
   kb.val((uint32_t)1); kb.graph(a.g); kb.plans(a.pl); kb.val(a.R); kb.val(a.seed); kb.put(a.slo->L_us, a.g->n_types * 8);
@@ -1006,7 +1034,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rate_hi_dev || !a.slo || !a.slo->L_us || !a.slo->att_num || !a.slo->att_den || !a.out_rate || !a.out_goodput)
     return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1)) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g))) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
   KeyBuilder kb;
@@ -1226,6 +1254,7 @@ int32_t cf_materialize_stream(const cf_graph* g, uint64_t seed, uint32_t variant
   g_launch_count = 0;
   if (int32_t rc = check_graph(g)) return rc;
   if (g->n_comp > 6 || n_variants < 1 || n_variants > 65535 || !out_stream) return CF_ERR_ARG;
+  if (graph_has_cpu(g)) return CF_ERR_ARG;  // the 32-byte record has no room for CPU times (R24)
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const uint32_t chunks = (g->n_req + 31) / 32;
   Blob blob;
@@ -1419,6 +1448,7 @@ int32_t aux_setup(const cf_graph* g, const cf_plans* pl, const cf_slo* slo, uint
   std::memcpy(ap.type_thresh, kp.type_thresh, sizeof(ap.type_thresh));
   std::memcpy(ap.type_mask, kp.type_mask, sizeof(ap.type_mask));
   std::memcpy(ap.svc_tab, kp.svc_tab, sizeof(ap.svc_tab));
+  std::memcpy(ap.cpu_tab, kp.cpu_tab, sizeof(ap.cpu_tab));
   std::memcpy(ap.L_us, kp.L_us, sizeof(ap.L_us));
   ap.edge_delay = kp.edge_delay; ap.seed_lo = kp.seed_lo; ap.seed_hi = kp.seed_hi; ap.variant = variant;
   // table descriptors in table-id order (fill_graph_params lays the pool out in that order)

@@ -49,6 +49,7 @@ struct AuxParams {
   uint32_t type_thresh[8];
   uint8_t type_mask[8];
   DevTab svc_tab[64];   // [i*8 + t]
+  DevTab cpu_tab[64];   // [i*8 + t] CPU pre-processing time (R24); levels == 0: none
   uint32_t tab_id[64];  // table id of (i, t): index into mean_q16
   const int32_t* qpool;
   const DevTab* tabs;   // [n_tabs]
@@ -180,6 +181,22 @@ __global__ void __launch_bounds__(256) mc_hist_kernel(const __grid_constant__ Au
       if (tm & 32u) total += qtab_sample(prm.qpool, prm.svc_tab[5 * 8 + t], b2.y);
       if (tm & 64u) total += qtab_sample(prm.qpool, prm.svc_tab[6 * 8 + t], b2.z);
       if (tm & 128u) total += qtab_sample(prm.qpool, prm.svc_tab[7 * 8 + t], b2.w);
+    }
+    // R24: nobody queues, so every executor is idle at every arrival: CPU time on top (blocks 3 + i/4)
+    uint32_t lo = 0, hi = 0;
+    for (uint32_t i = 0; i < prm.C; ++i)
+      if (((tm >> i) & 1u) && prm.cpu_tab[i * 8 + t].levels) { if (i < 4) lo = 1; else hi = 1; }
+    if (lo) {
+      const uint4 b3 = philox4x32_10(n, trial, 3, prm.variant, prm.seed_lo, prm.seed_hi);
+      const uint32_t u[4] = {b3.x, b3.y, b3.z, b3.w};
+      for (uint32_t i = 0; i < 4 && i < prm.C; ++i)
+        if (((tm >> i) & 1u) && prm.cpu_tab[i * 8 + t].levels) total += qtab_sample(prm.qpool, prm.cpu_tab[i * 8 + t], u[i]);
+    }
+    if (hi) {
+      const uint4 b4 = philox4x32_10(n, trial, 4, prm.variant, prm.seed_lo, prm.seed_hi);
+      const uint32_t u[4] = {b4.x, b4.y, b4.z, b4.w};
+      for (uint32_t i = 4; i < prm.C; ++i)
+        if (((tm >> i) & 1u) && prm.cpu_tab[i * 8 + t].levels) total += qtab_sample(prm.qpool, prm.cpu_tab[i * 8 + t], u[i - 4]);
     }
     atomicAdd(&h_s[t * 9 + 8], 1u);
     const int64_t L = prm.L_us[t];

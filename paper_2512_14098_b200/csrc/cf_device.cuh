@@ -64,6 +64,7 @@ struct KParams {
   uint32_t type_thresh[8];
   uint8_t type_mask[8];
   DevTab svc_tab[64];  // [i*8 + t]
+  DevTab cpu_tab[64];  // [i*8 + t] CPU pre-processing time (R24); levels == 0: none
   DevTab arr_tab;
   const int32_t* qpool;
   int64_t L_us[8];
@@ -98,6 +99,7 @@ struct KParams {
   int64_t* tr_departure;
   uint8_t* tr_type;
   uint32_t tr_plan;        // the traced plan (scan kernel: the warp whose simulation is written out)
+  uint32_t has_cpu;        // some (component, type) has a CPU pre-processing table (R24): 64-bit kernel only
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -149,22 +151,25 @@ __device__ __forceinline__ uint64_t warp_inclusive_sum(uint64_t v, int lane) {
 // Component-level record of one request in shared memory (and, for C <= 6, in the HBM stream):
 //   w0.x,w0.y = cu (56 bit) | type << 56 ; w0.z,w0.w,w1.* = svc[0..5] ; (C > 6: w2.x,w2.y = svc[6..7])
 // In-register mode cu is relative to the start of the 32-request chunk; the consumer adds the base.
-template <int CMAX>
+// HAS_CPU (R24, 64-bit kernel only): two more words hold the CPU pre-processing times cpu[0..7]
+template <int CMAX, bool HAS_CPU = false>
 struct CompRec {
-  static constexpr int kWords = (CMAX <= 6) ? 2 : 3;  // uint4 words
+  static constexpr int kBase = (CMAX <= 6) ? 2 : 3;  // uint4 words
+  static constexpr int kWords = kBase + (HAS_CPU ? 2 : 0);
 };
 
 // Stage-level record a warp builds for its topology: cu (absolute) | type<<56, then S[s] per stage
 // (-1 = stage not visited by this request's type).
-template <int VMAX>
+template <int VMAX, bool HAS_CPU = false>
 struct StageRec {
-  static constexpr int kWords = (VMAX <= 2) ? 1 : (VMAX <= 6 ? 2 : 3);
+  static constexpr int kBase = (VMAX <= 2) ? 1 : (VMAX <= 6 ? 2 : 3);
+  static constexpr int kWords = kBase + (HAS_CPU ? (VMAX <= 4 ? 1 : 2) : 0);  // + summed CPU time per stage
 };
 
 // ------------------------------------------------------------------------------------------------
 // Producer: chunk `chunk` (32 requests starting at n0) of the tile, one request per lane.
 // ------------------------------------------------------------------------------------------------
-template <int CMAX>
+template <int CMAX, bool HAS_CPU = false>
 __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_t n0, uint32_t trial,
                                                      uint32_t variant, uint4* tile_chunk,
                                                      uint64_t* chunk_total, uint32_t* cnt_s,
@@ -200,31 +205,62 @@ __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_
     }
     atomicAdd(&cnt_s[t], 1u);
   }
+  int32_t cpu[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) cpu[i] = 0;
+  if (HAS_CPU && valid) {  // R24: CPU times from Philox blocks 3 + i/4, word i % 4
+    const uint32_t tm = prm.type_mask[t];
+    bool lo = false, hi = false;
+#pragma unroll
+    for (int i = 0; i < CMAX; ++i) {
+      const bool has = ((tm >> i) & 1u) && prm.cpu_tab[i * 8 + t].levels != 0u;
+      if (i < 4) lo = lo || has; else hi = hi || has;
+    }
+    if (lo) {
+      const uint4 b3 = philox4x32_10(n, trial, 3, variant, prm.seed_lo, prm.seed_hi);
+      const uint32_t u[4] = {b3.x, b3.y, b3.z, b3.w};
+#pragma unroll
+      for (int i = 0; i < 4 && i < CMAX; ++i)
+        if (((tm >> i) & 1u) && prm.cpu_tab[i * 8 + t].levels) cpu[i] = qtab_sample(prm.qpool, prm.cpu_tab[i * 8 + t], u[i]);
+    }
+    if (hi) {
+      const uint4 b4 = philox4x32_10(n, trial, 4, variant, prm.seed_lo, prm.seed_hi);
+      const uint32_t u[4] = {b4.x, b4.y, b4.z, b4.w};
+#pragma unroll
+      for (int i = 4; i < CMAX; ++i)
+        if (((tm >> i) & 1u) && prm.cpu_tab[i * 8 + t].levels) cpu[i] = qtab_sample(prm.qpool, prm.cpu_tab[i * 8 + t], u[i - 4]);
+    }
+  }
   const uint64_t cu = warp_inclusive_sum((uint64_t)gap, lane);  // relative to the chunk start
   if (lane == 31) *chunk_total = cu;
-  uint4* dst = tile_chunk + lane * CompRec<CMAX>::kWords;
+  uint4* dst = tile_chunk + lane * CompRec<CMAX, HAS_CPU>::kWords;
   dst[0] = make_uint4((uint32_t)cu, (uint32_t)(cu >> 32) | (t << 24), (uint32_t)svc[0], (uint32_t)svc[1]);
   dst[1] = make_uint4((uint32_t)svc[2], (uint32_t)svc[3], (uint32_t)svc[4], (uint32_t)svc[5]);
   if (CMAX > 6) dst[2] = make_uint4((uint32_t)svc[6], (uint32_t)svc[7], 0u, 0u);
+  if (HAS_CPU) {
+    constexpr int kB = CompRec<CMAX, HAS_CPU>::kBase;
+    dst[kB] = make_uint4((uint32_t)cpu[0], (uint32_t)cpu[1], (uint32_t)cpu[2], (uint32_t)cpu[3]);
+    dst[kB + 1] = make_uint4((uint32_t)cpu[4], (uint32_t)cpu[5], (uint32_t)cpu[6], (uint32_t)cpu[7]);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
 // Producer of one CTA tile (kTile requests) into buffer tile_idx & 1: in-register Philox draws
 // (a1-a3) or a copy of the materialised stream (a10). Shared by both simulation kernels.
 // ------------------------------------------------------------------------------------------------
-template <int CMAX, int WARPS>
+template <int CMAX, int WARPS, bool HAS_CPU = false>
 __device__ __forceinline__ void produce_tile(const KParams& prm, uint32_t cta_variant, uint32_t trial,
                                              uint32_t variant, uint32_t tile_idx, uint4* tiles,
                                              uint64_t* totals, uint32_t* cnt_s, int tid, int warp,
                                              int lane) {
   const uint32_t buf = tile_idx & 1u;
-  uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
+  uint4* tb = tiles + buf * kTile * CompRec<CMAX, HAS_CPU>::kWords;
   const uint32_t n0 = tile_idx * kTile;
   if (prm.stream == nullptr) {
     for (int ch = warp; ch < kChunks; ch += WARPS)
-      produce_chunk_philox<CMAX>(prm, n0 + ch * 32, trial, variant,
-                                 tb + ch * 32 * CompRec<CMAX>::kWords, totals + buf * kChunks + ch,
-                                 cnt_s, lane);
+      produce_chunk_philox<CMAX, HAS_CPU>(prm, n0 + ch * 32, trial, variant,
+                                          tb + ch * 32 * CompRec<CMAX, HAS_CPU>::kWords,
+                                          totals + buf * kChunks + ch, cnt_s, lane);
   } else {
     // a10: copy kTile 32-byte records (2 x uint4 each) from the materialised stream; cu is absolute
     const uint4* src = prm.stream + ((size_t)(cta_variant * prm.K + trial) * prm.N + n0) * 2;
@@ -276,10 +312,10 @@ __device__ __forceinline__ void heap_replace_min(uint8_t* smem, int64_t& root, u
 // The simulation kernel. grid = (CTAs of this launch, K trials); block = kThreads.
 // Dynamic shared memory: [tiles 2 x kTile x CompRec][chunk totals][cnt][L][warp stage buffers][heaps]
 // ------------------------------------------------------------------------------------------------
-template <int VMAX, int CMAX, int WARPS>
+template <int VMAX, int CMAX, int WARPS, bool HAS_CPU = false>
 struct SmemLayout {
-  static constexpr uint32_t kCompRecBytes = CompRec<CMAX>::kWords * 16;
-  static constexpr uint32_t kStageRecBytes = StageRec<VMAX>::kWords * 16;
+  static constexpr uint32_t kCompRecBytes = CompRec<CMAX, HAS_CPU>::kWords * 16;
+  static constexpr uint32_t kStageRecBytes = StageRec<VMAX, HAS_CPU>::kWords * 16;
   static constexpr uint32_t tiles = 0;
   static constexpr uint32_t totals = tiles + 2 * kTile * kCompRecBytes;
   static constexpr uint32_t cnt = totals + 2 * kChunks * 8;
@@ -289,10 +325,13 @@ struct SmemLayout {
   static constexpr uint32_t fixed_bytes = heaps;
 };
 
-template <int VMAX, int CMAX, bool HAS_DELAY, int WARPS>
+// HAS_CPU: the CPU-GPU overlap rule of PAPER.md:318-320 (R24): a request that finds the earliest-free
+// replica idle pays its CPU pre-processing time on top of the GPU time, a queued one GPU time alone
+template <int VMAX, int CMAX, bool HAS_DELAY, int WARPS, bool HAS_CPU = false>
 __global__ void __launch_bounds__(WARPS * 32)
 cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
-  using SL = SmemLayout<VMAX, CMAX, WARPS>;
+  using SL = SmemLayout<VMAX, CMAX, WARPS, HAS_CPU>;
+  constexpr int kCW = CompRec<CMAX, HAS_CPU>::kWords, kSW = StageRec<VMAX, HAS_CPU>::kWords;
   extern __shared__ __align__(16) uint8_t smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t trial = prm.trial_base + blockIdx.x % prm.k_launch;
@@ -303,7 +342,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   uint64_t* totals = reinterpret_cast<uint64_t*>(smem + SL::totals);
   uint32_t* cnt_s = reinterpret_cast<uint32_t*>(smem + SL::cnt);
   int64_t* L_s = reinterpret_cast<int64_t*>(smem + SL::lus);
-  uint4* wbuf = reinterpret_cast<uint4*>(smem + SL::wbuf) + warp * 32 * StageRec<VMAX>::kWords;
+  uint4* wbuf = reinterpret_cast<uint4*>(smem + SL::wbuf) + warp * 32 * kSW;
 
   if (tid < 8) {
     cnt_s[tid] = 0;
@@ -376,7 +415,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
   // ---- producer for one tile -----------------------------------------------------------------
   const uint32_t n_tiles = (prm.N + kTile - 1) / kTile;
   auto produce = [&](uint32_t tile_idx) {
-    produce_tile<CMAX, WARPS>(prm, cta.variant, trial, variant, tile_idx, tiles, totals, cnt_s, tid, warp, lane);
+    produce_tile<CMAX, WARPS, HAS_CPU>(prm, cta.variant, trial, variant, tile_idx, tiles, totals, cnt_s, tid, warp, lane);
   };
 
   __syncthreads();
@@ -391,7 +430,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
     if (!streamed && tile_idx + 1 < n_tiles) produce(tile_idx + 1);
     if (consume) {
       const uint32_t buf = tile_idx & 1u;
-      const uint4* tb = tiles + buf * kTile * CompRec<CMAX>::kWords;
+      const uint4* tb = tiles + buf * kTile * kCW;
       const uint32_t n0 = tile_idx * kTile;
 #pragma unroll 1
       for (int ch = 0; ch < kChunks; ++ch) {
@@ -400,7 +439,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
         const int n_here = (int)min(32u, prm.N - nc0);
         // ---- a4: component-level -> stage-level records for this warp's topology -------------
         {
-          const uint4* src = tb + (ch * 32 + lane) * CompRec<CMAX>::kWords;
+          const uint4* src = tb + (ch * 32 + lane) * kCW;
           uint4 w0 = make_uint4(0u, 0u, 0u, 0u), w1 = w0;
           if (!streamed) {
             w0 = src[0]; w1 = src[1];
@@ -421,16 +460,36 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
             }
           const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;
           const uint32_t tm = prm.type_mask[t];
-          int32_t S[VMAX];
+          int32_t cpu[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) cpu[i] = 0;
+          if (HAS_CPU) {
+            const uint4 c0 = src[CompRec<CMAX, HAS_CPU>::kBase], c1 = src[CompRec<CMAX, HAS_CPU>::kBase + 1];
+            cpu[0] = (int32_t)c0.x; cpu[1] = (int32_t)c0.y; cpu[2] = (int32_t)c0.z; cpu[3] = (int32_t)c0.w;
+            cpu[4] = (int32_t)c1.x; cpu[5] = (int32_t)c1.y; cpu[6] = (int32_t)c1.z; cpu[7] = (int32_t)c1.w;
+          }
+          int32_t S[VMAX], Sc[VMAX];
 #pragma unroll
           for (int s = 0; s < VMAX; ++s) {
             const uint32_t sm = (s < topo.n_stages) ? topo.mask[s] : 0u;
-            int32_t acc = 0;
+            int32_t acc = 0, accc = 0;
 #pragma unroll
-            for (int i = 0; i < CMAX; ++i) acc += ((sm >> i) & 1u) ? svc[i] : 0;
+            for (int i = 0; i < CMAX; ++i) {
+              acc += ((sm >> i) & 1u) ? svc[i] : 0;
+              accc += ((sm >> i) & 1u) ? cpu[i] : 0;
+            }
             S[s] = (sm & tm) ? acc : -1;
+            Sc[s] = accc;
           }
-          uint4* dst = wbuf + lane * StageRec<VMAX>::kWords;
+          uint4* dst = wbuf + lane * kSW;
+          if (HAS_CPU) {
+            constexpr int kB = StageRec<VMAX, HAS_CPU>::kBase;
+            dst[kB] = make_uint4((uint32_t)Sc[0], (uint32_t)Sc[VMAX > 1 ? 1 : 0], (uint32_t)Sc[VMAX > 2 ? 2 : 0],
+                                 (uint32_t)Sc[VMAX > 3 ? 3 : 0]);
+            if (VMAX > 4)
+              dst[kB + 1] = make_uint4((uint32_t)Sc[VMAX > 4 ? 4 : 0], (uint32_t)Sc[VMAX > 5 ? 5 : 0],
+                                       (uint32_t)Sc[VMAX > 6 ? 6 : 0], (uint32_t)Sc[VMAX > 7 ? 7 : 0]);
+          }
           const uint32_t hi = (uint32_t)(cu >> 32) | (t << 24);
           if (VMAX <= 2) {
             dst[0] = make_uint4((uint32_t)cu, hi, (uint32_t)S[0], (uint32_t)S[VMAX > 1 ? 1 : 0]);
@@ -446,8 +505,26 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
         uint64_t hp = 0;  // per-type hit counters of this chunk, one byte each
 #pragma unroll 1
         for (int r = 0; r < n_here; ++r) {
-          const uint4* rp = wbuf + r * StageRec<VMAX>::kWords;
+          const uint4* rp = wbuf + r * kSW;
           const uint4 w0 = rp[0];
+          int32_t Sc[VMAX];
+#pragma unroll
+          for (int s = 0; s < VMAX; ++s) Sc[s] = 0;
+          if (HAS_CPU) {
+            constexpr int kB = StageRec<VMAX, HAS_CPU>::kBase;
+            const uint4 c0 = rp[kB];
+            Sc[0] = (int32_t)c0.x;
+            if (VMAX > 1) Sc[1] = (int32_t)c0.y;
+            if (VMAX > 2) Sc[2] = (int32_t)c0.z;
+            if (VMAX > 3) Sc[3] = (int32_t)c0.w;
+            if (VMAX > 4) {
+              const uint4 c1 = rp[kB + 1];
+              Sc[4] = (int32_t)c1.x;
+              if (VMAX > 5) Sc[5] = (int32_t)c1.y;
+              if (VMAX > 6) Sc[6] = (int32_t)c1.z;
+              if (VMAX > 7) Sc[7] = (int32_t)c1.w;
+            }
+          }
           int32_t S[VMAX];
           S[0] = (int32_t)w0.z;
           if (VMAX > 1) S[1] = (int32_t)w0.w;
@@ -474,7 +551,9 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
             if (S[s] >= 0) {
               if (HAS_DELAY) { if (!first) x += delay; first = false; }
               const int64_t f = root[s];
-              x = (x > f ? x : f) + (int64_t)S[s];  // a5/a6: start at max(arrival, earliest free)
+              if (HAS_CPU) x = (f <= x) ? x + (int64_t)Sc[s] : f;  // idle: CPU + GPU; queued: GPU alone (R24)
+              else x = x > f ? x : f;                              // a5/a6: start at max(arrival, earliest free)
+              x += (int64_t)S[s];
               heap_replace_min(smem, root[s], hb[s], sim_c[s], x);
             }
           }

@@ -192,3 +192,46 @@ def erlang_c(c: int, a: float) -> float:
         s += term
     last = term * a / c / (1.0 - a / c)
     return last / (s + last)
+
+
+def fcfs_event_sim(A: List[int], routes, stage_c: List[int], edge_delay: int = 0) -> List[int]:
+    """Textbook FCFS at every stage: a stage serves its visitors in the order in which they REACH
+    the stage (ties by request index), on the server that frees first. This is the discipline
+    index-order service (R2) departs from when stage arrivals are not monotone in the
+    request index; used to measure that gap, not to pin the oracle."""
+    n_stage = len(stage_c)
+    free = [[0] * c for c in stage_c]
+    queue = [[] for _ in range(n_stage)]          # heap of (arrival at the stage, request)
+    pos = [0] * len(A)
+    dep = [None] * len(A)
+    ev = []                                        # (time, kind, request/stage): 0 = arrival, 1 = a server frees
+    for n in range(len(A)):
+        if routes[n]:
+            heapq.heappush(ev, (A[n], 0, n))
+        else:
+            dep[n] = A[n]
+
+    def dispatch(st, now):
+        while queue[st]:
+            k = min(range(stage_c[st]), key=lambda j: free[st][j])
+            if free[st][k] > now:
+                break
+            at, r = heapq.heappop(queue[st])
+            done = max(at, free[st][k]) + routes[r][pos[r]][1]
+            free[st][k] = done
+            heapq.heappush(ev, (done, 1, st))
+            pos[r] += 1
+            if pos[r] == len(routes[r]):
+                dep[r] = done
+            else:
+                heapq.heappush(ev, (done + edge_delay, 0, r))
+
+    while ev:
+        now, kind, x = heapq.heappop(ev)
+        if kind == 0:
+            st = routes[x][pos[x]][0]
+            heapq.heappush(queue[st], (now, x))
+            dispatch(st, now)
+        else:
+            dispatch(x, now)
+    return dep

@@ -202,9 +202,29 @@ void simulate(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate
       }
     int64_t x = A;
     bool first = true;
+    int64_t done[8]; /* R25: departure of the request from every stage it has visited so far */
+    bool visited[8] = {false, false, false, false, false, false, false, false};
+    int64_t last = A;
     for (uint32_t s = 0; s < V; ++s) { /* stages in the plan's order */
       const uint8_t m = smask[s] & tm;
       if (m == 0) continue;
+      if (g->join_mode) {
+        /* fork-join (Fig. 1: encoders feed the LLM): the request reaches stage s
+         * when every predecessor stage -- one holding a component u of the request with a DAG
+         * edge (u, v) into a component v of the request on stage s -- has finished, plus the
+         * transfer delay of that edge; with no predecessor, at its system arrival. */
+        x = A;
+        for (uint32_t sp = 0; sp < s; ++sp) {
+          if (!visited[sp]) continue;
+          bool feeds = false;
+          for (uint32_t e = 0; e < g->n_edges; ++e) {
+            const uint32_t u = g->edges[2 * e], v = g->edges[2 * e + 1];
+            if (((smask[sp] & tm) >> u) & 1 && ((m >> v) & 1)) feeds = true;
+          }
+          if (feeds) x = std::max(x, done[sp] + g->edge_delay_us);
+        }
+        first = true; /* the hop delay has been applied per edge above */
+      }
       int64_t S = 0, S_cpu = 0;
       for (uint32_t i = 0; i < C; ++i)
         if ((m >> i) & 1) { S += svc[i]; S_cpu += cpu[i]; }
@@ -217,9 +237,13 @@ void simulate(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate
        * GPU time alone" -- idle: the executor is free at the request's arrival (f <= x). */
       if (f <= x) x = x + S_cpu + S;
       else x = f + S;
+      done[s] = x;
+      visited[s] = true;
+      last = std::max(last, x);
       F[s][0] = x;
       std::sort(F[s].begin(), F[s].end());
     }
+    if (g->join_mode) x = last; /* R25: the request is done when its last branch is */
     out->cnt[t]++;
     if (x - A <= slo->L_us[t]) out->hits[t]++;
     out->dep_sum += (uint64_t)x;

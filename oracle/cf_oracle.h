@@ -58,6 +58,9 @@ typedef struct {
   int64_t edge_delay_us;       /* PAPER.md:322; added between consecutive visited stages   */
   const uint16_t* cpu_tab;     /* [C*T] table id of the CPU pre-processing time of (i, t), 0xffff = none;
                                   NULL = no component has any (R24) */
+  uint32_t join_mode;          /* 0: a request visits its stages one after another (R7); 1: fork-join along
+                                  the DAG edges (R25): a stage starts when all its predecessor
+                                  stages on the request's subgraph have finished */
 } orc_graph;
 
 /* P physical plans, each an ordered list of stages = (component bitmask, replica count). */

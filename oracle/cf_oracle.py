@@ -41,7 +41,8 @@ class _Graph(C.Structure):
                 ("type_thresh", C.POINTER(C.c_uint32)), ("svc_tab", C.POINTER(C.c_uint16)),
                 ("tabs", C.POINTER(_QTab)), ("n_tabs", C.c_uint32), ("arr_tab", _QTab),
                 ("edges", C.POINTER(C.c_uint8)), ("n_edges", C.c_uint32),
-                ("edge_delay_us", C.c_int64), ("cpu_tab", C.POINTER(C.c_uint16))]
+                ("edge_delay_us", C.c_int64), ("cpu_tab", C.POINTER(C.c_uint16)),
+                ("join_mode", C.c_uint32)]
 
 
 class _Plans(C.Structure):
@@ -96,7 +97,8 @@ class _Marshalled:
                         len(g.tabs), _QTab(g.arr_tab.levels, g.arr_tab.log2_cells,
                                            _ptr(g.arr_tab.q, C.c_int32)),
                         _ptr(edges if edges.size else None, C.c_uint8), edges.size // 2,
-                        int(g.edge_delay_us), _ptr(getattr(g, "cpu_tab", None), C.c_uint16))
+                        int(g.edge_delay_us), _ptr(getattr(g, "cpu_tab", None), C.c_uint16),
+                        int(getattr(g, "join_mode", 0)))
         self.pl = None
         if plans is not None:
             sm = np.ascontiguousarray(plans.stage_mask).reshape(-1)

@@ -120,6 +120,7 @@ int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* 
                        uint32_t* out_goodput_mrps) {
   if (int32_t rc = orc_validate(g, pl)) return rc;
   if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return ORC_ERR_ARG;
+  if (g->join_mode) return ORC_ERR_ARG; /* fork-join latency is a critical path, not a sum: not offered (R25) */
   const uint32_t C = g->n_comp, T = g->n_types, N = g->n_req, K = g->n_trials;
   const uint32_t key[2] = {(uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32)};
   for (uint32_t p = 0; p < pl->n_plans; ++p) {

@@ -82,6 +82,13 @@ typedef struct {
                                   finds the stage's earliest-free replica idle pays CPU + GPU time (svc_tab is
                                   the GPU time), a request that queued pays GPU time alone. Such graphs run on
                                   the 64-bit kernel and cannot be materialised as a stream (CF_ERR_ARG).    */
+  uint32_t join_mode;          /* 0: a request visits its stages one after another in the plan's order (R7).
+                                  1: fork-join along `edges` (R25; Fig. 1, encoders
+                                  feeding the LLM): a request reaches a stage when every predecessor stage --
+                                  one holding a component u of the request with an edge (u, v) into a
+                                  component v of the request on that stage -- has finished, plus
+                                  edge_delay_us; with no predecessor at its system arrival; it is done when
+                                  its last stage is. 64-bit kernel only; no stream; cf_mc_latency refuses.  */
 } cf_graph;
 
 /* P physical plans; plan p is an ORDERED list of n_stages[p] stages, stage s = (bitmask of the

@@ -72,6 +72,7 @@ int32_t check_graph(const cf_graph* g) {
   for (uint32_t j = 0; j < g->n_tabs; ++j)
     if (int32_t rc = check_tab(g->tabs[j])) return rc;
   if (int32_t rc = check_tab(g->arr_tab)) return rc;
+  if (g->join_mode > 1) return CF_ERR_ARG;
   if (g->edge_delay_us < 0 || g->edge_delay_us >= (1ll << 31)) return CF_ERR_RANGE;
   // DESIGN.md R17: a request's total service over all its components must fit int32
   int64_t worst = 0;
@@ -149,21 +150,23 @@ struct Schedule {
   // every stage of every plan has one replica: the call runs on the max-plus scan kernel (cf_scan.cuh)
   bool all_c1 = false;
   std::vector<uint32_t> plan_topo_v, plan_var_v;  // [P] topology id / stream variant of each plan
+  std::vector<uint8_t> topo_pred;                 // fork-join (R25): [topology][type 8][stage 8] predecessor masks
   uint32_t R = 1;
 };
 
-template <int W, bool HAS_CPU>
+template <int W, bool HAS_CPU, bool JOIN>
 uint32_t fixed_smem_w(int vmax, int cmax) {
   if (cmax <= 6) {
-    if (vmax <= 2) return SmemLayout<2, 6, W, HAS_CPU>::fixed_bytes;
-    if (vmax <= 6) return SmemLayout<6, 6, W, HAS_CPU>::fixed_bytes;
-    return SmemLayout<8, 6, W, HAS_CPU>::fixed_bytes;
+    if (vmax <= 2) return SmemLayout<2, 6, W, HAS_CPU, JOIN>::fixed_bytes;
+    if (vmax <= 6) return SmemLayout<6, 6, W, HAS_CPU, JOIN>::fixed_bytes;
+    return SmemLayout<8, 6, W, HAS_CPU, JOIN>::fixed_bytes;
   }
-  return SmemLayout<8, 8, W, HAS_CPU>::fixed_bytes;
+  return SmemLayout<8, 8, W, HAS_CPU, JOIN>::fixed_bytes;
 }
-uint32_t fixed_smem(int vmax, int cmax, int warps, bool has_cpu) {
-  if (has_cpu) return warps == 4 ? fixed_smem_w<4, true>(vmax, cmax) : fixed_smem_w<8, true>(vmax, cmax);
-  return warps == 4 ? fixed_smem_w<4, false>(vmax, cmax) : fixed_smem_w<8, false>(vmax, cmax);
+uint32_t fixed_smem(int vmax, int cmax, int warps, bool has_cpu, bool join) {
+  if (join) return warps == 4 ? fixed_smem_w<4, true, true>(vmax, cmax) : fixed_smem_w<8, true, true>(vmax, cmax);
+  if (has_cpu) return warps == 4 ? fixed_smem_w<4, true, false>(vmax, cmax) : fixed_smem_w<8, true, false>(vmax, cmax);
+  return warps == 4 ? fixed_smem_w<4, false, false>(vmax, cmax) : fixed_smem_w<8, false, false>(vmax, cmax);
 }
 
 template <int W, bool PW>
@@ -224,6 +227,21 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       plan_quads[p] += heap_quads(c);
     }
   }
+  if (g->join_mode) {  // R25: per (topology, type, stage) the visited stages that feed it along a DAG edge
+    sc.topo_pred.assign(sc.topos.size() * 64, 0);
+    for (size_t ti = 0; ti < sc.topos.size(); ++ti)
+      for (uint32_t t = 0; t < g->n_types; ++t)
+        for (uint32_t s = 0; s < sc.topos[ti].n_stages; ++s) {
+          const uint32_t ms = sc.topos[ti].mask[s] & g->type_mask[t];
+          uint8_t pm = 0;
+          for (uint32_t sp = 0; sp < s && ms; ++sp) {
+            const uint32_t mp = sc.topos[ti].mask[sp] & g->type_mask[t];
+            for (uint32_t e = 0; e < g->n_edges; ++e)
+              if (((mp >> g->edges[2 * e]) & 1u) && ((ms >> g->edges[2 * e + 1]) & 1u)) pm |= (uint8_t)(1u << sp);
+          }
+          sc.topo_pred[ti * 64 + t * 8 + s] = pm;
+        }
+  }
   sc.cmax = g->n_comp <= 6 ? 6 : 8;
   sc.R = R;
   sc.plan_topo_v = plan_topo;
@@ -235,7 +253,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   // thread per simulation when the call has few simulations (config 0: 32 per call), 5.7x slower
   // when there are enough to fill the GPU with threads (measured crossover near 9 000 simulations).
   if (!only_plan && (uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
-  if (graph_has_cpu(g)) sc.all_c1 = false;  // the idle/busy rule (R24) is not max-plus linear
+  if (graph_has_cpu(g) || g->join_mode) sc.all_c1 = false;  // the idle/busy rule (R24) is not max-plus linear; fork-join (R25) runs on the 64-bit kernel
   if (kernel_mode == CF_KERNEL_SCAN && !sc.all_c1) return CF_ERR_ARG;  // one replica everywhere, <= 8192 simulations
   // the forced thread-per-simulation modes (cf_debug.h) keep that path; so do traces unless asked otherwise
   if (kernel_mode == CF_KERNEL_WIDE64 || kernel_mode == CF_KERNEL_FAST32) sc.all_c1 = false;
@@ -250,7 +268,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   const bool pw = streamed;
   sc.warps_per_cta = (R >= 8 && !pw) ? 8 : 4;
   const uint32_t kWarpsPerCta = (uint32_t)sc.warps_per_cta;
-  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax, sc.warps_per_cta, graph_has_cpu(g)),
+  const uint32_t fixed_w = fixed_smem(sc.vmax, sc.cmax, sc.warps_per_cta, graph_has_cpu(g), g->join_mode != 0),
                  fixed_f = fixed_smem32(sc.vmax32, sc.cmax, sc.warps_per_cta, pw);
   const uint32_t fixed = fast ? fixed_f : fixed_w;  // the layout that is packed for occupancy
 
@@ -488,12 +506,13 @@ size_t fill_graph_params(const cf_graph* g, const cf_slo* slo, uint64_t seed, Bl
         }
       }
   kp->edge_delay = g->edge_delay_us;
+  kp->join = g->join_mode ? 1u : 0u;
   kp->seed_lo = (uint32_t)seed;
   kp->seed_hi = (uint32_t)(seed >> 32);
   return blob->add(pool.data(), pool.size() * sizeof(int32_t));
 }
 
-struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c, plan_topo, plan_var; };
+struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c, plan_topo, plan_var, topo_pred; };
 
 SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
   SchedOffsets o;
@@ -504,6 +523,7 @@ SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
   o.plan_c = blob->add(sc.plan_c.data(), sc.plan_c.size() * sizeof(uint16_t));
   o.plan_topo = blob->add(sc.plan_topo_v.data(), sc.plan_topo_v.size() * sizeof(uint32_t));
   o.plan_var = blob->add(sc.plan_var_v.data(), sc.plan_var_v.size() * sizeof(uint32_t));
+  o.topo_pred = blob->add(sc.topo_pred.data(), sc.topo_pred.size());
   return o;
 }
 
@@ -516,6 +536,7 @@ void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool
   kp->plan_c = reinterpret_cast<const uint16_t*>(ws + o.plan_c);
   kp->plan_topo = reinterpret_cast<const uint32_t*>(ws + o.plan_topo);
   kp->plan_var = reinterpret_cast<const uint32_t*>(ws + o.plan_var);
+  kp->topo_pred = ws + o.topo_pred;
   kp->status = reinterpret_cast<int32_t*>(ws);
 }
 
@@ -567,7 +588,7 @@ cudaError_t launch_sims32(KParams kp, const Schedule& sc, uint32_t n_trials, cud
 // at 2^30. Anything else runs on the 64-bit kernel alone.
 bool fast_path_ok(const cf_graph* g, uint32_t kernel_mode) {
   if (kernel_mode == CF_KERNEL_WIDE64) return false;
-  if (graph_has_cpu(g)) return false;  // CPU-GPU overlap (R24) runs on the 64-bit kernel
+  if (graph_has_cpu(g) || g->join_mode) return false;  // CPU-GPU overlap (R24) and fork-join (R25) run on the 64-bit kernel
   int64_t worst = 0;
   for (uint32_t i = 0; i < g->n_comp; ++i) {
     int64_t mx = 0;
@@ -929,6 +950,7 @@ struct KeyBuilder {
     for (uint32_t j = 0; j < g->n_tabs; ++j) tab(g->tabs[j]);
     tab(g->arr_tab);
     if (g->n_edges) put(g->edges, 2 * g->n_edges);
+    val(g->join_mode);
     val((uint32_t)(g->cpu_tab != nullptr));
     if (g->cpu_tab) put(g->cpu_tab, (size_t)g->n_comp * g->n_types * 2);
   }
@@ -982,7 +1004,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_graph(a.g)) return rc;
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g))) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   KeyBuilder kb;
   kb.val((uint32_t)1); kb.graph(a.g); kb.plans(a.pl); kb.val(a.R); kb.val(a.seed); kb.put(a.slo->L_us, a.g->n_types * 8);
@@ -1034,7 +1056,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rate_hi_dev || !a.slo || !a.slo->L_us || !a.slo->att_num || !a.slo->att_den || !a.out_rate || !a.out_goodput)
     return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g))) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
   KeyBuilder kb;
@@ -1144,7 +1166,7 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   const size_t max_warps = P * R / 32 + P + 1;
   n += align_up(max_warps * sizeof(WarpDesc));
   n += align_up(max_warps * sizeof(CtaDesc));
-  n += align_up(P * 8 * 2) + 2 * align_up(P * 4);
+  n += align_up(P * 8 * 2) + 2 * align_up(P * 4) + align_up(P * 64);  // plan_c, plan_topo / plan_var, topo_pred
   n += 4 * kAlign + 3 * align_up(P * 4) + align_up(P * Rb * 4);  // bisection: att, lo/hi, probes, tree
   n += align_up(P * Rb * K * T * 2 * 4) + align_up(P * K * T * 2 * 4) + kAlign;  // probe + at_lo counts
   n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch
@@ -1538,6 +1560,7 @@ int32_t cf_mc_latency(const cf_graph* g, const cf_plans* pl, const uint32_t* rat
   if (int32_t rc = check_graph(g)) return rc;
   if (int32_t rc = check_plans(g, pl)) return rc;
   if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return CF_ERR_ARG;
+  if (g->join_mode) return CF_ERR_ARG;  // fork-join latency is a critical path, not a sum (R25)
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   AuxSetup a;
   if (int32_t rc = aux_setup(g, pl, slo, seed, variant, workspace, workspace_bytes, st, &a)) return rc;

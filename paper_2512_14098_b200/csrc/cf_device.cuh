@@ -100,6 +100,8 @@ struct KParams {
   uint8_t* tr_type;
   uint32_t tr_plan;        // the traced plan (scan kernel: the warp whose simulation is written out)
   uint32_t has_cpu;        // some (component, type) has a CPU pre-processing table (R24): 64-bit kernel only
+  uint32_t join;           // fork-join routing along the DAG edges (R25): 64-bit kernel only
+  const uint8_t* topo_pred;  // join: [topology][type 8][stage 8] bitmask of the stage's predecessor stages
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -160,10 +162,11 @@ struct CompRec {
 
 // Stage-level record a warp builds for its topology: cu (absolute) | type<<56, then S[s] per stage
 // (-1 = stage not visited by this request's type).
-template <int VMAX, bool HAS_CPU = false>
+template <int VMAX, bool HAS_CPU = false, bool JOIN = false>
 struct StageRec {
   static constexpr int kBase = (VMAX <= 2) ? 1 : (VMAX <= 6 ? 2 : 3);
-  static constexpr int kWords = kBase + (HAS_CPU ? (VMAX <= 4 ? 1 : 2) : 0);  // + summed CPU time per stage
+  static constexpr int kCpu = HAS_CPU ? (VMAX <= 4 ? 1 : 2) : 0;  // + summed CPU time per stage
+  static constexpr int kWords = kBase + kCpu + (JOIN ? 1 : 0);    // + predecessor masks of the stages (R25)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -312,10 +315,10 @@ __device__ __forceinline__ void heap_replace_min(uint8_t* smem, int64_t& root, u
 // The simulation kernel. grid = (CTAs of this launch, K trials); block = kThreads.
 // Dynamic shared memory: [tiles 2 x kTile x CompRec][chunk totals][cnt][L][warp stage buffers][heaps]
 // ------------------------------------------------------------------------------------------------
-template <int VMAX, int CMAX, int WARPS, bool HAS_CPU = false>
+template <int VMAX, int CMAX, int WARPS, bool HAS_CPU = false, bool JOIN = false>
 struct SmemLayout {
   static constexpr uint32_t kCompRecBytes = CompRec<CMAX, HAS_CPU>::kWords * 16;
-  static constexpr uint32_t kStageRecBytes = StageRec<VMAX, HAS_CPU>::kWords * 16;
+  static constexpr uint32_t kStageRecBytes = StageRec<VMAX, HAS_CPU, JOIN>::kWords * 16;
   static constexpr uint32_t tiles = 0;
   static constexpr uint32_t totals = tiles + 2 * kTile * kCompRecBytes;
   static constexpr uint32_t cnt = totals + 2 * kChunks * 8;
@@ -327,11 +330,13 @@ struct SmemLayout {
 
 // HAS_CPU: the CPU-GPU overlap rule of PAPER.md:318-320 (R24): a request that finds the earliest-free
 // replica idle pays its CPU pre-processing time on top of the GPU time, a queued one GPU time alone
-template <int VMAX, int CMAX, bool HAS_DELAY, int WARPS, bool HAS_CPU = false>
+// JOIN: fork-join routing (R25): a request reaches a stage when all its predecessor stages have
+// finished (+ the edge delay each), and is done when its last branch is
+template <int VMAX, int CMAX, bool HAS_DELAY, int WARPS, bool HAS_CPU = false, bool JOIN = false>
 __global__ void __launch_bounds__(WARPS * 32)
 cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
-  using SL = SmemLayout<VMAX, CMAX, WARPS, HAS_CPU>;
-  constexpr int kCW = CompRec<CMAX, HAS_CPU>::kWords, kSW = StageRec<VMAX, HAS_CPU>::kWords;
+  using SL = SmemLayout<VMAX, CMAX, WARPS, HAS_CPU, JOIN>;
+  constexpr int kCW = CompRec<CMAX, HAS_CPU>::kWords, kSW = StageRec<VMAX, HAS_CPU, JOIN>::kWords;
   extern __shared__ __align__(16) uint8_t smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t trial = prm.trial_base + blockIdx.x % prm.k_launch;
@@ -482,6 +487,10 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
             Sc[s] = accc;
           }
           uint4* dst = wbuf + lane * kSW;
+          if (JOIN) {  // the predecessor masks of this topology's stages for the request's type
+            const uint2 pm = *reinterpret_cast<const uint2*>(prm.topo_pred + ((size_t)wd.topo * 8 + t) * 8);
+            dst[StageRec<VMAX, HAS_CPU, JOIN>::kBase + StageRec<VMAX, HAS_CPU, JOIN>::kCpu] = make_uint4(pm.x, pm.y, 0u, 0u);
+          }
           if (HAS_CPU) {
             constexpr int kB = StageRec<VMAX, HAS_CPU>::kBase;
             dst[kB] = make_uint4((uint32_t)Sc[0], (uint32_t)Sc[VMAX > 1 ? 1 : 0], (uint32_t)Sc[VMAX > 2 ? 2 : 0],
@@ -546,17 +555,31 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
           const int64_t A = (int64_t)((cu * (uint64_t)period + 32768ull) >> 16);
           int64_t x = A;
           bool first = true;
+          int64_t xs[VMAX], last = A;  // JOIN: departures of the visited stages so far
+          uint64_t pmask = 0;
+          if (JOIN) {
+            const uint4 pw = rp[StageRec<VMAX, HAS_CPU, JOIN>::kBase + StageRec<VMAX, HAS_CPU, JOIN>::kCpu];
+            pmask = ((uint64_t)pw.y << 32) | pw.x;
+          }
 #pragma unroll
           for (int s = 0; s < VMAX; ++s) {
             if (S[s] >= 0) {
-              if (HAS_DELAY) { if (!first) x += delay; first = false; }
+              if (JOIN) {
+                x = A;
+                const uint32_t pm = (uint32_t)(pmask >> (8 * s)) & 0xffu;
+#pragma unroll
+                for (int sp = 0; sp < s; ++sp)
+                  if ((pm >> sp) & 1u) { const int64_t a = xs[sp] + delay; x = a > x ? a : x; }
+              } else if (HAS_DELAY) { if (!first) x += delay; first = false; }
               const int64_t f = root[s];
               if (HAS_CPU) x = (f <= x) ? x + (int64_t)Sc[s] : f;  // idle: CPU + GPU; queued: GPU alone (R24)
               else x = x > f ? x : f;                              // a5/a6: start at max(arrival, earliest free)
               x += (int64_t)S[s];
               heap_replace_min(smem, root[s], hb[s], sim_c[s], x);
+              if (JOIN) { xs[s] = x; last = x > last ? x : last; }
             }
           }
+          if (JOIN) x = last;
           // a8
           const bool hit = (x - A) <= L_s[t];
           hp += (uint64_t)(hit ? 1u : 0u) << (t * 8u);

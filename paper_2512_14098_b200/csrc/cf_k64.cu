@@ -6,9 +6,9 @@ namespace {
 
 constexpr uint32_t kMaxSmem = 227u * 1024u;
 
-template <int VMAX, int CMAX, bool HAS_DELAY, int W, bool HAS_CPU = false>
+template <int VMAX, int CMAX, bool HAS_DELAY, int W, bool HAS_CPU = false, bool JOIN = false>
 cudaError_t launch_one(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) {
-  auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY, W, HAS_CPU>;
+  auto kern = cf_sim_kernel<VMAX, CMAX, HAS_DELAY, W, HAS_CPU, JOIN>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
   if (e != cudaSuccess) return e;
   kern<<<lc.blocks, W * 32, lc.smem_bytes, st>>>(kp, 0u);
@@ -18,6 +18,10 @@ cudaError_t launch_one(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) 
 template <int VMAX, int CMAX>
 cudaError_t launch_v(const KParams& kp, const LaunchCfg& lc, cudaStream_t st) {
   const bool d = kp.edge_delay != 0;
+  if (kp.join) {  // fork-join routing (R25): the CPU variant covers graphs without CPU tables (times of 0)
+    if (lc.warps_per_cta == 4) return launch_one<VMAX, CMAX, true, 4, true, true>(kp, lc, st);
+    return launch_one<VMAX, CMAX, true, 8, true, true>(kp, lc, st);
+  }
   if (kp.has_cpu) {  // CPU-GPU overlap (R24): the delay variant covers delay 0 as well
     if (lc.warps_per_cta == 4) return launch_one<VMAX, CMAX, true, 4, true>(kp, lc, st);
     return launch_one<VMAX, CMAX, true, 8, true>(kp, lc, st);

@@ -121,7 +121,40 @@ int32_t validate(const orc_graph* g, const orc_plans* pl) {
   if (!pl->n_stages || !pl->stage_mask || !pl->stage_c) return ORC_ERR_ARG;
   uint8_t used = 0;
   for (uint32_t t = 0; t < T; ++t) used |= g->type_mask[t];
-  for (uint32_t p = 0; p < pl->n_plans; ++p) {
+  if (pl->max_routes > 4 || (pl->max_routes > 0 && (!pl->route_mask || !pl->route_cum))) return ORC_ERR_ARG;
+  for (uint32_t p = 0; p < pl->n_plans && pl->max_routes > 0; ++p) { /* R26: plans with routing */
+    const uint32_t V = pl->n_stages[p], MR = pl->max_routes;
+    if (V < 1 || V > pl->max_stages) return ORC_ERR_PLAN;
+    uint8_t all = 0;
+    for (uint32_t s = 0; s < V; ++s) {
+      const uint8_t m = pl->stage_mask[p * pl->max_stages + s];
+      if (m == 0 || (m >> C) || pl->stage_c[p * pl->max_stages + s] < 1) return ORC_ERR_PLAN;
+      all |= m;
+    }
+    if (used & ~all) return ORC_ERR_PLAN;
+    for (uint32_t t = 0; t < T; ++t)
+      for (uint32_t r = 0; r < MR; ++r) {
+        const size_t at = ((size_t)p * T + t) * MR + r;
+        if (r > 0 && pl->route_cum[at] < pl->route_cum[at - 1]) return ORC_ERR_PLAN;
+        uint8_t seen = 0;
+        int stage_of[8];
+        for (int i = 0; i < 8; ++i) stage_of[i] = -1;
+        for (uint32_t s = 0; s < V; ++s) {
+          if (!((pl->route_mask[at] >> s) & 1)) continue;
+          const uint8_t m = pl->stage_mask[p * pl->max_stages + s] & g->type_mask[t];
+          if (m & seen) return ORC_ERR_PLAN; /* a component served twice along the route */
+          seen |= m;
+          for (uint32_t i = 0; i < C; ++i)
+            if ((m >> i) & 1) stage_of[i] = (int)s;
+        }
+        if (seen != g->type_mask[t]) return ORC_ERR_PLAN; /* the route misses a component of the type */
+        for (uint32_t e = 0; e < g->n_edges; ++e) {
+          int su = stage_of[g->edges[2 * e]], sv = stage_of[g->edges[2 * e + 1]];
+          if (su >= 0 && sv >= 0 && su > sv) return ORC_ERR_PLAN;
+        }
+      }
+  }
+  for (uint32_t p = 0; p < pl->n_plans && pl->max_routes == 0; ++p) {
     uint32_t V = pl->n_stages[p];
     if (V < 1 || V > pl->max_stages) return ORC_ERR_PLAN;
     uint8_t seen = 0;
@@ -188,6 +221,14 @@ void simulate(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate
     for (uint32_t tt = 0; tt < T; ++tt)
       if (b0[1] < g->type_thresh[tt]) { t = tt; break; }
     const uint8_t tm = g->type_mask[t];
+    uint8_t route = 0xff; /* R26: the stages this request may visit */
+    if (pl->max_routes > 0) {
+      const uint32_t MR = pl->max_routes;
+      uint32_t r = MR - 1;
+      for (uint32_t rr = 0; rr < MR; ++rr)
+        if (b0[2] < pl->route_cum[((size_t)p * T + t) * MR + rr]) { r = rr; break; }
+      route = pl->route_mask[((size_t)p * T + t) * MR + r];
+    }
     int64_t svc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int64_t cpu[8] = {0, 0, 0, 0, 0, 0, 0, 0}; /* R24: CPU pre-processing time, paid only at an idle executor */
     for (uint32_t i = 0; i < C; ++i)
@@ -207,7 +248,7 @@ void simulate(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate
     int64_t last = A;
     for (uint32_t s = 0; s < V; ++s) { /* stages in the plan's order */
       const uint8_t m = smask[s] & tm;
-      if (m == 0) continue;
+      if (m == 0 || !((route >> s) & 1)) continue;
       if (g->join_mode) {
         /* fork-join (Fig. 1: encoders feed the LLM): the request reaches stage s
          * when every predecessor stage -- one holding a component u of the request with a DAG

@@ -69,6 +69,15 @@ typedef struct {
   const uint8_t* n_stages;    /* [P] */
   const uint8_t* stage_mask;  /* [P*max_stages] */
   const uint16_t* stage_c;    /* [P*max_stages] */
+  /* Routing between alternative paths (R26). max_routes == 0: none, a
+   * request visits every stage that holds one of its components. Else 1..4 routes per (plan,
+   * type): the request draws a route with the cumulative probabilities route_cum (Q32, the last
+   * route takes the rest) and visits the stages of route_mask (a bitmask over the plan's stages)
+   * that hold one of its components. Stage masks may then overlap across stages; along every
+   * route they must cover the type's components exactly once. */
+  uint32_t max_routes;
+  const uint8_t* route_mask;  /* [P*T*max_routes] */
+  const uint32_t* route_cum;  /* [P*T*max_routes] */
 } orc_plans;
 
 typedef struct {

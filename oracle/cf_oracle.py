@@ -48,7 +48,8 @@ class _Graph(C.Structure):
 class _Plans(C.Structure):
     _fields_ = [("n_plans", C.c_uint32), ("max_stages", C.c_uint32),
                 ("n_stages", C.POINTER(C.c_uint8)), ("stage_mask", C.POINTER(C.c_uint8)),
-                ("stage_c", C.POINTER(C.c_uint16))]
+                ("stage_c", C.POINTER(C.c_uint16)), ("max_routes", C.c_uint32),
+                ("route_mask", C.POINTER(C.c_uint8)), ("route_cum", C.POINTER(C.c_uint32))]
 
 
 class _Slo(C.Structure):
@@ -104,8 +105,15 @@ class _Marshalled:
             sm = np.ascontiguousarray(plans.stage_mask).reshape(-1)
             sc = np.ascontiguousarray(plans.stage_c).reshape(-1)
             self.keep += [sm, sc]
+            rm = getattr(plans, "route_mask", None)
+            rc = getattr(plans, "route_cum", None)
+            if rm is not None:
+                rm = np.ascontiguousarray(rm, dtype=np.uint8).reshape(-1)
+                rc = np.ascontiguousarray(rc, dtype=np.uint32).reshape(-1)
+                self.keep += [rm, rc]
             self.pl = _Plans(plans.n_plans, plans.max_stages, _ptr(plans.n_stages, C.c_uint8),
-                             _ptr(sm, C.c_uint8), _ptr(sc, C.c_uint16))
+                             _ptr(sm, C.c_uint8), _ptr(sc, C.c_uint16), int(getattr(plans, "max_routes", 0)),
+                             _ptr(rm, C.c_uint8), _ptr(rc, C.c_uint32))
         self.slo = None
         if slo is not None:
             self.slo = _Slo(_ptr(slo.L_us, C.c_int64), _ptr(slo.att_num, C.c_uint32),

@@ -48,6 +48,36 @@ uint64_t stage_demand_q16(const orc_graph* g, uint8_t mask) {
   return (uint64_t)(D >> 32);
 }
 
+/* R26: with routing, type t loads stage s of plan p only on the routes that include it:
+ * D = floor( sum_t sum_r floor(w_t * q_{t,r} / 2^32) * sum_{i in mask & M_t} mean_q16(i,t) / 2^32 ),
+ * q_{t,r} the route's probability in Q32 (the last route takes the rest). */
+uint64_t routed_stage_demand_q16(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t s) {
+  const uint32_t T = g->n_types, MR = pl->max_routes;
+  const uint8_t mask = pl->stage_mask[p * pl->max_stages + s];
+  u128 D = 0;
+  for (uint32_t t = 0; t < T; ++t) {
+    uint64_t mu = 0;
+    for (uint32_t i = 0; i < g->n_comp; ++i)
+      if (((mask & g->type_mask[t]) >> i) & 1)
+        mu += orc_qtab_mean_q16(&g->tabs[g->svc_tab[i * T + t]]);
+    for (uint32_t r = 0; r < MR; ++r) {
+      const size_t at = ((size_t)p * T + t) * MR + r;
+      if (!((pl->route_mask[at] >> s) & 1)) continue;
+      const uint64_t hi = (r + 1 == MR) ? (1ull << 32) : (uint64_t)pl->route_cum[at];
+      const uint64_t lo = (r == 0) ? 0ull : (uint64_t)pl->route_cum[at - 1];
+      const uint64_t q = hi > lo ? hi - lo : 0ull;
+      const uint64_t pr = (uint64_t)(((u128)type_weight_q32(g, t) * q) >> 32);
+      D += (u128)pr * mu;
+    }
+  }
+  return (uint64_t)(D >> 32);
+}
+
+uint64_t demand_of(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t s) {
+  return pl->max_routes ? routed_stage_demand_q16(g, pl, p, s)
+                        : stage_demand_q16(g, pl->stage_mask[p * pl->max_stages + s]);
+}
+
 /* Rate (milli-requests/s) at which c replicas saturate under demand Dq (Q16 us per request):
  * c / (Dq / 65536 us) requests per us = c * 65536 * 1e9 / Dq milli-requests per second. */
 uint64_t saturation_mrps(uint64_t c, uint64_t Dq) { return c * 65536ull * 1000000000ull / Dq; }
@@ -89,7 +119,7 @@ int32_t orc_flow_bound(const orc_graph* g, const orc_plans* pl, uint32_t alpha_n
     uint64_t R = UINT64_MAX;
     uint8_t bott = 0xff;
     for (uint32_t s = 0; s < V; ++s) {
-      const uint64_t Dq = stage_demand_q16(g, pl->stage_mask[p * pl->max_stages + s]);
+      const uint64_t Dq = demand_of(g, pl, p, s);
       if (Dq == 0) continue; /* nothing flows through this node */
       const uint64_t r = saturation_mrps(pl->stage_c[p * pl->max_stages + s], Dq);
       if (r < R) { R = r; bott = (uint8_t)s; } /* the node whose demand first reaches capacity */
@@ -98,7 +128,7 @@ int32_t orc_flow_bound(const orc_graph* g, const orc_plans* pl, uint32_t alpha_n
     for (uint32_t s = 0; s < V; ++s) {
       const uint64_t c = pl->stage_c[p * pl->max_stages + s];
       if (c < 2) continue;
-      const uint64_t Dq = stage_demand_q16(g, pl->stage_mask[p * pl->max_stages + s]);
+      const uint64_t Dq = demand_of(g, pl, p, s);
       if (Dq == 0 || saturation_mrps(c - 1, Dq) >= R) redundant = true;
     }
     const uint64_t bound = std::min<uint64_t>(R, RATE_MAX);
@@ -121,6 +151,7 @@ int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* 
   if (int32_t rc = orc_validate(g, pl)) return rc;
   if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return ORC_ERR_ARG;
   if (g->join_mode) return ORC_ERR_ARG; /* fork-join latency is a critical path, not a sum: not offered (R25) */
+  if (pl->max_routes) return ORC_ERR_ARG; /* routed plans: not offered (R26) */
   const uint32_t C = g->n_comp, T = g->n_types, N = g->n_req, K = g->n_trials;
   const uint32_t key[2] = {(uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32)};
   for (uint32_t p = 0; p < pl->n_plans; ++p) {

@@ -67,8 +67,14 @@ class Plans:
     n_stages: np.ndarray    # uint8 [P]
     stage_mask: np.ndarray  # uint8 [P, max_stages]
     stage_c: np.ndarray     # uint16 [P, max_stages]
+    max_routes: int = 0                        # R26: 0 = no routing, else 1..4 routes per (plan, type)
+    route_mask: Optional[np.ndarray] = None    # uint8 [P, T, max_routes] bitmask over the plan's stages
+    route_cum: Optional[np.ndarray] = None     # uint32 [P, T, max_routes] cumulative probability, Q32
 
     def __post_init__(self):
+        if self.route_mask is not None:
+            self.route_mask = np.ascontiguousarray(self.route_mask, dtype=np.uint8)
+            self.route_cum = np.ascontiguousarray(self.route_cum, dtype=np.uint32)
         self.n_stages = np.ascontiguousarray(self.n_stages, dtype=np.uint8)
         self.stage_mask = np.ascontiguousarray(self.stage_mask, dtype=np.uint8)
         self.stage_c = np.ascontiguousarray(self.stage_c, dtype=np.uint16)
@@ -85,7 +91,10 @@ class Plans:
 
     def subset(self, idx) -> "Plans":
         idx = np.asarray(idx)
-        return Plans(self.n_stages[idx], self.stage_mask[idx], self.stage_c[idx])
+        if self.route_mask is None:
+            return Plans(self.n_stages[idx], self.stage_mask[idx], self.stage_c[idx])
+        return Plans(self.n_stages[idx], self.stage_mask[idx], self.stage_c[idx], self.max_routes,
+                     self.route_mask[idx], self.route_cum[idx])
 
 
 @dataclasses.dataclass

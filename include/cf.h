@@ -99,6 +99,17 @@ typedef struct {
   const uint8_t* n_stages;      /* [P] */
   const uint8_t* stage_mask;    /* [P*max_stages] */
   const uint16_t* stage_c;      /* [P*max_stages] */
+  /* Routing between alternative paths ("routing probabilities ... between alternative
+   * parallel paths in the logical plan"; R26). max_routes = 0 (and NULL pointers): none.
+   * Else 1..4 routes per (plan, type): a request of type t draws route r with the cumulative
+   * probabilities route_cum (Q32, non-decreasing; the last route takes the rest; Philox block 0,
+   * word 2) and visits the stages of bitmask route_mask (bit s = stage s) that hold one of its
+   * components. Stage masks may then overlap across stages; along every route they must serve
+   * each component of the type exactly once, in an order the DAG allows. Routed plans cannot be
+   * evaluated on a materialised stream, and cf_mc_latency refuses them (CF_ERR_ARG). */
+  uint32_t max_routes;
+  const uint8_t* route_mask;    /* [P*T*max_routes] */
+  const uint32_t* route_cum;    /* [P*T*max_routes] */
 } cf_plans;
 
 /* Per-type latency targets L_t and the attainment target used by the rate

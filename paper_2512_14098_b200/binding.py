@@ -55,7 +55,8 @@ class cf_graph(C.Structure):
 class cf_plans(C.Structure):
     _fields_ = [("n_plans", C.c_uint32), ("max_stages", C.c_uint32),
                 ("n_stages", C.POINTER(C.c_uint8)), ("stage_mask", C.POINTER(C.c_uint8)),
-                ("stage_c", C.POINTER(C.c_uint16))]
+                ("stage_c", C.POINTER(C.c_uint16)), ("max_routes", C.c_uint32),
+                ("route_mask", C.POINTER(C.c_uint8)), ("route_cum", C.POINTER(C.c_uint32))]
 
 
 class cf_options(C.Structure):
@@ -151,8 +152,15 @@ class Marshalled:
             sm = np.ascontiguousarray(plans.stage_mask).reshape(-1)
             sc = np.ascontiguousarray(plans.stage_c).reshape(-1)
             self.keep += [sm, sc]
+            rm = getattr(plans, "route_mask", None)
+            rcum = getattr(plans, "route_cum", None)
+            if rm is not None:
+                rm = np.ascontiguousarray(rm, dtype=np.uint8).reshape(-1)
+                rcum = np.ascontiguousarray(rcum, dtype=np.uint32).reshape(-1)
+                self.keep += [rm, rcum]
             self.pl = cf_plans(plans.n_plans, plans.max_stages, _hp(plans.n_stages, C.c_uint8),
-                               _hp(sm, C.c_uint8), _hp(sc, C.c_uint16))
+                               _hp(sm, C.c_uint8), _hp(sc, C.c_uint16), int(getattr(plans, "max_routes", 0)),
+                               _hp(rm, C.c_uint8), _hp(rcum, C.c_uint32))
         self.slo = None
         if slo is not None:
             self.slo = cf_slo(_hp(slo.L_us, C.c_int64), _hp(slo.att_num, C.c_uint32),

@@ -109,6 +109,44 @@ int32_t check_plans(const cf_graph* g, const cf_plans* pl) {
   if (!pl->n_stages || !pl->stage_mask || !pl->stage_c) return CF_ERR_ARG;
   uint32_t used = 0;
   for (uint32_t t = 0; t < g->n_types; ++t) used |= g->type_mask[t];
+  if (pl->max_routes > 4 || (pl->max_routes && (!pl->route_mask || !pl->route_cum))) return CF_ERR_ARG;
+  if (pl->max_routes) {  // R26: masks may overlap across stages; every route serves each component of its type once
+    const uint32_t MR = pl->max_routes, T = g->n_types;
+    for (uint32_t p = 0; p < pl->n_plans; ++p) {
+      const uint32_t V = pl->n_stages[p];
+      if (V < 1 || V > pl->max_stages) return CF_ERR_PLAN;
+      uint32_t all = 0;
+      for (uint32_t s = 0; s < V; ++s) {
+        const uint32_t m = pl->stage_mask[p * pl->max_stages + s];
+        if (!m || (m >> g->n_comp) || pl->stage_c[p * pl->max_stages + s] < 1) return CF_ERR_PLAN;
+        all |= m;
+      }
+      if (used & ~all) return CF_ERR_PLAN;
+      for (uint32_t t = 0; t < T; ++t) {
+        const uint8_t* rm = pl->route_mask + ((size_t)p * T + t) * MR;
+        const uint32_t* rc = pl->route_cum + ((size_t)p * T + t) * MR;
+        for (uint32_t r = 0; r < MR; ++r) {
+          if (r && rc[r] < rc[r - 1]) return CF_ERR_PLAN;
+          uint32_t got = 0;
+          int where[8] = {-1, -1, -1, -1, -1, -1, -1, -1};
+          for (uint32_t s = 0; s < V; ++s) {
+            if (!((rm[r] >> s) & 1)) continue;
+            const uint32_t m = pl->stage_mask[p * pl->max_stages + s] & g->type_mask[t];
+            if (m & got) return CF_ERR_PLAN;
+            got |= m;
+            for (uint32_t i = 0; i < g->n_comp; ++i)
+              if ((m >> i) & 1) where[i] = (int)s;
+          }
+          if (got != g->type_mask[t]) return CF_ERR_PLAN;
+          for (uint32_t e = 0; e < g->n_edges; ++e) {
+            const int a = where[g->edges[2 * e]], b = where[g->edges[2 * e + 1]];
+            if (a >= 0 && b >= 0 && a > b) return CF_ERR_PLAN;
+          }
+        }
+      }
+    }
+    return CF_OK;
+  }
   for (uint32_t p = 0; p < pl->n_plans; ++p) {
     const uint32_t V = pl->n_stages[p];
     if (V < 1 || V > pl->max_stages) return CF_ERR_PLAN;
@@ -151,6 +189,7 @@ struct Schedule {
   bool all_c1 = false;
   std::vector<uint32_t> plan_topo_v, plan_var_v;  // [P] topology id / stream variant of each plan
   std::vector<uint8_t> topo_pred;                 // fork-join (R25): [topology][type 8][stage 8] predecessor masks
+  std::vector<TopoRoutes> topo_routes;            // routing (R26): [topology]
   uint32_t R = 1;
 };
 
@@ -210,6 +249,13 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
     const uint32_t V = pl->n_stages[p];
     maxV = std::max(maxV, V);
     std::vector<uint8_t> key(pl->stage_mask + (size_t)p * MS, pl->stage_mask + (size_t)p * MS + V);
+    if (pl->max_routes) {  // R26: plans share a topology only if they route alike
+      const size_t nr = (size_t)g->n_types * pl->max_routes;
+      key.push_back(0xfe);
+      key.insert(key.end(), pl->route_mask + (size_t)p * nr, pl->route_mask + (size_t)(p + 1) * nr);
+      const uint8_t* cb = reinterpret_cast<const uint8_t*>(pl->route_cum + (size_t)p * nr);
+      key.insert(key.end(), cb, cb + nr * 4);
+    }
     auto it = topo_id.find(key);
     if (it == topo_id.end()) {
       TopoDesc td;
@@ -218,6 +264,16 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
       for (uint32_t s = 0; s < V; ++s) td.mask[s] = key[s];
       it = topo_id.emplace(key, (uint32_t)sc.topos.size()).first;
       sc.topos.push_back(td);
+      if (pl->max_routes) {
+        TopoRoutes tr;
+        std::memset(&tr, 0, sizeof(tr));
+        for (uint32_t t = 0; t < g->n_types; ++t)
+          for (uint32_t r = 0; r < pl->max_routes; ++r) {
+            tr.cum[t][r] = pl->route_cum[((size_t)p * g->n_types + t) * pl->max_routes + r];
+            tr.mask[t][r] = pl->route_mask[((size_t)p * g->n_types + t) * pl->max_routes + r];
+          }
+        sc.topo_routes.push_back(tr);
+      }
     }
     plan_topo[p] = it->second;
     for (uint32_t s = 0; s < V; ++s) {
@@ -242,7 +298,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
           sc.topo_pred[ti * 64 + t * 8 + s] = pm;
         }
   }
-  sc.cmax = g->n_comp <= 6 ? 6 : 8;
+  sc.cmax = (g->n_comp <= 6 && !pl->max_routes) ? 6 : 8;  // routed calls carry the route draw in the 3-word record
   sc.R = R;
   sc.plan_topo_v = plan_topo;
   sc.all_c1 = true;
@@ -253,7 +309,7 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   // thread per simulation when the call has few simulations (config 0: 32 per call), 5.7x slower
   // when there are enough to fill the GPU with threads (measured crossover near 9 000 simulations).
   if (!only_plan && (uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
-  if (graph_has_cpu(g) || g->join_mode) sc.all_c1 = false;  // the idle/busy rule (R24) is not max-plus linear; fork-join (R25) runs on the 64-bit kernel
+  if (graph_has_cpu(g) || g->join_mode || pl->max_routes) sc.all_c1 = false;  // the idle/busy rule (R24) is not max-plus linear; fork-join (R25) runs on the 64-bit kernel
   if (kernel_mode == CF_KERNEL_SCAN && !sc.all_c1) return CF_ERR_ARG;  // one replica everywhere, <= 8192 simulations
   // the forced thread-per-simulation modes (cf_debug.h) keep that path; so do traces unless asked otherwise
   if (kernel_mode == CF_KERNEL_WIDE64 || kernel_mode == CF_KERNEL_FAST32) sc.all_c1 = false;
@@ -512,7 +568,7 @@ size_t fill_graph_params(const cf_graph* g, const cf_slo* slo, uint64_t seed, Bl
   return blob->add(pool.data(), pool.size() * sizeof(int32_t));
 }
 
-struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c, plan_topo, plan_var, topo_pred; };
+struct SchedOffsets { size_t topos, sims, warps, ctas, plan_c, plan_topo, plan_var, topo_pred, topo_routes; };
 
 SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
   SchedOffsets o;
@@ -524,6 +580,7 @@ SchedOffsets add_schedule(const Schedule& sc, Blob* blob) {
   o.plan_topo = blob->add(sc.plan_topo_v.data(), sc.plan_topo_v.size() * sizeof(uint32_t));
   o.plan_var = blob->add(sc.plan_var_v.data(), sc.plan_var_v.size() * sizeof(uint32_t));
   o.topo_pred = blob->add(sc.topo_pred.data(), sc.topo_pred.size());
+  o.topo_routes = blob->add(sc.topo_routes.data(), sc.topo_routes.size() * sizeof(TopoRoutes));
   return o;
 }
 
@@ -537,6 +594,7 @@ void point_schedule(KParams* kp, uint8_t* ws, const SchedOffsets& o, size_t pool
   kp->plan_topo = reinterpret_cast<const uint32_t*>(ws + o.plan_topo);
   kp->plan_var = reinterpret_cast<const uint32_t*>(ws + o.plan_var);
   kp->topo_pred = ws + o.topo_pred;
+  kp->topo_routes = reinterpret_cast<const TopoRoutes*>(ws + o.topo_routes);
   kp->status = reinterpret_cast<int32_t*>(ws);
 }
 
@@ -958,6 +1016,12 @@ struct KeyBuilder {
     val(pl->n_plans); val(pl->max_stages);
     put(pl->n_stages, pl->n_plans); put(pl->stage_mask, (size_t)pl->n_plans * pl->max_stages);
     put(pl->stage_c, (size_t)pl->n_plans * pl->max_stages * 2);
+    val(pl->max_routes);
+  }
+  void routes(const cf_plans* pl, uint32_t T) {
+    if (!pl->max_routes) return;
+    put(pl->route_mask, (size_t)pl->n_plans * T * pl->max_routes);
+    put(pl->route_cum, (size_t)pl->n_plans * T * pl->max_routes * 4);
   }
 };
 
@@ -1004,10 +1068,10 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_graph(a.g)) return rc;
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode)) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode || a.pl->max_routes)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   KeyBuilder kb;
-  kb.val((uint32_t)1); kb.graph(a.g); kb.plans(a.pl); kb.val(a.R); kb.val(a.seed); kb.put(a.slo->L_us, a.g->n_types * 8);
+  kb.val((uint32_t)1); kb.graph(a.g); kb.plans(a.pl); kb.routes(a.pl, a.g->n_types); kb.val(a.R); kb.val(a.seed); kb.put(a.slo->L_us, a.g->n_types * 8);
   kb.val(a.opt); kb.val((uint32_t)(a.stream_records != nullptr)); kb.val(a.n_variants);
   if (a.stream_records && a.plan_variant) kb.put(a.plan_variant, (size_t)a.pl->n_plans * 4);
   std::shared_ptr<Prepared> pp = cache_find(kb.b);
@@ -1032,6 +1096,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = cuda_rc(p.upload(ws, a.st))) return rc;
   KParams kp = p.kp;
   point_schedule(&kp, ws, p.so, p.pool_off);
+  kp.max_routes = a.pl->max_routes;
   kp.stream = static_cast<const uint4*>(a.stream_records);
   kp.variant_lo = a.stream_records ? 0 : a.variant;
   kp.rates = a.rates_dev;
@@ -1056,11 +1121,11 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rate_hi_dev || !a.slo || !a.slo->L_us || !a.slo->att_num || !a.slo->att_den || !a.out_rate || !a.out_goodput)
     return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode)) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode || a.pl->max_routes)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
   KeyBuilder kb;
-  kb.val((uint32_t)2); kb.graph(a.g); kb.plans(a.pl); kb.val(a.n_steps); kb.val(a.seed); kb.put(a.slo->L_us, T * 8);
+  kb.val((uint32_t)2); kb.graph(a.g); kb.plans(a.pl); kb.routes(a.pl, a.g->n_types); kb.val(a.n_steps); kb.val(a.seed); kb.put(a.slo->L_us, T * 8);
   kb.put(a.slo->att_num, T * 4); kb.put(a.slo->att_den, T * 4);
   kb.val(a.opt); kb.val((uint32_t)(a.stream_records != nullptr)); kb.val(a.n_variants);
   if (a.stream_records && a.plan_variant) kb.put(a.plan_variant, (size_t)P * 4);
@@ -1106,6 +1171,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (int32_t rc = cuda_rc(p.upload(ws, a.st))) return rc;
   KParams kp = p.kp;
   point_schedule(&kp, ws, p.so, p.pool_off);
+  kp.max_routes = a.pl->max_routes;
   BisectState bs;
   bs.lo = reinterpret_cast<uint32_t*>(ws + lo_off);
   bs.hi = reinterpret_cast<uint32_t*>(ws + hi_off);
@@ -1166,7 +1232,7 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   const size_t max_warps = P * R / 32 + P + 1;
   n += align_up(max_warps * sizeof(WarpDesc));
   n += align_up(max_warps * sizeof(CtaDesc));
-  n += align_up(P * 8 * 2) + 2 * align_up(P * 4) + align_up(P * 64);  // plan_c, plan_topo / plan_var, topo_pred
+  n += align_up(P * 8 * 2) + 2 * align_up(P * 4) + align_up(P * 64) + align_up(P * sizeof(TopoRoutes));  // plan_c, plan_topo / plan_var, topo_pred, topo_routes
   n += 4 * kAlign + 3 * align_up(P * 4) + align_up(P * Rb * 4);  // bisection: att, lo/hi, probes, tree
   n += align_up(P * Rb * K * T * 2 * 4) + align_up(P * K * T * 2 * 4) + kAlign;  // probe + at_lo counts
   n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch
@@ -1337,6 +1403,7 @@ int32_t cf_trace_sim_opt(const cf_options* opt_in, const cf_graph* g, const cf_p
   if (int32_t rc = cuda_rc(cudaMemcpyAsync(ws, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, st)))
     return rc;
   point_schedule(&kp, ws, so, pool_off);
+  kp.max_routes = pl->max_routes;
   kp.variant_lo = variant;
   kp.rates = reinterpret_cast<const uint32_t*>(ws + rate_off);
   kp.out_counts = reinterpret_cast<uint32_t*>(ws + scratch_off);
@@ -1485,12 +1552,17 @@ int32_t aux_setup(const cf_graph* g, const cf_plans* pl, const cf_slo* slo, uint
       if ((g->type_mask[t] >> i) & 1) ap.tab_id[i * 8 + t] = g->svc_tab[i * g->n_types + t];
   ap.n_tabs = g->n_tabs;
   const size_t tabs_off = a.blob.add(tabs.data(), tabs.size() * sizeof(DevTab));
-  size_t ns_off = 0, sm_off = 0, sc_off = 0;
+  size_t ns_off = 0, sm_off = 0, sc_off = 0, rm_off = 0, rc_off = 0;
   if (pl) {
     ap.P = pl->n_plans; ap.MS = pl->max_stages;
     ns_off = a.blob.add(pl->n_stages, (size_t)pl->n_plans);
     sm_off = a.blob.add(pl->stage_mask, (size_t)pl->n_plans * pl->max_stages);
     sc_off = a.blob.add(pl->stage_c, (size_t)pl->n_plans * pl->max_stages * sizeof(uint16_t));
+    if (pl->max_routes) {
+      ap.max_routes = pl->max_routes;
+      rm_off = a.blob.add(pl->route_mask, (size_t)pl->n_plans * g->n_types * pl->max_routes);
+      rc_off = a.blob.add(pl->route_cum, (size_t)pl->n_plans * g->n_types * pl->max_routes * 4);
+    }
   }
   a.mean_off = align_up(a.blob.bytes.size());
   a.demand_off = align_up(a.mean_off + (size_t)g->n_tabs * 8);
@@ -1506,6 +1578,8 @@ int32_t aux_setup(const cf_graph* g, const cf_plans* pl, const cf_slo* slo, uint
     ap.n_stages = w + ns_off;
     ap.stage_mask = w + sm_off;
     ap.stage_c = reinterpret_cast<const uint16_t*>(w + sc_off);
+    ap.route_mask = w + rm_off;
+    ap.route_cum = reinterpret_cast<const uint32_t*>(w + rc_off);
   }
   ap.mean_q16 = reinterpret_cast<uint64_t*>(w + a.mean_off);
   ap.demand_q16 = reinterpret_cast<uint64_t*>(w + a.demand_off);
@@ -1528,7 +1602,8 @@ extern "C" {
 size_t cf_aux_workspace_bytes(const cf_graph* g, const cf_plans* pl) {
   if (!g || !g->tabs) return 0;
   size_t n = 2 * kAlign + align_up(pool_entries(g) * 4) + align_up((size_t)g->n_tabs * sizeof(DevTab));
-  if (pl) n += 3 * kAlign + align_up((size_t)pl->n_plans) + align_up((size_t)pl->n_plans * pl->max_stages * 3);
+  if (pl) n += 5 * kAlign + align_up((size_t)pl->n_plans) + align_up((size_t)pl->n_plans * pl->max_stages * 3) +
+               align_up((size_t)pl->n_plans * g->n_types * pl->max_routes * 5);
   n += align_up((size_t)g->n_tabs * 8) + align_up(256 * 8) + align_up((size_t)g->n_trials * 72 * 4);
   return n + 4 * kAlign;
 }
@@ -1561,6 +1636,7 @@ int32_t cf_mc_latency(const cf_graph* g, const cf_plans* pl, const uint32_t* rat
   if (int32_t rc = check_plans(g, pl)) return rc;
   if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return CF_ERR_ARG;
   if (g->join_mode) return CF_ERR_ARG;  // fork-join latency is a critical path, not a sum (R25)
+  if (pl->max_routes) return CF_ERR_ARG;  // routed plans: not offered (R26)
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   AuxSetup a;
   if (int32_t rc = aux_setup(g, pl, slo, seed, variant, workspace, workspace_bytes, st, &a)) return rc;

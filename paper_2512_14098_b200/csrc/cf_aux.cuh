@@ -61,6 +61,9 @@ struct AuxParams {
   const uint8_t* n_stages;    // [P]
   const uint8_t* stage_mask;  // [P*MS]
   const uint16_t* stage_c;    // [P*MS]
+  uint32_t max_routes;        // R26: 0 = none
+  const uint8_t* route_mask;  // [P*T*max_routes]
+  const uint32_t* route_cum;  // [P*T*max_routes]
   uint64_t* mean_q16;         // [n_tabs]
   uint64_t* demand_q16;       // [256] demand of the node with component mask m
   uint32_t* hist;             // [K][8][9]: hits for h = 0..7 hops, [8] = requests of the type
@@ -125,6 +128,32 @@ __device__ __forceinline__ uint64_t saturation_mrps(uint64_t c, uint64_t Dq) {
   return c * 65536ull * 1000000000ull / Dq;
 }
 
+// R26: demand of stage s of plan p when types reach it only on some of their routes
+__device__ __forceinline__ uint64_t routed_demand_q16(const AuxParams& prm, uint32_t p, uint32_t s) {
+  const uint32_t mask = prm.stage_mask[(size_t)p * prm.MS + s], MR = prm.max_routes;
+  U128 D{0, 0};
+  for (uint32_t t = 0; t < prm.T; ++t) {
+    const uint64_t thi = (t + 1 == prm.T) ? (1ull << 32) : (uint64_t)prm.type_thresh[t];
+    const uint64_t tlo = t == 0 ? 0ull : (uint64_t)prm.type_thresh[t - 1];
+    const uint64_t w = thi > tlo ? thi - tlo : 0ull;
+    uint64_t mu = 0;
+    for (uint32_t i = 0; i < prm.C; ++i)
+      if (((mask & prm.type_mask[t]) >> i) & 1u) mu += prm.mean_q16[prm.tab_id[i * 8 + t]];
+    for (uint32_t r = 0; r < MR; ++r) {
+      const size_t at = ((size_t)p * prm.T + t) * MR + r;
+      if (!((prm.route_mask[at] >> s) & 1u)) continue;
+      const uint64_t hi = (r + 1 == MR) ? (1ull << 32) : (uint64_t)prm.route_cum[at];
+      const uint64_t lo = r == 0 ? 0ull : (uint64_t)prm.route_cum[at - 1];
+      const uint64_t q = hi > lo ? hi - lo : 0ull;
+      // floor(w * q / 2^32): w, q <= 2^32, so the product needs 65 bits at most
+      const uint64_t pl = w * q, ph = __umul64hi(w, q);
+      const uint64_t pr = (pl >> 32) | (ph << 32);
+      u128_add_mul(D, pr, mu);
+    }
+  }
+  return (D.lo >> 32) | (D.hi << 32);
+}
+
 __global__ void __launch_bounds__(128)
 flow_plan_kernel(const __grid_constant__ AuxParams prm, uint32_t* out_rate, uint32_t* out_bound,
                  uint8_t* out_bottleneck, uint8_t* out_redundant) {
@@ -134,7 +163,7 @@ flow_plan_kernel(const __grid_constant__ AuxParams prm, uint32_t* out_rate, uint
   uint64_t R = UINT64_MAX;
   uint32_t bott = 0xffu;
   for (uint32_t s = 0; s < V; ++s) {
-    const uint64_t Dq = prm.demand_q16[prm.stage_mask[(size_t)p * prm.MS + s]];
+    const uint64_t Dq = prm.max_routes ? routed_demand_q16(prm, p, s) : prm.demand_q16[prm.stage_mask[(size_t)p * prm.MS + s]];
     if (Dq == 0) continue;
     const uint64_t r = saturation_mrps(prm.stage_c[(size_t)p * prm.MS + s], Dq);
     if (r < R) { R = r; bott = s; }
@@ -143,7 +172,7 @@ flow_plan_kernel(const __grid_constant__ AuxParams prm, uint32_t* out_rate, uint
   for (uint32_t s = 0; s < V; ++s) {
     const uint64_t c = prm.stage_c[(size_t)p * prm.MS + s];
     if (c < 2) continue;
-    const uint64_t Dq = prm.demand_q16[prm.stage_mask[(size_t)p * prm.MS + s]];
+    const uint64_t Dq = prm.max_routes ? routed_demand_q16(prm, p, s) : prm.demand_q16[prm.stage_mask[(size_t)p * prm.MS + s]];
     if (Dq == 0 || saturation_mrps(c - 1, Dq) >= R) redundant = true;
   }
   const uint64_t bound = R < 1000000000ull ? R : 1000000000ull;

@@ -35,6 +35,13 @@ struct TopoDesc {  // one plan topology = ordered stage masks
   uint8_t pad[7];
 };
 
+// R26: routing table of a topology: per type up to 4 routes = (cumulative probability Q32, bitmask
+// over the topology's stages the route may visit); the last route is the catch-all
+struct TopoRoutes {
+  uint32_t cum[8][4];
+  uint8_t mask[8][4];
+};
+
 struct SimDesc {
   uint32_t plan;  // plan index (for replica counts)
   uint32_t pr;    // p*R + r : index into the rate array; output slot is pr*K + k
@@ -100,6 +107,8 @@ struct KParams {
   uint8_t* tr_type;
   uint32_t tr_plan;        // the traced plan (scan kernel: the warp whose simulation is written out)
   uint32_t has_cpu;        // some (component, type) has a CPU pre-processing table (R24): 64-bit kernel only
+  uint32_t max_routes;     // R26: 0 = no routing tables; else routes per (topology, type)
+  const TopoRoutes* topo_routes;  // [topology]
   uint32_t join;           // fork-join routing along the DAG edges (R25): 64-bit kernel only
   const uint8_t* topo_pred;  // join: [topology][type 8][stage 8] bitmask of the stage's predecessor stages
 };
@@ -141,6 +150,16 @@ __device__ __forceinline__ int32_t qtab_sample(const int32_t* __restrict__ pool,
   return q0 + (int32_t)(((int64_t)(q1 - q0) * (int64_t)f) >> 16);
 }
 
+// R26: stages the request of type t with route draw u may visit on topology `topo` (0xff: no routing)
+__device__ __forceinline__ uint32_t route_stages(const KParams& prm, uint32_t topo, uint32_t t, uint32_t u) {
+  if (prm.max_routes == 0u) return 0xffu;
+  const TopoRoutes* tr = prm.topo_routes + topo;
+  uint32_t r = prm.max_routes - 1u;
+  for (int rr = (int)prm.max_routes - 2; rr >= 0; --rr)
+    if (u < __ldg(&tr->cum[t][rr])) r = (uint32_t)rr;  // first route with u < cum
+  return __ldg(&tr->mask[t][r]);
+}
+
 __device__ __forceinline__ uint64_t warp_inclusive_sum(uint64_t v, int lane) {
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
@@ -179,13 +198,14 @@ __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_
                                                      int lane) {
   const uint32_t n = n0 + lane;
   const bool valid = n < prm.N;
-  uint32_t gap = 0, t = 0;
+  uint32_t gap = 0, t = 0, route_u = 0;
   int32_t svc[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) svc[i] = 0;
   if (valid) {
     const uint4 b0 = philox4x32_10(n, trial, 0, variant, prm.seed_lo, prm.seed_hi);
     gap = (uint32_t)qtab_sample(prm.qpool, prm.arr_tab, b0.x);
+    route_u = b0.z;  // R26: the route draw (block 0, word 2)
     t = prm.T - 1;
     for (int tt = (int)prm.T - 2; tt >= 0; --tt)
       if (b0.y < prm.type_thresh[tt]) t = tt;  // first tt with u < thresh[tt]
@@ -239,7 +259,7 @@ __device__ __forceinline__ void produce_chunk_philox(const KParams& prm, uint32_
   uint4* dst = tile_chunk + lane * CompRec<CMAX, HAS_CPU>::kWords;
   dst[0] = make_uint4((uint32_t)cu, (uint32_t)(cu >> 32) | (t << 24), (uint32_t)svc[0], (uint32_t)svc[1]);
   dst[1] = make_uint4((uint32_t)svc[2], (uint32_t)svc[3], (uint32_t)svc[4], (uint32_t)svc[5]);
-  if (CMAX > 6) dst[2] = make_uint4((uint32_t)svc[6], (uint32_t)svc[7], 0u, 0u);
+  if (CMAX > 6) dst[2] = make_uint4((uint32_t)svc[6], (uint32_t)svc[7], route_u, 0u);  // routed calls use this record
   if (HAS_CPU) {
     constexpr int kB = CompRec<CMAX, HAS_CPU>::kBase;
     dst[kB] = make_uint4((uint32_t)cpu[0], (uint32_t)cpu[1], (uint32_t)cpu[2], (uint32_t)cpu[3]);
@@ -456,8 +476,10 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
           svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x;
           svc[3] = (int32_t)w1.y; svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w;
           svc[6] = 0; svc[7] = 0;
-          if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
+          uint32_t route_u = 0;
+          if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; route_u = w2.z; }
           const uint32_t t = w0.y >> 24;
+          const uint32_t rmask = CMAX > 6 ? route_stages(prm, wd.topo, t, route_u) : 0xffu;  // R26
           if (streamed)
             for (uint32_t tt = 0; tt < prm.T; ++tt) {
               const uint32_t b = __ballot_sync(0xffffffffu, lane < n_here && t == tt);
@@ -483,7 +505,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
               acc += ((sm >> i) & 1u) ? svc[i] : 0;
               accc += ((sm >> i) & 1u) ? cpu[i] : 0;
             }
-            S[s] = (sm & tm) ? acc : -1;
+            S[s] = ((sm & tm) && ((rmask >> s) & 1u)) ? acc : -1;
             Sc[s] = accc;
           }
           uint4* dst = wbuf + lane * kSW;
@@ -569,7 +591,7 @@ cf_sim_kernel(const __grid_constant__ KParams prm, uint32_t cta_base) {
                 const uint32_t pm = (uint32_t)(pmask >> (8 * s)) & 0xffu;
 #pragma unroll
                 for (int sp = 0; sp < s; ++sp)
-                  if ((pm >> sp) & 1u) { const int64_t a = xs[sp] + delay; x = a > x ? a : x; }
+                  if (((pm >> sp) & 1u) && S[sp] >= 0) { const int64_t a = xs[sp] + delay; x = a > x ? a : x; }
               } else if (HAS_DELAY) { if (!first) x += delay; first = false; }
               const int64_t f = root[s];
               if (HAS_CPU) x = (f <= x) ? x + (int64_t)Sc[s] : f;  // idle: CPU + GPU; queued: GPU alone (R24)

@@ -368,8 +368,10 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
           svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x;
           svc[3] = (int32_t)w1.y; svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w;
           svc[6] = 0; svc[7] = 0;
-          if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; }
+          uint32_t route_u = 0;
+          if (CMAX > 6) { const uint4 w2 = src[2]; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y; route_u = w2.z; }
           const uint32_t t = w0.y >> 24;
+          const uint32_t rmask = CMAX > 6 ? route_stages(prm, wd.topo, t, route_u) : 0xffu;  // R26
           if (PW) {
             for (uint32_t tt = 0; tt < prm.T; ++tt) {
               const uint32_t b = __ballot_sync(kFull, lane < n_here && t == tt);
@@ -392,7 +394,7 @@ cf_sim32_kernel(const __grid_constant__ KParams prm) {
 #pragma unroll
           for (int s = 0; s < VMAX; ++s) {
             const uint32_t sm = (s < (int)n_stages) ? topo.mask[s] : 0u;
-            if (sm & tm) {
+            if ((sm & tm) && ((rmask >> s) & 1u)) {
               int32_t acc = 0;
 #pragma unroll
               for (int i = 0; i < CMAX; ++i) acc += ((sm >> i) & 1u) ? svc[i] : 0;

@@ -94,6 +94,86 @@ def test_random_eval(cf, orc, seed):
         np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
 
 
+STREAM_SEEDS = [sd for sd in range(200, 330)] + list(range(12000, 12000 + EXTRA // 2))
+
+
+@pytest.mark.parametrize("seed", STREAM_SEEDS)
+def test_random_stream_eval_and_bisect(cf, orc, seed):
+    """The materialised-stream path (per-warp chunk rings of the fast kernel, per-warp loads of the
+    64-bit kernel, blocks that mix stream variants) on random graphs with at most 6 components."""
+    w, R_p = random_case(seed)
+    g, pl = w.graph, w.plans
+    if g.n_comp > 6:
+        pytest.skip("the 32-byte stream record holds 6 components")
+    if orc.validate(g, pl) != 0:
+        pytest.skip("the generator drew services whose worst-case sum exceeds int32 (R17)")
+    rng = np.random.default_rng(seed)
+    n_var = int(rng.integers(1, 4))
+    pv = rng.integers(0, n_var, pl.n_plans).astype(np.uint32)
+    rec = cf.cf_materialize_stream(g, w.seed, 7, n_var)
+    np.testing.assert_array_equal(rec.cpu().numpy().reshape(-1),
+                                  orc.materialize_stream(g, w.seed, 7, n_var).view(np.uint8).reshape(-1))
+    for mode in (0, 1):
+        cf.cf_debug_kernel_mode(mode)
+        try:
+            got = cf.cf_eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, stream_records=rec, n_variants=n_var, plan_variant=pv)
+            status = cf.cf_workspace_status(got["workspace"])
+        finally:
+            cf.cf_debug_kernel_mode(0)
+        rc = 0
+        for v in range(n_var):
+            idx = np.nonzero(pv == v)[0]
+            if idx.size == 0:
+                continue
+            o = orc.eval_plans(g, pl.subset(idx), w.rate_mrps[idx], w.slo, w.seed, 7 + v, n_threads=NT)
+            rc = rc or o["rc"]
+            np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"])[idx], o["counts"])
+            np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"])[idx], o["dep_sum"])
+            np.testing.assert_array_equal(got["makespan"].cpu().numpy()[idx], o["makespan"])
+        assert status == rc
+    if seed % 4 == 0:
+        hi = np.minimum(np.ceil(1.5 * np.minimum(R_p, 1e9)), 1_000_000_000).astype(np.uint32)
+        b = cf.cf_goodput_bisect(g, pl, hi, 9, w.slo, w.seed, stream_records=rec, n_variants=n_var, plan_variant=pv)
+        for v in range(n_var):
+            idx = np.nonzero(pv == v)[0]
+            if idx.size == 0:
+                continue
+            bo = orc.goodput_bisect(g, pl.subset(idx), hi[idx], 9, w.slo, w.seed, 7 + v, n_threads=NT)
+            np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"])[idx], bo["rate_mrps"])
+            np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"])[idx], bo["counts"])
+
+
+VARIANT_SEEDS = list(range(400, 448)) + list(range(15000, 15000 + EXTRA // 4))
+
+
+@pytest.mark.parametrize("seed", VARIANT_SEEDS)
+def test_random_fidelity_variants(cf, orc, seed):
+    """CPU-GPU overlap (R24) and fork-join (R25), alone and together, on the random graphs (chain DAGs
+    with a few extra forward edges so that stages really fork)."""
+    w, _ = random_case(seed)
+    g, pl = w.graph, w.plans
+    rng = np.random.default_rng(seed + 1)
+    C, T = g.n_comp, g.n_types
+    if seed % 3 != 1:  # overlap: CPU tables for a random subset of the components
+        g.tabs = g.tabs + [W.exponential_qtab(float(rng.uniform(500.0, 40_000.0))) for _ in range(2)]
+        cpu = np.full(C * T, 0xFFFF, np.uint16)
+        for i in range(C):
+            if rng.random() < 0.5:
+                cpu[i * T:(i + 1) * T] = C + int(rng.integers(0, 2))
+        g.cpu_tab = cpu
+    if seed % 3 != 0:  # fork-join: skip-edges i -> i+2 turn the chain into a DAG with parallel branches
+        edges = [[i, i + 2] for i in range(C - 2)] + ([[0, 1]] if C > 1 and rng.random() < 0.5 else [])
+        g.edges = np.asarray(edges, dtype=np.uint8).reshape(-1, 2)
+        g.join_mode = 1
+    assert orc.validate(g, pl) == 0
+    want = orc.eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, 2, n_threads=NT)
+    got = cf.cf_eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, 2)
+    assert cf.cf_workspace_status(got["workspace"]) == want["rc"]
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+    np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+
+
 @pytest.mark.parametrize("seed", BISECT_SEEDS)
 def test_random_bisect(cf, orc, seed):
     w, R_p = random_case(seed)

@@ -45,8 +45,12 @@ def random_case(seed):
         kind = rng.integers(0, 3)
         m = scale * float(rng.uniform(0.2, 3.0))
         L, B = SHAPES[int(rng.integers(0, len(SHAPES)))] if seed >= 64 else (16, 6)  # seeds < 64: round 1's cases
-        tabs.append(W.lognormal_qtab(m, float(rng.uniform(0.2, 0.9)), L, B) if kind == 0 else
-                    W.exponential_qtab(m, L, B) if kind == 1 else W.constant_qtab(int(m), L, B))
+        sigma = float(rng.uniform(0.2, 0.9))
+        try:
+            tabs.append(W.lognormal_qtab(m, sigma, L, B) if kind == 0 else
+                        W.exponential_qtab(m, L, B) if kind == 1 else W.constant_qtab(int(m), L, B))
+        except AssertionError:  # a 32-level tail beyond int32 microseconds: keep the shape, drop the tail
+            tabs.append(W.constant_qtab(int(m), L, B))
     masks = [int(rng.integers(0, 1 << C)) for _ in range(T)]
     if rng.random() < 0.8:
         masks = [m | (1 << int(rng.integers(0, C))) for m in masks]  # mostly non-empty routes
@@ -79,7 +83,9 @@ def random_case(seed):
 @pytest.mark.parametrize("seed", EVAL_SEEDS)
 def test_random_eval(cf, orc, seed):
     w, _ = random_case(seed)
-    assert orc.validate(w.graph, w.plans) == 0
+    if orc.validate(w.graph, w.plans) != 0:
+        assert seed >= 128  # none of the committed seeds
+        pytest.skip("the generator drew services whose worst-case sum exceeds int32 (R17)")
     want = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, 3, n_threads=NT)
     for mode in (0, 1):
         cf.cf_debug_kernel_mode(mode)
@@ -165,7 +171,9 @@ def test_random_fidelity_variants(cf, orc, seed):
         edges = [[i, i + 2] for i in range(C - 2)] + ([[0, 1]] if C > 1 and rng.random() < 0.5 else [])
         g.edges = np.asarray(edges, dtype=np.uint8).reshape(-1, 2)
         g.join_mode = 1
-    assert orc.validate(g, pl) == 0
+    if orc.validate(g, pl) != 0:
+        assert seed >= 448  # none of the committed seeds
+        pytest.skip("the generator drew services whose worst-case sum exceeds int32 (R17)")
     want = orc.eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, 2, n_threads=NT)
     got = cf.cf_eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, 2)
     assert cf.cf_workspace_status(got["workspace"]) == want["rc"]

@@ -185,6 +185,9 @@ def test_random_fidelity_variants(cf, orc, seed):
 @pytest.mark.parametrize("seed", BISECT_SEEDS)
 def test_random_bisect(cf, orc, seed):
     w, R_p = random_case(seed)
+    if orc.validate(w.graph, w.plans) != 0:
+        assert seed >= 124  # none of the committed seeds
+        pytest.skip("the generator drew services whose worst-case sum exceeds int32 (R17)")
     hi = np.minimum(np.ceil(1.5 * np.minimum(R_p, 1e9)), 1_000_000_000).astype(np.uint32)
     steps = int(np.random.default_rng(seed).integers(1, 22))
     bo = orc.goodput_bisect(w.graph, w.plans, hi, steps, w.slo, w.seed, n_threads=NT)

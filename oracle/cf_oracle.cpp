@@ -82,6 +82,7 @@ int32_t validate(const orc_graph* g, const orc_plans* pl) {
   if (!g->type_mask || !g->type_thresh || !g->svc_tab || !g->tabs || g->n_tabs < 1)
     return ORC_ERR_ARG;
   if (g->n_edges > 0 && !g->edges) return ORC_ERR_ARG;
+  if (g->order_mode > 1 || (g->order_mode && g->join_mode)) return ORC_ERR_ARG; /* R27: path routing only */
   for (uint32_t t = 0; t < T; ++t) {
     if (g->type_mask[t] >> C) return ORC_ERR_ARG;
     if (t > 0 && g->type_thresh[t] < g->type_thresh[t - 1]) return ORC_ERR_ARG;
@@ -185,11 +186,112 @@ struct SimOut {
   int32_t status;
 };
 
+/* One simulation with ARRIVAL-ORDER service (orc_graph.order_mode = 1; R27, SURVEY.md 8(f)
+ * NEXT-4 "true stage-arrival-order FCFS", the discipline reading R2 departs from): every stage
+ * serves its visitors in the order in which they REACH the stage, ties by request index -- textbook
+ * FCFS at a c-server node. The plan's stages are in topological order and a request only moves
+ * forward, so the arrivals at stage s are known once stages 0..s-1 are done: the stages are
+ * processed one after another, each over all its visitors sorted by (arrival at the stage, index).
+ * Same draws, same arrival times, same per-visit rule (Kiefer-Wolfowitz, idle/busy R24, hop delay
+ * R9, routes R26) as simulate(); only the order of service differs. */
+void simulate_fcfs(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate_mrps, uint32_t k,
+                   const orc_slo* slo, uint64_t seed, uint32_t variant, SimOut* out,
+                   int64_t* trace_arr, int64_t* trace_dep, uint8_t* trace_type) {
+  std::memset(out, 0, sizeof(*out));
+  const uint32_t C = g->n_comp, T = g->n_types, N = g->n_req;
+  const uint32_t V = pl->n_stages[p];
+  const uint8_t* smask = pl->stage_mask + (size_t)p * pl->max_stages;
+  const uint16_t* sc = pl->stage_c + (size_t)p * pl->max_stages;
+  if (rate_mrps < 1 || rate_mrps > 1000000000u) {
+    out->status = ORC_ERR_RANGE;
+    return;
+  }
+  const int64_t period_us = (int64_t)((1000000000ull + rate_mrps / 2) / rate_mrps);
+  const uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
+  /* the requests of the trial: the draws of simulate(), kept per request */
+  std::vector<int64_t> A(N), x(N), svc((size_t)N * 8, 0), cpu((size_t)N * 8, 0);
+  std::vector<uint8_t> type(N), route(N, 0xff), hops(N, 0);
+  uint64_t CU = 0;
+  for (uint32_t n = 0; n < N; ++n) {
+    uint32_t b0[4];
+    philox(n, k, 0, variant, k0, k1, b0);
+    CU += (uint64_t)qtab_sample(g->arr_tab, b0[0]);
+    unsigned __int128 wide = (unsigned __int128)CU * (uint64_t)period_us + 32768u;
+    if (wide >= (unsigned __int128)RANGE_LIMIT) { /* R17 */
+      out->status = ORC_ERR_RANGE;
+      return;
+    }
+    A[n] = (int64_t)((CU * (uint64_t)period_us + 32768u) >> 16);
+    uint32_t t = T - 1;
+    for (uint32_t tt = 0; tt < T; ++tt)
+      if (b0[1] < g->type_thresh[tt]) { t = tt; break; }
+    type[n] = (uint8_t)t;
+    if (pl->max_routes > 0) { /* R26 */
+      const uint32_t MR = pl->max_routes;
+      uint32_t r = MR - 1;
+      for (uint32_t rr = 0; rr < MR; ++rr)
+        if (b0[2] < pl->route_cum[((size_t)p * T + t) * MR + rr]) { r = rr; break; }
+      route[n] = pl->route_mask[((size_t)p * T + t) * MR + r];
+    }
+    for (uint32_t i = 0; i < C; ++i)
+      if ((g->type_mask[t] >> i) & 1) {
+        uint32_t b[4];
+        philox(n, k, 1 + i / 4, variant, k0, k1, b);
+        svc[(size_t)n * 8 + i] = qtab_sample(g->tabs[g->svc_tab[i * T + t]], b[i % 4]);
+        if (g->cpu_tab && g->cpu_tab[i * T + t] != 0xffff) { /* R24 */
+          philox(n, k, 3 + i / 4, variant, k0, k1, b);
+          cpu[(size_t)n * 8 + i] = qtab_sample(g->tabs[g->cpu_tab[i * T + t]], b[i % 4]);
+        }
+      }
+    x[n] = A[n]; /* a request that visits no stage leaves at once (R14) */
+  }
+  for (uint32_t s = 0; s < V; ++s) { /* stages in the plan's (topological) order */
+    std::vector<std::pair<int64_t, uint32_t>> order; /* (arrival at stage s, request index) */
+    for (uint32_t n = 0; n < N; ++n) {
+      const uint8_t m = smask[s] & g->type_mask[type[n]];
+      if (m == 0 || !((route[n] >> s) & 1)) continue;
+      order.emplace_back(x[n] + (hops[n] ? g->edge_delay_us : 0), n); /* R9: a hop delay after the first visit */
+    }
+    std::sort(order.begin(), order.end()); /* first come, first served; ties: lower index */
+    std::vector<int64_t> F(sc[s], 0); /* free times of the c replicas, sorted ascending */
+    for (const auto& e : order) {
+      const int64_t a = e.first;
+      const uint32_t n = e.second;
+      const uint8_t m = smask[s] & g->type_mask[type[n]];
+      int64_t S = 0, S_cpu = 0;
+      for (uint32_t i = 0; i < C; ++i)
+        if ((m >> i) & 1) { S += svc[(size_t)n * 8 + i]; S_cpu += cpu[(size_t)n * 8 + i]; }
+      const int64_t f = F[0];
+      int64_t d;
+      if (f <= a) d = a + S_cpu + S; /* idle executor: CPU + GPU time */
+      else d = f + S;                /* busy: GPU time alone */
+      x[n] = d;
+      hops[n]++;
+      F[0] = d;
+      std::sort(F.begin(), F.end());
+    }
+  }
+  for (uint32_t n = 0; n < N; ++n) {
+    const uint32_t t = type[n];
+    out->cnt[t]++;
+    if (x[n] - A[n] <= slo->L_us[t]) out->hits[t]++;
+    out->dep_sum += (uint64_t)x[n];
+    out->makespan = std::max(out->makespan, x[n]);
+    if (trace_arr) trace_arr[n] = A[n];
+    if (trace_dep) trace_dep[n] = x[n];
+    if (trace_type) trace_type[n] = (uint8_t)t;
+  }
+}
+
 /* One simulation, SURVEY.md 8(c) / DESIGN.md "Algorithm", literally.
  * trace_*: optional [N] outputs. */
 void simulate(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate_mrps, uint32_t k,
               const orc_slo* slo, uint64_t seed, uint32_t variant, SimOut* out,
               int64_t* trace_arr, int64_t* trace_dep, uint8_t* trace_type) {
+  if (g->order_mode) { /* R27: arrival-order service, stage by stage */
+    simulate_fcfs(g, pl, p, rate_mrps, k, slo, seed, variant, out, trace_arr, trace_dep, trace_type);
+    return;
+  }
   std::memset(out, 0, sizeof(*out));
   const uint32_t C = g->n_comp, T = g->n_types, N = g->n_req;
   const uint32_t V = pl->n_stages[p];

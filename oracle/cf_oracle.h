@@ -61,6 +61,9 @@ typedef struct {
   uint32_t join_mode;          /* 0: a request visits its stages one after another (R7); 1: fork-join along
                                   the DAG edges (R25): a stage starts when all its predecessor
                                   stages on the request's subgraph have finished */
+  uint32_t order_mode;         /* 0: every stage serves its visitors in request-index order (R2);
+                                  1: in the order in which they reach the stage, ties by index -- textbook
+                                  FCFS (R27); not with join_mode = 1 */
 } orc_graph;
 
 /* P physical plans, each an ordered list of stages = (component bitmask, replica count). */

@@ -42,7 +42,7 @@ class _Graph(C.Structure):
                 ("tabs", C.POINTER(_QTab)), ("n_tabs", C.c_uint32), ("arr_tab", _QTab),
                 ("edges", C.POINTER(C.c_uint8)), ("n_edges", C.c_uint32),
                 ("edge_delay_us", C.c_int64), ("cpu_tab", C.POINTER(C.c_uint16)),
-                ("join_mode", C.c_uint32)]
+                ("join_mode", C.c_uint32), ("order_mode", C.c_uint32)]
 
 
 class _Plans(C.Structure):
@@ -99,7 +99,7 @@ class _Marshalled:
                                            _ptr(g.arr_tab.q, C.c_int32)),
                         _ptr(edges if edges.size else None, C.c_uint8), edges.size // 2,
                         int(g.edge_delay_us), _ptr(getattr(g, "cpu_tab", None), C.c_uint16),
-                        int(getattr(g, "join_mode", 0)))
+                        int(getattr(g, "join_mode", 0)), int(getattr(g, "order_mode", 0)))
         self.pl = None
         if plans is not None:
             sm = np.ascontiguousarray(plans.stage_mask).reshape(-1)

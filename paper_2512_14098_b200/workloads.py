@@ -52,6 +52,7 @@ class Graph:
     type_frac: Optional[np.ndarray] = None  # float64 [T], the mix the thresholds were built from
     cpu_tab: Optional[np.ndarray] = None    # uint16 [C*T] CPU pre-processing table of (i, t), 0xffff = none (R24)
     join_mode: int = 0                      # 1: fork-join along the DAG edges instead of a path (R25)
+    order_mode: int = 0                     # 1: stages serve in arrival order (textbook FCFS, R27) instead of index order (R2)
 
     def __post_init__(self):
         if self.cpu_tab is not None:

@@ -198,7 +198,10 @@ def fcfs_event_sim(A: List[int], routes, stage_c: List[int], edge_delay: int = 0
     """Textbook FCFS at every stage: a stage serves its visitors in the order in which they REACH
     the stage (ties by request index), on the server that frees first. This is the discipline
     index-order service (R2) departs from when stage arrivals are not monotone in the
-    request index; used to measure that gap, not to pin the oracle."""
+    request index: it measures that gap, and it pins the oracle's arrival-order mode (DESIGN.md
+    R27), which reaches the same result stage by stage with a sort instead of an event queue.
+    A hop may carry a third entry, the CPU pre-processing time paid only when the request finds
+    a server idle on arrival (R24)."""
     n_stage = len(stage_c)
     free = [[0] * c for c in stage_c]
     queue = [[] for _ in range(n_stage)]          # heap of (arrival at the stage, request)
@@ -217,7 +220,11 @@ def fcfs_event_sim(A: List[int], routes, stage_c: List[int], edge_delay: int = 0
             if free[st][k] > now:
                 break
             at, r = heapq.heappop(queue[st])
-            done = max(at, free[st][k]) + routes[r][pos[r]][1]
+            hop = routes[r][pos[r]]
+            if free[st][k] <= at:                    # idle on arrival: CPU + GPU time
+                done = at + (hop[2] if len(hop) > 2 else 0) + hop[1]
+            else:                                    # the request queued: GPU time alone
+                done = free[st][k] + hop[1]
             free[st][k] = done
             heapq.heappush(ev, (done, 1, st))
             pos[r] += 1

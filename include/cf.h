@@ -89,6 +89,13 @@ typedef struct {
                                   component v of the request on that stage -- has finished, plus
                                   edge_delay_us; with no predecessor at its system arrival; it is done when
                                   its last stage is. 64-bit kernel only; no stream; cf_mc_latency refuses.  */
+  uint32_t order_mode;         /* 0: every stage serves its visitors in request-index order (R2).
+                                  1: in the order in which they REACH the stage, ties by request index --
+                                  textbook FCFS at every node (R27). Runs on
+                                  the arrival-order kernel: one warp per simulation, stage by stage, over
+                                  40 N bytes of workspace per simulation in flight (cf_workspace_bytes asks for
+                                  up to 1184 of them; a larger workspace runs up to 4736 at once). Replicas
+                                  per stage <= 256; path routing only (join_mode = 0); no stream.           */
 } cf_graph;
 
 /* P physical plans; plan p is an ORDERED list of n_stages[p] stages, stage s = (bitmask of the

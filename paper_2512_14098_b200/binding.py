@@ -49,7 +49,7 @@ class cf_graph(C.Structure):
                 ("tabs", C.POINTER(cf_qtab)), ("n_tabs", C.c_uint32), ("arr_tab", cf_qtab),
                 ("edges", C.POINTER(C.c_uint8)), ("n_edges", C.c_uint32),
                 ("edge_delay_us", C.c_int64), ("cpu_tab", C.POINTER(C.c_uint16)),
-                ("join_mode", C.c_uint32)]
+                ("join_mode", C.c_uint32), ("order_mode", C.c_uint32)]
 
 
 class cf_plans(C.Structure):
@@ -146,7 +146,7 @@ class Marshalled:
                                                _hp(g.arr_tab.q, C.c_int32)),
                           _hp(edges if edges.size else None, C.c_uint8), edges.size // 2,
                           int(g.edge_delay_us), _hp(getattr(g, "cpu_tab", None), C.c_uint16),
-                          int(getattr(g, "join_mode", 0)))
+                          int(getattr(g, "join_mode", 0)), int(getattr(g, "order_mode", 0)))
         self.pl = None
         if plans is not None:
             sm = np.ascontiguousarray(plans.stage_mask).reshape(-1)

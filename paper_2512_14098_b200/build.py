@@ -14,12 +14,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(_HERE, "libcf_b200.so")
-HEADERS = ["cf_device.cuh", "cf_rel32.cuh", "cf_scan.cuh", "cf_launch.h", "cf_aux.cuh",
+HEADERS = ["cf_device.cuh", "cf_rel32.cuh", "cf_scan.cuh", "cf_launch.h", "cf_aux.cuh", "cf_fcfs.cuh",
            os.path.join("..", "..", "include", "cf.h"), os.path.join("..", "..", "include", "cf_debug.h")]
 # (object name, source, extra defines)
 UNITS = [("cf_api", "cf_api.cu", []),
          ("cf_k64", "cf_k64.cu", []),
-         ("cf_scan", "cf_scan.cu", [])] + \
+         ("cf_scan", "cf_scan.cu", []),
+         ("cf_fcfs", "cf_fcfs.cu", [])] + \
         [(f"cf_k32_v{v}c{c}", "cf_k32.cu", [f"-DCF_VMAX={v}", f"-DCF_CMAX={c}"])
          for v, c in ((2, 6), (4, 6), (6, 6), (8, 6), (8, 8))]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

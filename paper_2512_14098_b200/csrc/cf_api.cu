@@ -73,6 +73,7 @@ int32_t check_graph(const cf_graph* g) {
     if (int32_t rc = check_tab(g->tabs[j])) return rc;
   if (int32_t rc = check_tab(g->arr_tab)) return rc;
   if (g->join_mode > 1) return CF_ERR_ARG;
+  if (g->order_mode > 1 || (g->order_mode && g->join_mode)) return CF_ERR_ARG;  // R27: arrival order on path routing only
   if (g->edge_delay_us < 0 || g->edge_delay_us >= (1ll << 31)) return CF_ERR_RANGE;
   // DESIGN.md R17: a request's total service over all its components must fit int32
   int64_t worst = 0;
@@ -103,10 +104,16 @@ bool graph_has_cpu(const cf_graph* g) {
   return false;
 }
 
+constexpr uint32_t kFcfsMaxC = 256;  // arrival-order kernel: 8 free-time elements per lane
+
 int32_t check_plans(const cf_graph* g, const cf_plans* pl) {
   if (!pl) return CF_ERR_ARG;
   if (pl->n_plans < 1 || pl->max_stages < 1 || pl->max_stages > 8) return CF_ERR_ARG;
   if (!pl->n_stages || !pl->stage_mask || !pl->stage_c) return CF_ERR_ARG;
+  if (g->order_mode)
+    for (uint32_t p = 0; p < pl->n_plans; ++p)
+      for (uint32_t s = 0; s < pl->n_stages[p] && s < pl->max_stages; ++s)
+        if (pl->stage_c[(size_t)p * pl->max_stages + s] > kFcfsMaxC) return CF_ERR_RANGE;
   uint32_t used = 0;
   for (uint32_t t = 0; t < g->n_types; ++t) used |= g->type_mask[t];
   if (pl->max_routes > 4 || (pl->max_routes && (!pl->route_mask || !pl->route_cum))) return CF_ERR_ARG;
@@ -187,6 +194,9 @@ struct Schedule {
   int warps_per_cta = 8;         // 4 or 8 (template choice of both kernels)
   // every stage of every plan has one replica: the call runs on the max-plus scan kernel (cf_scan.cuh)
   bool all_c1 = false;
+  // arrival-order service (R27): the call runs on the warp-per-simulation kernel of cf_fcfs.cuh
+  bool fcfs = false;
+  int fcfs_cpl = 1;              // free-time elements per lane: 32 * cpl >= the largest replica count
   std::vector<uint32_t> plan_topo_v, plan_var_v;  // [P] topology id / stream variant of each plan
   std::vector<uint8_t> topo_pred;                 // fork-join (R25): [topology][type 8][stage 8] predecessor masks
   std::vector<TopoRoutes> topo_routes;            // routing (R26): [topology]
@@ -309,6 +319,14 @@ int32_t build_schedule(const cf_graph* g, const cf_plans* pl, uint32_t R,
   // thread per simulation when the call has few simulations (config 0: 32 per call), 5.7x slower
   // when there are enough to fill the GPU with threads (measured crossover near 9 000 simulations).
   if (!only_plan && (uint64_t)P * R * g->n_trials > 8192ull) sc.all_c1 = false;
+  sc.fcfs = g->order_mode != 0;
+  if (sc.fcfs) {
+    uint32_t cmax_rep = 1;
+    for (uint32_t p = only_plan ? *only_plan : 0; p < (only_plan ? *only_plan + 1 : P); ++p)
+      for (uint32_t st = 0; st < pl->n_stages[p]; ++st) cmax_rep = std::max<uint32_t>(cmax_rep, pl->stage_c[(size_t)p * MS + st]);
+    sc.fcfs_cpl = cmax_rep <= 32 ? 1 : (cmax_rep <= 64 ? 2 : (cmax_rep <= 128 ? 4 : 8));
+    sc.all_c1 = false;  // the scan kernel serves in index order
+  }
   if (graph_has_cpu(g) || g->join_mode || pl->max_routes) sc.all_c1 = false;  // the idle/busy rule (R24) is not max-plus linear; fork-join (R25) runs on the 64-bit kernel
   if (kernel_mode == CF_KERNEL_SCAN && !sc.all_c1) return CF_ERR_ARG;  // one replica everywhere, <= 8192 simulations
   // the forced thread-per-simulation modes (cf_debug.h) keep that path; so do traces unless asked otherwise
@@ -646,6 +664,7 @@ cudaError_t launch_sims32(KParams kp, const Schedule& sc, uint32_t n_trials, cud
 // at 2^30. Anything else runs on the 64-bit kernel alone.
 bool fast_path_ok(const cf_graph* g, uint32_t kernel_mode) {
   if (kernel_mode == CF_KERNEL_WIDE64) return false;
+  if (g->order_mode) return false;  // arrival order (R27) has its own kernel
   if (graph_has_cpu(g) || g->join_mode) return false;  // CPU-GPU overlap (R24) and fork-join (R25) run on the 64-bit kernel
   int64_t worst = 0;
   for (uint32_t i = 0; i < g->n_comp; ++i) {
@@ -671,7 +690,50 @@ cudaError_t launch_scan(KParams kp, const Schedule& sc, uint32_t n_trials, cudaS
   return launch_scan_k(sc.cmax, kp, (uint32_t)blocks, sc.R, (uint32_t)n_sims, st);
 }
 
-cudaError_t launch_pass(KParams kp, const Schedule& sc, uint32_t n_trials, bool fast, cudaStream_t st) {
+// ---- arrival-order kernel (cf_fcfs.cuh): scratch of the simulations in flight, after `used` bytes of workspace
+constexpr uint32_t kFcfsAskSlots = 148 * 8, kFcfsMaxSlots = 148 * 32;
+
+FcfsParams fcfs_slot_layout(const cf_graph* g) {
+  FcfsParams fp;
+  std::memset(&fp, 0, sizeof(fp));
+  const size_t N = g->n_req;
+  uint32_t n_pad = 2;
+  while (n_pad < N) n_pad <<= 1;
+  fp.n_pad = n_pad;
+  size_t off = align_up(N * 8);
+  fp.off_key = (uint32_t)off; off += align_up((size_t)n_pad * 8);
+  fp.off_idx = (uint32_t)off; off += align_up((size_t)n_pad * 4);
+  fp.off_sv = (uint32_t)off;  off += align_up(N * 4);
+  fp.off_scpu = (uint32_t)off;
+  if (graph_has_cpu(g)) off += align_up(N * 4);
+  fp.slot_bytes = off;
+  fp.only_plan = 0xffffffffu;
+  return fp;
+}
+
+int32_t fcfs_place(const cf_graph* g, uint8_t* ws, size_t used, size_t ws_bytes, uint64_t n_sims, uint32_t R, FcfsParams* out) {
+  FcfsParams fp = fcfs_slot_layout(g);
+  const size_t off = align_up(used);
+  if (off >= ws_bytes) return CF_ERR_WORKSPACE;
+  const uint64_t fit = (ws_bytes - off) / fp.slot_bytes;
+  const uint64_t slots = std::min<uint64_t>(std::min<uint64_t>(fit, n_sims), kFcfsMaxSlots);
+  if (slots < 1 || n_sims > 0xffffffffull) return CF_ERR_WORKSPACE;
+  fp.scratch = ws + off;
+  fp.n_slots = (uint32_t)slots;
+  fp.n_sims = (uint32_t)n_sims;
+  fp.R = R;
+  *out = fp;
+  return CF_OK;
+}
+
+cudaError_t launch_pass(KParams kp, const Schedule& sc, uint32_t n_trials, bool fast, cudaStream_t st,
+                        const FcfsParams* fcfs = nullptr) {
+  if (sc.fcfs) {  // arrival-order service (R27): one warp per simulation, stage by stage
+    if (!fcfs) return cudaErrorInvalidValue;
+    kp.k_launch = n_trials;
+    ++g_launch_count;
+    return launch_fcfs_k(sc.cmax, kp.has_cpu != 0, sc.fcfs_cpl, kp, *fcfs, st);
+  }
   if (sc.all_c1) return launch_scan(kp, sc, n_trials, st);  // one replica everywhere: max-plus scan
   if (!fast) {
     kp.fixup = 0;
@@ -1008,7 +1070,7 @@ struct KeyBuilder {
     for (uint32_t j = 0; j < g->n_tabs; ++j) tab(g->tabs[j]);
     tab(g->arr_tab);
     if (g->n_edges) put(g->edges, 2 * g->n_edges);
-    val(g->join_mode);
+    val(g->join_mode); val(g->order_mode);
     val((uint32_t)(g->cpu_tab != nullptr));
     if (g->cpu_tab) put(g->cpu_tab, (size_t)g->n_comp * g->n_types * 2);
   }
@@ -1068,7 +1130,7 @@ int32_t eval_impl(const EvalArgs& a) {
   if (int32_t rc = check_graph(a.g)) return rc;
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rates_dev || a.R < 1 || !a.slo || !a.slo->L_us || !a.out_counts) return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode || a.pl->max_routes)) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode || a.pl->max_routes || a.g->order_mode)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, a.R))) return rc;
   KeyBuilder kb;
   kb.val((uint32_t)1); kb.graph(a.g); kb.plans(a.pl); kb.routes(a.pl, a.g->n_types); kb.val(a.R); kb.val(a.seed); kb.put(a.slo->L_us, a.g->n_types * 8);
@@ -1104,7 +1166,12 @@ int32_t eval_impl(const EvalArgs& a) {
   kp.out_dep_sum = a.out_dep_sum;
   kp.out_makespan = a.out_makespan;
   kp.flags = ws + flags_off;
-  return cuda_rc(launch_pass(kp, p.sc, a.g->n_trials, p.fast, a.st));
+  FcfsParams fp;
+  if (p.sc.fcfs)
+    if (int32_t rc = fcfs_place(a.g, ws, flags_off + (size_t)a.pl->n_plans * a.R * a.g->n_trials, a.ws_bytes,
+                                (uint64_t)a.pl->n_plans * a.R * a.g->n_trials, a.R, &fp))
+      return rc;
+  return cuda_rc(launch_pass(kp, p.sc, a.g->n_trials, p.fast, a.st, &fp));
 }
 
 struct BisectArgs {
@@ -1121,7 +1188,7 @@ int32_t bisect_impl(const BisectArgs& a) {
   if (int32_t rc = check_plans(a.g, a.pl)) return rc;
   if (!a.rate_hi_dev || !a.slo || !a.slo->L_us || !a.slo->att_num || !a.slo->att_den || !a.out_rate || !a.out_goodput)
     return CF_ERR_ARG;
-  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode || a.pl->max_routes)) return CF_ERR_ARG;
+  if (a.stream_records && (a.g->n_comp > 6 || a.n_variants < 1 || graph_has_cpu(a.g) || a.g->join_mode || a.pl->max_routes || a.g->order_mode)) return CF_ERR_ARG;
   if (int32_t rc = check_workspace(a.ws, a.ws_bytes, cf_workspace_bytes(a.g, a.pl, 1))) return rc;
   const uint32_t P = a.pl->n_plans, K = a.g->n_trials, T = a.g->n_types;
   KeyBuilder kb;
@@ -1138,7 +1205,9 @@ int32_t bisect_impl(const BisectArgs& a) {
     uint32_t depth = a.opt.bisect_depth;
     if (depth == 0) {
       depth = 1;
-      while (depth < kMaxSpecDepth && (uint64_t)P * K * ((1u << depth) - 1u) < 90000ull) ++depth;
+      // (the arrival-order kernel spends a warp per simulation: 148 x 32 of them fill the GPU)
+      const uint64_t want = a.g->order_mode ? (uint64_t)kFcfsMaxSlots : 90000ull;
+      while (depth < kMaxSpecDepth && (uint64_t)P * K * ((1u << depth) - 1u) < want) ++depth;
     }
     p.depth = std::min(depth, std::max(1u, a.n_steps));
     if (int32_t rc = build_schedule(a.g, a.pl, (1u << p.depth) - 1u, a.plan_variant, a.stream_records ? a.n_variants : 1,
@@ -1186,14 +1255,17 @@ int32_t bisect_impl(const BisectArgs& a) {
   kp.rates = bs.tree;
   kp.out_counts = bs.probe;
   kp.flags = ws + flags_off;
+  FcfsParams fp;
+  if (sc.fcfs)
+    if (int32_t rc = fcfs_place(a.g, ws, flags_off + (size_t)P * R * K, a.ws_bytes, (uint64_t)P * R * K, R, &fp)) return rc;
   const uint32_t nb = (P + 127) / 128;
   bisect_init_kernel<<<nb, 128, 0, a.st>>>(bs, a.rate_hi_dev, P, (uint32_t)per_plan, std::min(depth, a.n_steps));
   ++g_launch_count;
   for (uint32_t step = 0; step < a.n_steps; step += depth) {
     const uint32_t levels = std::min(depth, a.n_steps - step);
     const uint32_t next_levels = std::min(depth, a.n_steps - step - levels);
-    if (!fast || sc.all_c1) {
-      if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, false, a.st))) return rc;
+    if (!fast || sc.all_c1 || sc.fcfs) {
+      if (int32_t rc = cuda_rc(launch_pass(kp, sc, K, false, a.st, &fp))) return rc;
     } else {
       if (int32_t rc = cuda_rc(launch_sims32(kp, sc, K, a.st))) return rc;
       bisect_triage_kernel<<<nb, 128, 0, a.st>>>(bs, P, K, T, reinterpret_cast<const uint32_t*>(ws + att_off),
@@ -1237,8 +1309,10 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   n += align_up(P * Rb * K * T * 2 * 4) + align_up(P * K * T * 2 * 4) + kAlign;  // probe + at_lo counts
   n += align_up(K * T * 2 * 4) + kAlign;                    // trace scratch
   n += align_up(P * R * K) + kAlign;                        // 32-bit window flags
-  const size_t chunks = ((size_t)g->n_req + 31) / 32;
-  (void)chunks;
+  if (g->order_mode) {  // arrival-order kernel: scratch of the simulations in flight
+    const FcfsParams fp = fcfs_slot_layout(g);
+    n += kAlign + (size_t)fp.slot_bytes * std::min<uint64_t>((uint64_t)P * R * K, kFcfsAskSlots);
+  }
   return n + 4 * kAlign;
 }
 
@@ -1413,6 +1487,12 @@ int32_t cf_trace_sim_opt(const cf_options* opt_in, const cf_graph* g, const cf_p
   kp.tr_type = out_type;
   kp.tr_plan = plan;
   kp.trial_base = trial;
+  if (sc.fcfs) {  // R27: the traced simulation alone, on one warp
+    FcfsParams fp;
+    if (int32_t rc = fcfs_place(g, ws, blob.bytes.size(), workspace_bytes, 1, 1, &fp)) return rc;
+    fp.only_plan = plan;
+    return cuda_rc(launch_pass(kp, sc, 1, false, st, &fp));
+  }
   if (sc.all_c1) return cuda_rc(launch_scan(kp, sc, 1, st));
   if (fast) {
     if (int32_t rc = cuda_rc(launch_sims32(kp, sc, 1, st))) return rc;

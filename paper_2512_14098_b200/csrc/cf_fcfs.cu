@@ -1,0 +1,29 @@
+// cf_fcfs.cu -- instantiations and launches of the arrival-order kernel (cf_fcfs.cuh).
+#include "cf_launch.h"
+#include "cf_fcfs.cuh"
+
+namespace cfk {
+
+namespace {
+template <int CMAX, bool HAS_CPU>
+cudaError_t launch_cpl(int cpl, const KParams& kp, const FcfsParams& fp, cudaStream_t st) {
+  const uint32_t blocks = (fp.n_slots + kFcfsWarps - 1) / kFcfsWarps;
+  const dim3 b(kFcfsWarps * 32);
+  switch (cpl) {
+    case 1: cf_fcfs_kernel<CMAX, HAS_CPU, 1><<<blocks, b, 0, st>>>(kp, fp); break;
+    case 2: cf_fcfs_kernel<CMAX, HAS_CPU, 2><<<blocks, b, 0, st>>>(kp, fp); break;
+    case 4: cf_fcfs_kernel<CMAX, HAS_CPU, 4><<<blocks, b, 0, st>>>(kp, fp); break;
+    case 8: cf_fcfs_kernel<CMAX, HAS_CPU, 8><<<blocks, b, 0, st>>>(kp, fp); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+}  // namespace
+
+cudaError_t launch_fcfs_k(int cmax, bool has_cpu, int cpl, const KParams& kp, const FcfsParams& fp, cudaStream_t st) {
+  if (fp.n_slots == 0) return cudaErrorInvalidValue;
+  if (cmax == 8) return has_cpu ? launch_cpl<8, true>(cpl, kp, fp, st) : launch_cpl<8, false>(cpl, kp, fp, st);
+  return has_cpu ? launch_cpl<6, true>(cpl, kp, fp, st) : launch_cpl<6, false>(cpl, kp, fp, st);
+}
+
+}  // namespace cfk

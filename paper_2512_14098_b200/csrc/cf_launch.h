@@ -30,4 +30,7 @@ CF_K32_DECL(8, 8)
 cudaError_t launch_scan_k(int cmax, const KParams& kp, uint32_t blocks, uint32_t R, uint32_t n_sims,
                           cudaStream_t st);
 
+// arrival-order kernel (cf_fcfs.cu): cmax in {6, 8}, cpl = free-time elements per lane in {1, 2, 4, 8}
+cudaError_t launch_fcfs_k(int cmax, bool has_cpu, int cpl, const KParams& kp, const FcfsParams& fp, cudaStream_t st);
+
 }  // namespace cfk

@@ -501,6 +501,39 @@ def measure_phases(torch, cf, stream, n_plans=1_000_000):
                              "plans, planner host CPU not stated"}
 
 
+def measure_fidelity(torch, cf, stream):
+    """Sub-record: arrival-order service (cf_graph.order_mode = 1, R27) on configs[1] at
+    full size next to the index-order run of the same call: milliseconds through the C ABI (best of
+    3) and the largest per-type attainment difference between the two disciplines over all (plan,
+    rate). Parity of this variant with the oracle: tests/test_gpu_fcfs.py."""
+    w = W.config1_mllm()
+    g, pl = w.graph, w.plans
+    out = {"workload": workload_name(1)}
+    for mode, name in ((0, "index_order"), (1, "arrival_order")):
+        g.order_mode = mode
+        ws = cf.alloc_workspace(g, pl, w.rate_mrps.shape[1])
+        best = None
+        for _ in range(3):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            res = cf.cf_eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, workspace=ws, stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
+        counts = cf.to_numpy_u32(res["counts"])
+        upd = int(W.count_updates(g, pl, counts))
+        out[name] = {"ms": best, "updates_per_s": upd / (best * 1e-3), "workspace_gib": ws.numel() / 2**30}
+        if mode == 1:
+            out["attainment_shift_vs_index_order"] = float(np.abs(
+                counts[..., 1].sum(axis=2) / np.maximum(counts[..., 0].sum(axis=2), 1) - out.pop("_att0")).max())
+        else:
+            out["_att0"] = counts[..., 1].sum(axis=2) / np.maximum(counts[..., 0].sum(axis=2), 1)
+        del ws
+    g.order_mode = 0
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -563,6 +596,10 @@ def main():
                 config["phases"] = measure_phases(torch, cf, stream)
             except Exception as e:  # noqa: BLE001
                 config["phases"] = {"error": str(e)}
+            try:
+                config["fidelity"] = measure_fidelity(torch, cf, stream)
+            except Exception as e:  # noqa: BLE001
+                config["fidelity"] = {"error": str(e)}
         if per:
             config["per_config"] = {f"cfg{c}": {k: v for k, v in r.items() if k != "stream_materialise"}
                                     for c, r in per.items()}

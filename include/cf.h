@@ -94,7 +94,7 @@ typedef struct {
                                   textbook FCFS at every node (R27). Runs on
                                   the arrival-order kernel: one warp per simulation, stage by stage, over
                                   40 N bytes of workspace per simulation in flight (cf_workspace_bytes asks for
-                                  up to 1184 of them; a larger workspace runs up to 4736 at once). Replicas
+                                  up to 2368 of them; a larger workspace runs up to 4736 at once). Replicas
                                   per stage <= 256; path routing only (join_mode = 0); no stream.           */
 } cf_graph;
 

@@ -691,18 +691,15 @@ cudaError_t launch_scan(KParams kp, const Schedule& sc, uint32_t n_trials, cudaS
 }
 
 // ---- arrival-order kernel (cf_fcfs.cuh): scratch of the simulations in flight, after `used` bytes of workspace
-constexpr uint32_t kFcfsAskSlots = 148 * 8, kFcfsMaxSlots = 148 * 32;
+constexpr uint32_t kFcfsAskSlots = 148 * 16, kFcfsMaxSlots = 148 * 32;
 
 FcfsParams fcfs_slot_layout(const cf_graph* g) {
   FcfsParams fp;
   std::memset(&fp, 0, sizeof(fp));
   const size_t N = g->n_req;
-  uint32_t n_pad = 2;
-  while (n_pad < N) n_pad <<= 1;
-  fp.n_pad = n_pad;
   size_t off = align_up(N * 8);
-  fp.off_key = (uint32_t)off; off += align_up((size_t)n_pad * 8);
-  fp.off_idx = (uint32_t)off; off += align_up((size_t)n_pad * 4);
+  for (int b = 0; b < 2; ++b) { fp.off_key[b] = (uint32_t)off; off += align_up(N * 8); }
+  for (int b = 0; b < 2; ++b) { fp.off_idx[b] = (uint32_t)off; off += align_up(N * 4); }
   fp.off_sv = (uint32_t)off;  off += align_up(N * 4);
   fp.off_scpu = (uint32_t)off;
   if (graph_has_cpu(g)) off += align_up(N * 4);
@@ -711,10 +708,27 @@ FcfsParams fcfs_slot_layout(const cf_graph* g) {
   return fp;
 }
 
-int32_t fcfs_place(const cf_graph* g, uint8_t* ws, size_t used, size_t ws_bytes, uint64_t n_sims, uint32_t R, FcfsParams* out) {
+// bytes of the request records and segment totals of n_trials trials (upper bound over the record formats)
+size_t fcfs_record_bytes(const cf_graph* g, uint32_t n_trials, uint32_t* n_seg_out, uint32_t* cps_out) {
+  const uint32_t n_chunks = (g->n_req + 31u) / 32u;
+  uint32_t n_seg = std::max(1u, std::min(n_chunks, 4096u / std::max(1u, std::min(n_trials, 4096u))));
+  const uint32_t cps = (n_chunks + n_seg - 1) / n_seg;
+  n_seg = (n_chunks + cps - 1) / cps;
+  if (n_seg_out) *n_seg_out = n_seg;
+  if (cps_out) *cps_out = cps;
+  return align_up((size_t)n_trials * g->n_req * 5 * 16) + align_up((size_t)n_trials * n_seg * 8);
+}
+
+// workspace after `used` bytes: records + segment totals of n_trials trials, then the scratch slots
+int32_t fcfs_place(const cf_graph* g, uint8_t* ws, size_t used, size_t ws_bytes, uint32_t n_trials, uint64_t n_sims,
+                   uint32_t R, FcfsParams* out) {
   FcfsParams fp = fcfs_slot_layout(g);
-  const size_t off = align_up(used);
-  if (off >= ws_bytes) return CF_ERR_WORKSPACE;
+  size_t off = align_up(used);
+  const size_t rec_bytes = fcfs_record_bytes(g, n_trials, &fp.n_seg, &fp.chunks_per_seg);
+  if (off + rec_bytes >= ws_bytes) return CF_ERR_WORKSPACE;
+  fp.records = reinterpret_cast<uint4*>(ws + off);
+  fp.seg_tot = reinterpret_cast<unsigned long long*>(ws + off + align_up((size_t)n_trials * g->n_req * 5 * 16));
+  off += rec_bytes;
   const uint64_t fit = (ws_bytes - off) / fp.slot_bytes;
   const uint64_t slots = std::min<uint64_t>(std::min<uint64_t>(fit, n_sims), kFcfsMaxSlots);
   if (slots < 1 || n_sims > 0xffffffffull) return CF_ERR_WORKSPACE;
@@ -724,6 +738,13 @@ int32_t fcfs_place(const cf_graph* g, uint8_t* ws, size_t used, size_t ws_bytes,
   fp.R = R;
   *out = fp;
   return CF_OK;
+}
+
+// the request records of the call's trials: drawn once, before the first pass
+cudaError_t launch_fcfs_records(KParams kp, const Schedule& sc, uint32_t n_trials, const FcfsParams& fp, cudaStream_t st) {
+  kp.k_launch = n_trials;
+  g_launch_count += 2;
+  return launch_fcfs_records_k(sc.cmax, kp.has_cpu != 0, kp, fp, st);
 }
 
 cudaError_t launch_pass(KParams kp, const Schedule& sc, uint32_t n_trials, bool fast, cudaStream_t st,
@@ -1168,9 +1189,12 @@ int32_t eval_impl(const EvalArgs& a) {
   kp.flags = ws + flags_off;
   FcfsParams fp;
   if (p.sc.fcfs)
-    if (int32_t rc = fcfs_place(a.g, ws, flags_off + (size_t)a.pl->n_plans * a.R * a.g->n_trials, a.ws_bytes,
+  {
+    if (int32_t rc = fcfs_place(a.g, ws, flags_off + (size_t)a.pl->n_plans * a.R * a.g->n_trials, a.ws_bytes, a.g->n_trials,
                                 (uint64_t)a.pl->n_plans * a.R * a.g->n_trials, a.R, &fp))
       return rc;
+    if (int32_t rc = cuda_rc(launch_fcfs_records(kp, p.sc, a.g->n_trials, fp, a.st))) return rc;
+  }
   return cuda_rc(launch_pass(kp, p.sc, a.g->n_trials, p.fast, a.st, &fp));
 }
 
@@ -1256,8 +1280,10 @@ int32_t bisect_impl(const BisectArgs& a) {
   kp.out_counts = bs.probe;
   kp.flags = ws + flags_off;
   FcfsParams fp;
-  if (sc.fcfs)
-    if (int32_t rc = fcfs_place(a.g, ws, flags_off + (size_t)P * R * K, a.ws_bytes, (uint64_t)P * R * K, R, &fp)) return rc;
+  if (sc.fcfs) {
+    if (int32_t rc = fcfs_place(a.g, ws, flags_off + (size_t)P * R * K, a.ws_bytes, K, (uint64_t)P * R * K, R, &fp)) return rc;
+    if (int32_t rc = cuda_rc(launch_fcfs_records(kp, sc, K, fp, a.st))) return rc;
+  }
   const uint32_t nb = (P + 127) / 128;
   bisect_init_kernel<<<nb, 128, 0, a.st>>>(bs, a.rate_hi_dev, P, (uint32_t)per_plan, std::min(depth, a.n_steps));
   ++g_launch_count;
@@ -1311,7 +1337,8 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   n += align_up(P * R * K) + kAlign;                        // 32-bit window flags
   if (g->order_mode) {  // arrival-order kernel: scratch of the simulations in flight
     const FcfsParams fp = fcfs_slot_layout(g);
-    n += kAlign + (size_t)fp.slot_bytes * std::min<uint64_t>((uint64_t)P * R * K, kFcfsAskSlots);
+    n += 2 * kAlign + fcfs_record_bytes(g, (uint32_t)K, nullptr, nullptr);
+    n += (size_t)fp.slot_bytes * std::min<uint64_t>((uint64_t)P * R * K, kFcfsAskSlots);
   }
   return n + 4 * kAlign;
 }
@@ -1489,8 +1516,9 @@ int32_t cf_trace_sim_opt(const cf_options* opt_in, const cf_graph* g, const cf_p
   kp.trial_base = trial;
   if (sc.fcfs) {  // R27: the traced simulation alone, on one warp
     FcfsParams fp;
-    if (int32_t rc = fcfs_place(g, ws, blob.bytes.size(), workspace_bytes, 1, 1, &fp)) return rc;
+    if (int32_t rc = fcfs_place(g, ws, blob.bytes.size(), workspace_bytes, 1, 1, 1, &fp)) return rc;
     fp.only_plan = plan;
+    if (int32_t rc = cuda_rc(launch_fcfs_records(kp, sc, 1, fp, st))) return rc;
     return cuda_rc(launch_pass(kp, sc, 1, false, st, &fp));
   }
   if (sc.all_c1) return cuda_rc(launch_scan(kp, sc, 1, st));

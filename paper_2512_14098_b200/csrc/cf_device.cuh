@@ -113,17 +113,22 @@ struct KParams {
   const uint8_t* topo_pred;  // join: [topology][type 8][stage 8] bitmask of the stage's predecessor stages
 };
 
-// Arrival-order kernel (cf_fcfs.cuh, R27): one warp per simulation in flight.
-// scratch of one concurrent simulation: x int64[N] | key int64[n_pad] | idx u32[n_pad] | sv i32[N] | scpu i32[N]
+// Arrival-order kernels (cf_fcfs.cuh, R27): one warp per simulation in flight.
+// Request records of the call's trials (drawn once, shared by every simulation of a trial):
+//   records[(trial - trial_base) * N + n] = CompRec<CMAX, HAS_CPU> words with the ABSOLUTE cumulative gap.
+// Scratch of one simulation in flight (byte offsets inside its slot; x at 0):
+//   x int64[N] | key int64[N] x 2 | idx u32[N] x 2 (the radix sort ping-pongs) | sv i32[N] | scpu i32[N]
 struct FcfsParams {
   uint8_t* scratch;
   unsigned long long slot_bytes;
+  uint4* records;
+  unsigned long long* seg_tot;  // [trial][segment] sum of the gaps of a segment of chunks
+  uint32_t n_seg, chunks_per_seg;
   uint32_t n_slots;    // warps (simulations in flight); simulation i runs on warp i mod n_slots
-  uint32_t n_pad;      // power of two >= N
   uint32_t R;          // rates per plan
   uint32_t n_sims;     // P * R * k_launch, or 1 with only_plan
   uint32_t only_plan;  // cf_trace_sim: the one plan to run (R = 1); 0xffffffff = all
-  uint32_t off_key, off_idx, off_sv, off_scpu;  // byte offsets inside a slot (x at 0)
+  uint32_t off_key[2], off_idx[2], off_sv, off_scpu;
 };
 
 // ------------------------------------------------------------------------------------------------

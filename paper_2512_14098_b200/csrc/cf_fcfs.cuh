@@ -4,20 +4,24 @@
 // A stage that serves in ARRIVAL order cannot be advanced request by request: whether request n is
 // next at stage s depends on when later requests get there. But the plan's stages are in topological
 // order and a request only moves forward, so every arrival at stage s is known once stages 0..s-1 are
-// done. One WARP runs one simulation, stage by stage, over scratch arrays in HBM (x[n] = the time at
-// which request n leaves the last stage it has visited so far):
-//   phase 0   the request stream, one request per lane (the producer code of the other kernels, hence
-//             the same draws): x[n] = A_n;
+// done. The request stream of every trial is drawn ONCE per call into HBM records (common random
+// numbers, R4: every simulation of a trial reads the same records; two small kernels, the producer
+// code of the other kernels, hence the same draws). Then one WARP runs one simulation, stage by stage,
+// over scratch arrays in HBM (x[n] = the time at which request n leaves the last stage it has visited):
+//   phase 0   x[n] = A_n;
 //   per stage gather   the visitors of the stage, compacted with ballots: (arrival = x[n] + hop
 //                      delay, n) and, by request, the summed service (and CPU time, R24) at the stage;
-//             sort     the pairs by (arrival, n) -- a bitonic network over the warp's segment, skipped
-//                      when the arrivals are already in order (every first stage);
+//             sort     by arrival, stable in the request index: LSD radix sort of the warp's segment,
+//                      8 bits a pass over the bits in which the keys differ (match.any ranks a chunk
+//                      of 32 keys); skipped when the arrivals are already in order (every first stage);
 //             serve    the Kiefer-Wolfowitz recursion in that order with the LANES AS REPLICAS: the
-//                      sorted free-time vector of the stage lives one element per lane (CPL elements
-//                      per lane for c > 32); replace-min = one ballot (where does the new departure
-//                      go) and one shuffle (everything below it moves down a lane);
-//   last      per-type counts and hits, checksum, makespan from x[n] - A_n (stream drawn once more).
-// All times are absolute int64. Results are bit-identical to the oracle's order_mode = 1.
+//                      sorted free-time vector of the stage lives one element per lane (CPL per lane
+//                      for c > 32); replace-min is F'[e] = min(F[e+1], max(F[e], D)) -- one shuffle, one
+//                      max, one min, no search for the insertion point. A batch of 32 visits whose
+//                      times span less than 2^32 us runs on 32-bit offsets from the batch's first
+//                      arrival (free times before it are clamped to it: exact, they are "idle");
+//   last      per-type counts and hits, checksum, makespan from x[n] - A_n.
+// All times are int64. Results are bit-identical to the oracle's order_mode = 1.
 #pragma once
 #include "cf_device.cuh"
 
@@ -25,49 +29,155 @@ namespace cfk {
 
 constexpr int kFcfsWarps = 4;
 constexpr uint32_t kAll = 0xffffffffu;
+constexpr uint32_t kInf32 = 0xffffffffu;
 
-__device__ __forceinline__ bool pair_greater(int64_t ka, uint32_t ia, int64_t kb, uint32_t ib) {
-  return ka > kb || (ka == kb && ia > ib);
+// ---- the request records of the call's trials -------------------------------------------------------
+// pass 1: gap totals of every segment of chunks_per_seg chunks (Philox block 0 + the arrival table only)
+__global__ void __launch_bounds__(kFcfsWarps * 32)
+cf_fcfs_totals_kernel(const __grid_constant__ KParams prm, const __grid_constant__ FcfsParams fp) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t gw = blockIdx.x * kFcfsWarps + (threadIdx.x >> 5);
+  if (gw >= prm.k_launch * fp.n_seg) return;
+  const uint32_t ti = gw / fp.n_seg, seg = gw % fp.n_seg, trial = prm.trial_base + ti;
+  const uint32_t n_chunks = (prm.N + 31u) / 32u;
+  const uint32_t c0 = seg * fp.chunks_per_seg, c1 = min(c0 + fp.chunks_per_seg, n_chunks);
+  uint64_t total = 0;
+  for (uint32_t ch = c0; ch < c1; ++ch) {
+    const uint32_t n = ch * 32u + lane;
+    if (n < prm.N) {
+      const uint4 b0 = philox4x32_10(n, trial, 0, prm.variant_lo, prm.seed_lo, prm.seed_hi);
+      total += (uint32_t)qtab_sample(prm.qpool, prm.arr_tab, b0.x);
+    }
+  }
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) total += __shfl_xor_sync(kAll, total, d);
+  if (lane == 0) fp.seg_tot[(size_t)ti * fp.n_seg + seg] = total;
 }
 
-// bitonic sort of (key, idx)[0..m_pad) ascending by (key, idx); m_pad a power of two; one warp
-__device__ __forceinline__ void warp_bitonic_sort(int64_t* key, uint32_t* idx, uint32_t m_pad, int lane) {
-  for (uint32_t k = 2; k <= m_pad; k <<= 1) {
-    for (uint32_t j = k >> 1; j > 0; j >>= 1) {
-      for (uint32_t t = lane; t < (m_pad >> 1); t += 32) {
-        const uint32_t i = ((t & ~(j - 1u)) << 1) | (t & (j - 1u)), l = i | j;
-        const bool up = (i & k) == 0u;
-        const int64_t ki = key[i], kl = key[l];
-        const uint32_t ii = idx[i], il = idx[l];
-        if (pair_greater(ki, ii, kl, il) == up) {
-          key[i] = kl; key[l] = ki;
-          idx[i] = il; idx[l] = ii;
-        }
-      }
-      __syncwarp();
+// pass 2: the records of a segment, cumulative gaps made absolute with the totals of the segments before
+template <int CMAX, bool HAS_CPU>
+__global__ void __launch_bounds__(kFcfsWarps * 32)
+cf_fcfs_records_kernel(const __grid_constant__ KParams prm, const __grid_constant__ FcfsParams fp) {
+  constexpr int kW = CompRec<CMAX, HAS_CPU>::kWords;
+  __shared__ __align__(16) uint4 rec_buf[kFcfsWarps][32 * kW];
+  __shared__ uint64_t chunk_tot[kFcfsWarps];
+  __shared__ uint32_t cnt_dummy[8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t gw = blockIdx.x * kFcfsWarps + warp;
+  if (gw >= prm.k_launch * fp.n_seg) return;
+  const uint32_t ti = gw / fp.n_seg, seg = gw % fp.n_seg, trial = prm.trial_base + ti;
+  const uint32_t n_chunks = (prm.N + 31u) / 32u;
+  const uint32_t c0 = seg * fp.chunks_per_seg, c1 = min(c0 + fp.chunks_per_seg, n_chunks);
+  uint64_t base = 0;
+  for (uint32_t s = lane; s < seg; s += 32) base += fp.seg_tot[(size_t)ti * fp.n_seg + s];
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) base += __shfl_xor_sync(kAll, base, d);
+  for (uint32_t ch = c0; ch < c1; ++ch) {
+    produce_chunk_philox<CMAX, HAS_CPU>(prm, ch * 32u, trial, prm.variant_lo, rec_buf[warp], &chunk_tot[warp], cnt_dummy, lane);
+    __syncwarp();
+    const uint32_t n = ch * 32u + lane;
+    if (n < prm.N) {
+      const uint4* src = rec_buf[warp] + lane * kW;
+      uint4* dst = fp.records + ((size_t)ti * prm.N + n) * kW;
+      uint4 w0 = src[0];
+      const uint64_t cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + base;
+      w0.x = (uint32_t)cu;
+      w0.y = (uint32_t)(cu >> 32) | (w0.y & 0xff000000u);
+      dst[0] = w0;
+#pragma unroll
+      for (int w = 1; w < kW; ++w) dst[w] = src[w];
     }
+    base += chunk_tot[warp];
+    __syncwarp();
   }
 }
 
-// One replace-min of the Kiefer-Wolfowitz recursion on a sorted free-time vector spread over the
-// warp: element e = j * 32 + lane lives in F[j] of that lane; elements >= c hold +inf.
-// Arrival a, service S, CPU time Sc (R24: paid when the earliest-free replica is idle at a).
-template <int CPL>
-__device__ __forceinline__ int64_t kw_step(int64_t (&F)[CPL], int64_t a, int32_t S, int32_t Sc, int lane) {
-  const int64_t f0 = __shfl_sync(kAll, F[0], 0);
-  const int64_t D = (f0 <= a) ? a + (int64_t)Sc + (int64_t)S : f0 + (int64_t)S;
-  uint32_t cnt = 0;
+// ---- stable LSD radix sort of (key, idx)[0..M) by the key bits [0, bits): one warp, 8 bits a pass --------
+// Returns the buffer (0 / 1) that holds the sorted pairs. cnt: 256 shared counters of this warp.
+__device__ __forceinline__ int warp_radix_sort(int64_t* const (&key)[2], uint32_t* const (&idx)[2], uint32_t M,
+                                               uint32_t bits, uint32_t* cnt, int lane) {
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  int cur = 0;
+  for (uint32_t shift = 0; shift < bits; shift += 8) {
+    const int64_t* ks = key[cur];
+    const uint32_t* is = idx[cur];
+    int64_t* kd = key[cur ^ 1];
+    uint32_t* id = idx[cur ^ 1];
 #pragma unroll
-  for (int j = 0; j < CPL; ++j) cnt += __popc(__ballot_sync(kAll, F[j] <= D));
-  const uint32_t q = cnt - 1u;  // D's place once the minimum is gone (F[0] <= D always)
+    for (int k = 0; k < 8; ++k) cnt[lane * 8 + k] = 0;
+    __syncwarp();
+    // (every loop below loads the next chunk of 32 before it works on the current one: the segment
+    //  streams from HBM and a warp has nothing else to hide the round trip with)
+    int64_t k_nx = lane < M ? ks[lane] : 0;
+    for (uint32_t base = 0; base < M; base += 32) {  // histogram of the digit
+      const uint32_t i = base + lane;
+      const bool valid = i < M;
+      const int64_t k = k_nx;
+      if (i + 32 < M) k_nx = ks[i + 32];
+      const uint32_t d = valid ? (uint32_t)((uint64_t)k >> shift) & 255u : 0x100u + lane;
+      const uint32_t m = __match_any_sync(kAll, d);
+      if (valid && (m & lt_mask) == 0u) cnt[d] += __popc(m);  // the lowest lane of each digit group
+      __syncwarp();
+    }
+    {  // exclusive scan of the 256 counters, 8 per lane
+      uint32_t v[8], s = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) { v[k] = cnt[lane * 8 + k]; s += v[k]; }
+      uint32_t incl = s;
+#pragma unroll
+      for (int dd = 1; dd < 32; dd <<= 1) {
+        const uint32_t o = __shfl_up_sync(kAll, incl, dd);
+        if (lane >= dd) incl += o;
+      }
+      uint32_t run = incl - s;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) { cnt[lane * 8 + k] = run; run += v[k]; }
+    }
+    __syncwarp();
+    k_nx = lane < M ? ks[lane] : 0;
+    uint32_t i_nx = lane < M ? is[lane] : 0;
+    for (uint32_t base = 0; base < M; base += 32) {  // stable scatter, a chunk of 32 at a time
+      const uint32_t i = base + lane;
+      const bool valid = i < M;
+      const int64_t k = k_nx;
+      const uint32_t ix = i_nx;
+      if (i + 32 < M) { k_nx = ks[i + 32]; i_nx = is[i + 32]; }
+      const uint32_t d = valid ? (uint32_t)((uint64_t)k >> shift) & 255u : 0x100u + lane;
+      const uint32_t m = __match_any_sync(kAll, d);
+      const uint32_t off = valid ? cnt[d] : 0u;
+      __syncwarp();
+      if (valid && (m & lt_mask) == 0u) cnt[d] = off + __popc(m);
+      __syncwarp();
+      if (valid) {
+        const uint32_t pos = off + __popc(m & lt_mask);
+        kd[pos] = k;
+        id[pos] = ix;
+      }
+    }
+    __syncwarp();
+    cur ^= 1;
+  }
+  return cur;
+}
+
+// ---- Kiefer-Wolfowitz on a sorted free-time vector spread over the warp ----------------------------------
+// Element e = j * 32 + lane lives in F[j] of that lane; elements >= c hold +inf. One visit with arrival
+// a, service S, CPU time Sc (R24: paid when the earliest-free replica is idle at a): departure D, then
+// the minimum leaves and D enters: F'[e] = min(F[e+1], max(F[e], D)) (F sorted, F[0] <= D).
+template <int CPL, bool HAS_CPU, typename TT>
+__device__ __forceinline__ TT kw_visit(TT (&F)[CPL], TT a, uint32_t S, uint32_t Sc, TT inf, int lane) {
+  const TT f0 = __shfl_sync(kAll, F[0], 0);
+  TT D;
+  if (HAS_CPU) D = (f0 <= a) ? a + (TT)Sc + (TT)S : f0 + (TT)S;
+  else D = (f0 > a ? f0 : a) + (TT)S;
 #pragma unroll
   for (int j = 0; j < CPL; ++j) {
-    int64_t next = __shfl_sync(kAll, F[j], (lane + 1) & 31);
-    int64_t wrap = kInf;
+    TT next = __shfl_sync(kAll, F[j], (lane + 1) & 31);
+    TT wrap = inf;
     if (j + 1 < CPL) wrap = __shfl_sync(kAll, F[j + 1 < CPL ? j + 1 : j], 0);
     if (lane == 31) next = wrap;
-    const uint32_t e = (uint32_t)(j * 32 + lane);
-    F[j] = e < q ? next : (e == q ? D : F[j]);
+    const TT up = F[j] > D ? F[j] : D;
+    F[j] = next < up ? next : up;
   }
   return D;
 }
@@ -77,16 +187,14 @@ __global__ void __launch_bounds__(kFcfsWarps * 32)
 cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ FcfsParams fp) {
   constexpr int kW = CompRec<CMAX, HAS_CPU>::kWords;
   constexpr int kB = CompRec<CMAX, HAS_CPU>::kBase;
-  __shared__ __align__(16) uint4 rec_buf[kFcfsWarps][32 * kW];
-  __shared__ uint64_t chunk_tot[kFcfsWarps];
-  __shared__ uint32_t cnt_dummy[8];
+  __shared__ uint32_t cnt_s[kFcfsWarps][256];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t wid = blockIdx.x * kFcfsWarps + warp;
   if (wid >= fp.n_slots) return;  // nothing below synchronises the block
   uint8_t* slot_mem = fp.scratch + (size_t)wid * fp.slot_bytes;
   int64_t* xs = reinterpret_cast<int64_t*>(slot_mem);
-  int64_t* key = reinterpret_cast<int64_t*>(slot_mem + fp.off_key);
-  uint32_t* idx = reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx);
+  int64_t* const key[2] = {reinterpret_cast<int64_t*>(slot_mem + fp.off_key[0]), reinterpret_cast<int64_t*>(slot_mem + fp.off_key[1])};
+  uint32_t* const idx[2] = {reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[0]), reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[1])};
   int32_t* sv = reinterpret_cast<int32_t*>(slot_mem + fp.off_sv);
   int32_t* scpu = reinterpret_cast<int32_t*>(slot_mem + fp.off_scpu);
   const int64_t delay = prm.edge_delay;
@@ -100,7 +208,6 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
     const TopoDesc topo = prm.topos[topo_id];
     const uint32_t rate = prm.rates[pr];
     const size_t slot = (size_t)pr * prm.K + trial;
-    const uint32_t variant = prm.variant_lo;
     bool rate_bad = false, skip = false;
     uint32_t period = 1;
     if (rate < 1u || rate > 1000000000u) {
@@ -109,30 +216,29 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
       period = (1000000000u + rate / 2u) / rate;
     }
     uint32_t my_cnt = 0, my_hits = 0;  // lane t: requests / hits of type t
-    uint64_t dep_sum = 0, last_cu = 0;
+    uint64_t dep_sum = 0;
     int64_t makespan = 0;
     bool bad = rate_bad;
+    const uint4* recs = fp.records + (size_t)(trial - prm.trial_base) * prm.N * kW;
 
-    // one chunk of the request stream: this lane's request n0 + lane (type, visited stages, services)
+    // this lane's request n0 + lane: type, visited stages, A_n, services
     struct Req { uint32_t t, vm; uint64_t cu; int32_t svc[8]; int32_t cpu[8]; bool valid; };
-    uint64_t cu_base = 0;
-    auto draw = [&](uint32_t n0) {
+    auto load = [&](uint32_t n0, bool want_svc) {
       Req r;
-      produce_chunk_philox<CMAX, HAS_CPU>(prm, n0, trial, variant, rec_buf[warp], &chunk_tot[warp], cnt_dummy, lane);
-      __syncwarp();
-      const uint4* src = rec_buf[warp] + lane * kW;
-      const uint4 w0 = src[0], w1 = src[1];
-      uint4 w2 = make_uint4(0, 0, 0, 0);
-      if (CMAX > 6) w2 = src[2];
       r.valid = n0 + lane < prm.N;
-      r.cu = (((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x) + cu_base;
+      const uint4* src = recs + (size_t)min(n0 + lane, prm.N - 1u) * kW;
+      const uint4 w0 = __ldg(src);
+      uint4 w1 = make_uint4(0, 0, 0, 0), w2 = w1;
+      if (want_svc) w1 = __ldg(src + 1);
+      if (CMAX > 6) w2 = __ldg(src + 2);
+      r.cu = ((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x;
       r.t = w0.y >> 24;
       r.svc[0] = (int32_t)w0.z; r.svc[1] = (int32_t)w0.w; r.svc[2] = (int32_t)w1.x; r.svc[3] = (int32_t)w1.y;
       r.svc[4] = (int32_t)w1.z; r.svc[5] = (int32_t)w1.w; r.svc[6] = (int32_t)w2.x; r.svc[7] = (int32_t)w2.y;
 #pragma unroll
       for (int i = 0; i < 8; ++i) r.cpu[i] = 0;
-      if (HAS_CPU) {
-        const uint4 c0 = src[kB], c1 = src[kB + 1];
+      if (HAS_CPU && want_svc) {
+        const uint4 c0 = __ldg(src + kB), c1 = __ldg(src + kB + 1);
         r.cpu[0] = (int32_t)c0.x; r.cpu[1] = (int32_t)c0.y; r.cpu[2] = (int32_t)c0.z; r.cpu[3] = (int32_t)c0.w;
         r.cpu[4] = (int32_t)c1.x; r.cpu[5] = (int32_t)c1.y; r.cpu[6] = (int32_t)c1.z; r.cpu[7] = (int32_t)c1.w;
       }
@@ -142,33 +248,40 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
 #pragma unroll
       for (int s = 0; s < 8; ++s)
         if (s < topo.n_stages && (topo.mask[s] & tm) && ((rmask >> s) & 1u)) r.vm |= 1u << s;
-      cu_base += chunk_tot[warp];
-      __syncwarp();
       return r;
     };
 
-    if (!skip && !bad) {
-      // ---- phase 0: x[n] = A_n -------------------------------------------------------------------
-      cu_base = 0;
-      for (uint32_t n0 = 0; n0 < prm.N; n0 += 32) {
-        const Req r = draw(n0);
-        const int n_here = (int)min(32u, prm.N - n0);
-        last_cu = __shfl_sync(kAll, r.cu, n_here - 1);
-        if (r.valid) xs[n0 + lane] = (int64_t)((r.cu * (uint64_t)period + 32768ull) >> 16);
-      }
+    if (!skip && !bad) {  // R17: the arrival horizon CU_N * period + 2^15 must stay below 2^62
+      const uint4 wl = __ldg(recs + (size_t)(prm.N - 1u) * kW);
+      const uint64_t last_cu = ((uint64_t)(wl.y & 0x00ffffffu) << 32) | wl.x;
       const uint64_t hi = __umul64hi(last_cu, (uint64_t)period);
       const uint64_t lo = last_cu * (uint64_t)period;
-      if (hi != 0 || lo >= (1ull << 62) - 32768ull) bad = true;  // R17
+      if (hi != 0 || lo >= (1ull << 62) - 32768ull) bad = true;
     }
     if (!skip && !bad) {
+      // ---- phase 0: x[n] = A_n -------------------------------------------------------------------
+#pragma unroll 4
+      for (uint32_t n = lane; n < prm.N; n += 32) {
+        const uint4 w0 = __ldg(recs + (size_t)n * kW);
+        const uint64_t cu = ((uint64_t)(w0.y & 0x00ffffffu) << 32) | w0.x;
+        xs[n] = (int64_t)((cu * (uint64_t)period + 32768ull) >> 16);
+      }
       __syncwarp();
       for (uint32_t s = 0; s < topo.n_stages; ++s) {
         // ---- gather the visitors of stage s ------------------------------------------------------
         const uint32_t sm = topo.mask[s];
         uint32_t M = 0;
-        cu_base = 0;
+        bool unsorted = false;
+        int64_t kmin = kInf, kmax = 0, prev_last = 0;
+        Req r_nx = load(0, true);
+        int64_t x_nx = lane < prm.N ? xs[lane] : 0;
         for (uint32_t n0 = 0; n0 < prm.N; n0 += 32) {
-          const Req r = draw(n0);
+          const Req r = r_nx;
+          const int64_t x_cur = x_nx;
+          if (n0 + 32 < prm.N) {
+            r_nx = load(n0 + 32, true);
+            if (n0 + 32 + lane < prm.N) x_nx = xs[n0 + 32 + lane];
+          }
           const bool vis = r.valid && ((r.vm >> s) & 1u);
           int32_t S = 0, Sc = 0;
 #pragma unroll
@@ -177,63 +290,117 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
             if (HAS_CPU) Sc += ((sm >> i) & 1u) ? r.cpu[i] : 0;
           }
           const uint32_t b = __ballot_sync(kAll, vis);
+          int64_t a = 0;
           if (vis) {
             const uint32_t n = n0 + lane, pos = M + __popc(b & lt_mask);
             const bool first = (r.vm & ((1u << s) - 1u)) == 0u;
-            key[pos] = xs[n] + (first ? 0 : delay);  // R9: a hop delay after the first visit
-            idx[pos] = n;
+            a = x_cur + (first ? 0 : delay);  // R9: a hop delay after the first visit
+            key[0][pos] = a;
+            idx[0][pos] = n;
             sv[n] = S;
             if (HAS_CPU) scpu[n] = Sc;
+            kmin = a < kmin ? a : kmin;
+            kmax = a > kmax ? a : kmax;
+          }
+          if (b) {  // in order? every visitor against the visitor before it (the previous chunk's last for the first)
+            const uint32_t below = b & lt_mask;
+            const int src = below ? 31 - __clz((int)below) : 0;
+            const int64_t pa = __shfl_sync(kAll, a, src);
+            if (vis && (below ? pa : prev_last) > a && (below || M > 0)) unsorted = true;
+            prev_last = __shfl_sync(kAll, a, 31 - __clz((int)b));
           }
           M += __popc(b);
         }
         __syncwarp();
         if (M == 0) continue;
-        // ---- order of service: (arrival, index) ---------------------------------------------------
-        bool unsorted = false;
-        for (uint32_t i = lane; i + 1 < M; i += 32) unsorted = unsorted || key[i] > key[i + 1];
+        // ---- order of service: by arrival, ties by index -----------------------------------------------
+        int cur = 0;
         if (__any_sync(kAll, unsorted)) {
-          uint32_t m_pad = 2;
-          while (m_pad < M) m_pad <<= 1;
-          for (uint32_t i = M + lane; i < m_pad; i += 32) { key[i] = kInf; idx[i] = 0xffffffffu; }
-          __syncwarp();
-          warp_bitonic_sort(key, idx, m_pad, lane);
+#pragma unroll
+          for (int dd = 16; dd >= 1; dd >>= 1) {
+            const int64_t o1 = __shfl_xor_sync(kAll, kmin, dd), o2 = __shfl_xor_sync(kAll, kmax, dd);
+            kmin = o1 < kmin ? o1 : kmin;
+            kmax = o2 > kmax ? o2 : kmax;
+          }
+          const uint32_t bits = 64u - (uint32_t)__clzll((long long)(kmin ^ kmax));  // keys agree above these bits
+          cur = warp_radix_sort(key, idx, M, bits, cnt_s[warp], lane);
         }
+        const int64_t* ks = key[cur];
+        const uint32_t* is = idx[cur];
         // ---- serve in that order, lanes as replicas -------------------------------------------------
         const uint32_t c = prm.plan_c[plan * 8 + s];
         int64_t F[CPL];
 #pragma unroll
         for (int j = 0; j < CPL; ++j) F[j] = (uint32_t)(j * 32 + lane) < c ? 0 : kInf;
+        // the sorted pairs are loaded two batches ahead, the services they point to one batch ahead
+        int64_t a_n1 = 0, a_n2 = 0;
+        uint32_t n_n1 = 0, n_n2 = 0, S_n1 = 0, Sc_n1 = 0;
+        if ((uint32_t)lane < M) { a_n1 = ks[lane]; n_n1 = is[lane]; S_n1 = (uint32_t)sv[n_n1]; if (HAS_CPU) Sc_n1 = (uint32_t)scpu[n_n1]; }
+        if (32u + lane < M) { a_n2 = ks[32u + lane]; n_n2 = is[32u + lane]; }
         for (uint32_t base = 0; base < M; base += 32) {
           const uint32_t e = base + lane;
           const int here = (int)min(32u, M - base);
-          int64_t a = 0, d = 0;
-          uint32_t n = 0;
-          int32_t S = 0, Sc = 0;
-          if (e < M) {
-            a = key[e];
-            n = idx[e];
-            S = sv[n];
-            if (HAS_CPU) Sc = scpu[n];
+          const int64_t a = a_n1;
+          const uint32_t n = n_n1, S = S_n1, Sc = Sc_n1;
+          int64_t d = 0;
+          a_n1 = a_n2; n_n1 = n_n2;
+          if (e + 32 < M) { S_n1 = (uint32_t)sv[n_n1]; if (HAS_CPU) Sc_n1 = (uint32_t)scpu[n_n1]; }
+          if (e + 64 < M) { a_n2 = ks[e + 64]; n_n2 = is[e + 64]; }
+          // 32-bit body if every time of the batch fits an offset from its first arrival
+          const int64_t a0 = __shfl_sync(kAll, a, 0), a_last = __shfl_sync(kAll, a, here - 1);
+          int64_t fm = 0;  // the largest free time: element c - 1 of the sorted vector
+#pragma unroll
+          for (int j = 0; j < CPL; ++j) {
+            const int64_t v = __shfl_sync(kAll, F[j], (c - 1u) & 31u);
+            if ((uint32_t)j == ((c - 1u) >> 5)) fm = v;
           }
-          for (int j = 0; j < here; ++j) {
-            const int64_t aj = __shfl_sync(kAll, a, j);
-            const int32_t Sj = __shfl_sync(kAll, S, j);
-            const int32_t Scj = HAS_CPU ? __shfl_sync(kAll, Sc, j) : 0;
-            const int64_t D = kw_step<CPL>(F, aj, Sj, Scj, lane);
-            if (lane == j) d = D;
+          const uint32_t work = (e < M) ? S + Sc : 0u;
+          const bool big = __any_sync(kAll, work >= (1u << 26));
+          const uint64_t sum = __reduce_add_sync(kAll, min(work, 1u << 26));
+          const int64_t top = fm > a_last ? fm : a_last;
+          if (!big && (uint64_t)(top - a0) + sum < 0xfffffff0ull) {
+            uint32_t G[CPL];
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) G[j] = F[j] == kInf ? kInf32 : (uint32_t)((F[j] > a0 ? F[j] : a0) - a0);
+            const uint32_t a32 = (uint32_t)(a - a0);
+            uint32_t d32 = 0;
+            for (int j = 0; j < here; ++j) {
+              const uint32_t aj = __shfl_sync(kAll, a32, j), Sj = __shfl_sync(kAll, S, j);
+              const uint32_t Scj = HAS_CPU ? __shfl_sync(kAll, Sc, j) : 0u;
+              const uint32_t D = kw_visit<CPL, HAS_CPU, uint32_t>(G, aj, Sj, Scj, kInf32, lane);
+              if (lane == j) d32 = D;
+            }
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) F[j] = G[j] == kInf32 ? kInf : a0 + (int64_t)G[j];
+            d = a0 + (int64_t)d32;
+          } else {
+            for (int j = 0; j < here; ++j) {
+              const int64_t aj = __shfl_sync(kAll, a, j);
+              const uint32_t Sj = __shfl_sync(kAll, S, j);
+              const uint32_t Scj = HAS_CPU ? __shfl_sync(kAll, Sc, j) : 0u;
+              const int64_t D = kw_visit<CPL, HAS_CPU, int64_t>(F, aj, Sj, Scj, kInf, lane);
+              if (lane == j) d = D;
+            }
           }
           if (e < M) xs[n] = d;
         }
         __syncwarp();
       }
       // ---- last: a8 over x[n] - A_n ------------------------------------------------------------------
-      cu_base = 0;
       const bool traced = fp.only_plan != 0xffffffffu;
+      uint4 w_nx = __ldg(recs + (size_t)min((uint32_t)lane, prm.N - 1u) * kW);
+      int64_t xf_nx = (uint32_t)lane < prm.N ? xs[lane] : 0;
       for (uint32_t n0 = 0; n0 < prm.N; n0 += 32) {
-        const Req r = draw(n0);
+        struct { bool valid; uint32_t t; uint64_t cu; } r;
+        r.valid = n0 + lane < prm.N;
+        r.t = w_nx.y >> 24;
+        r.cu = ((uint64_t)(w_nx.y & 0x00ffffffu) << 32) | w_nx.x;
+        const int64_t x = r.valid ? xf_nx : 0;
+        if (n0 + 32 < prm.N) {
+          w_nx = __ldg(recs + (size_t)min(n0 + 32 + lane, prm.N - 1u) * kW);
+          if (n0 + 32 + lane < prm.N) xf_nx = xs[n0 + 32 + lane];
+        }
         const int64_t A = (int64_t)((r.cu * (uint64_t)period + 32768ull) >> 16);
-        const int64_t x = r.valid ? xs[n0 + lane] : 0;
         if (traced && r.valid) {
           if (prm.tr_arrival) prm.tr_arrival[n0 + lane] = A;
           if (prm.tr_departure) prm.tr_departure[n0 + lane] = x;

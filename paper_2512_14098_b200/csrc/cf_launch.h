@@ -32,5 +32,7 @@ cudaError_t launch_scan_k(int cmax, const KParams& kp, uint32_t blocks, uint32_t
 
 // arrival-order kernel (cf_fcfs.cu): cmax in {6, 8}, cpl = free-time elements per lane in {1, 2, 4, 8}
 cudaError_t launch_fcfs_k(int cmax, bool has_cpu, int cpl, const KParams& kp, const FcfsParams& fp, cudaStream_t st);
+// ... and the two launches that draw the request records of the call's kp.k_launch trials
+cudaError_t launch_fcfs_records_k(int cmax, bool has_cpu, const KParams& kp, const FcfsParams& fp, cudaStream_t st);
 
 }  // namespace cfk

@@ -93,9 +93,10 @@ typedef struct {
                                   1: in the order in which they REACH the stage, ties by request index --
                                   textbook FCFS at every node (R27). Runs on
                                   the arrival-order kernel: one warp per simulation, stage by stage, over
-                                  40 N bytes of workspace per simulation in flight (cf_workspace_bytes asks for
-                                  up to 2368 of them; a larger workspace runs up to 4736 at once). Replicas
-                                  per stage <= 256; path routing only (join_mode = 0); no stream.           */
+                                  36 N bytes of workspace per simulation in flight (40 N with cpu_tab) plus
+                                  80 N K bytes of request records; cf_workspace_bytes asks for 2368
+                                  simulations in flight, a larger workspace runs up to 2960 at once.
+                                  Replicas per stage <= 256; path routing only (join_mode = 0); no stream.  */
 } cf_graph;
 
 /* P physical plans; plan p is an ORDERED list of n_stages[p] stages, stage s = (bitmask of the

@@ -106,18 +106,33 @@ __device__ __forceinline__ int warp_radix_sort(int64_t* const (&key)[2], uint32_
 #pragma unroll
     for (int k = 0; k < 8; ++k) cnt[lane * 8 + k] = 0;
     __syncwarp();
-    // (every loop below loads the next chunk of 32 before it works on the current one: the segment
-    //  streams from HBM and a warp has nothing else to hide the round trip with)
-    int64_t k_nx = lane < M ? ks[lane] : 0;
-    for (uint32_t base = 0; base < M; base += 32) {  // histogram of the digit
-      const uint32_t i = base + lane;
-      const bool valid = i < M;
-      const int64_t k = k_nx;
-      if (i + 32 < M) k_nx = ks[i + 32];
-      const uint32_t d = valid ? (uint32_t)((uint64_t)k >> shift) & 255u : 0x100u + lane;
-      const uint32_t m = __match_any_sync(kAll, d);
-      if (valid && (m & lt_mask) == 0u) cnt[d] += __popc(m);  // the lowest lane of each digit group
-      __syncwarp();
+    // (the segment streams from HBM and a warp has nothing else to hide the round trip with: every
+    //  loop below loads the NEXT group of 4 chunks of 32 before it works on the current one)
+    int64_t kn[4];
+    uint32_t in[4];
+    auto fetch_keys = [&](uint32_t b0) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const uint32_t i = b0 + (uint32_t)r * 32u + lane;
+        kn[r] = i < M ? ks[i] : 0;
+      }
+    };
+    fetch_keys(0);
+    for (uint32_t base = 0; base < M; base += 128) {  // histogram of the digit
+      int64_t kc[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) kc[r] = kn[r];
+      if (base + 128 < M) fetch_keys(base + 128);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const uint32_t i = base + (uint32_t)r * 32u + lane;
+        if (base + (uint32_t)r * 32u >= M) break;
+        const bool valid = i < M;
+        const uint32_t d = valid ? (uint32_t)((uint64_t)kc[r] >> shift) & 255u : 0x100u + lane;
+        const uint32_t m = __match_any_sync(kAll, d);
+        if (valid && (m & lt_mask) == 0u) cnt[d] += __popc(m);  // the lowest lane of each digit group
+        __syncwarp();
+      }
     }
     {  // exclusive scan of the 256 counters, 8 per lane
       uint32_t v[8], s = 0;
@@ -134,24 +149,37 @@ __device__ __forceinline__ int warp_radix_sort(int64_t* const (&key)[2], uint32_
       for (int k = 0; k < 8; ++k) { cnt[lane * 8 + k] = run; run += v[k]; }
     }
     __syncwarp();
-    k_nx = lane < M ? ks[lane] : 0;
-    uint32_t i_nx = lane < M ? is[lane] : 0;
-    for (uint32_t base = 0; base < M; base += 32) {  // stable scatter, a chunk of 32 at a time
-      const uint32_t i = base + lane;
-      const bool valid = i < M;
-      const int64_t k = k_nx;
-      const uint32_t ix = i_nx;
-      if (i + 32 < M) { k_nx = ks[i + 32]; i_nx = is[i + 32]; }
-      const uint32_t d = valid ? (uint32_t)((uint64_t)k >> shift) & 255u : 0x100u + lane;
-      const uint32_t m = __match_any_sync(kAll, d);
-      const uint32_t off = valid ? cnt[d] : 0u;
-      __syncwarp();
-      if (valid && (m & lt_mask) == 0u) cnt[d] = off + __popc(m);
-      __syncwarp();
-      if (valid) {
-        const uint32_t pos = off + __popc(m & lt_mask);
-        kd[pos] = k;
-        id[pos] = ix;
+    auto fetch_pairs = [&](uint32_t b0) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const uint32_t i = b0 + (uint32_t)r * 32u + lane;
+        kn[r] = i < M ? ks[i] : 0;
+        in[r] = i < M ? is[i] : 0u;
+      }
+    };
+    fetch_pairs(0);
+    for (uint32_t base = 0; base < M; base += 128) {  // stable scatter, a chunk of 32 at a time
+      int64_t kc[4];
+      uint32_t ic[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) { kc[r] = kn[r]; ic[r] = in[r]; }
+      if (base + 128 < M) fetch_pairs(base + 128);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const uint32_t i = base + (uint32_t)r * 32u + lane;
+        if (base + (uint32_t)r * 32u >= M) break;
+        const bool valid = i < M;
+        const uint32_t d = valid ? (uint32_t)((uint64_t)kc[r] >> shift) & 255u : 0x100u + lane;
+        const uint32_t m = __match_any_sync(kAll, d);
+        const uint32_t off = valid ? cnt[d] : 0u;
+        __syncwarp();
+        if (valid && (m & lt_mask) == 0u) cnt[d] = off + __popc(m);
+        __syncwarp();
+        if (valid) {
+          const uint32_t pos = off + __popc(m & lt_mask);
+          kd[pos] = kc[r];
+          id[pos] = ic[r];
+        }
       }
     }
     __syncwarp();

@@ -182,6 +182,43 @@ def test_random_fidelity_variants(cf, orc, seed):
     np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
 
 
+FCFS_SEEDS = list(range(500, 564)) + list(range(18000, 18000 + EXTRA // 4))
+
+
+@pytest.mark.parametrize("seed", FCFS_SEEDS)
+def test_random_arrival_order(cf, orc, seed):
+    """Arrival-order service (R27, cf_fcfs.cuh) on the random graphs: radix sorts of 0..5 passes, both
+    bodies of the recursion (rates of 1 milli-request/s span more than 2^32 us per batch), replica
+    counts up to 40 (two free-time elements per lane); a third with CPU-GPU overlap, a fourth bisected."""
+    w, R_p = random_case(seed)
+    g, pl = w.graph, w.plans
+    g.order_mode = 1
+    rng = np.random.default_rng(seed + 2)
+    if seed % 3 == 0:
+        C, T = g.n_comp, g.n_types
+        g.tabs = g.tabs + [W.exponential_qtab(float(rng.uniform(500.0, 40_000.0))) for _ in range(2)]
+        cpu = np.full(C * T, 0xFFFF, np.uint16)
+        for i in range(C):
+            if rng.random() < 0.5:
+                cpu[i * T:(i + 1) * T] = C + int(rng.integers(0, 2))
+        g.cpu_tab = cpu
+    if orc.validate(g, pl) != 0:
+        assert seed >= 564  # none of the committed seeds
+        pytest.skip("the generator drew services whose worst-case sum exceeds int32 (R17)")
+    want = orc.eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, 4, n_threads=NT)
+    got = cf.cf_eval_plans(g, pl, w.rate_mrps, w.slo, w.seed, 4)
+    assert cf.cf_workspace_status(got["workspace"]) == want["rc"]
+    np.testing.assert_array_equal(cf.to_numpy_u32(got["counts"]), want["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u64(got["dep_sum"]), want["dep_sum"])
+    np.testing.assert_array_equal(got["makespan"].cpu().numpy(), want["makespan"])
+    if seed % 4 == 0:
+        hi = np.minimum(np.ceil(1.5 * np.minimum(R_p, 1e9)), 1_000_000_000).astype(np.uint32)
+        b = cf.cf_goodput_bisect(g, pl, hi, 9, w.slo, w.seed)
+        bo = orc.goodput_bisect(g, pl, hi, 9, w.slo, w.seed, n_threads=NT)
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["rate_mrps"]), bo["rate_mrps"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(b["counts"]), bo["counts"])
+
+
 @pytest.mark.parametrize("seed", BISECT_SEEDS)
 def test_random_bisect(cf, orc, seed):
     w, R_p = random_case(seed)

@@ -144,17 +144,18 @@ int32_t orc_flow_bound(const orc_graph* g, const orc_plans* pl, uint32_t alpha_n
  * cf_oracle.cpp's simulate: common random numbers, R4); a request's latency is the sum of its
  * sampled processing latencies along its path plus the transfer delay per hop,
  * "queuing not modeled"; F_{t,d}(L_t) = hits_t / cnt_t and
- * G_{t,d} = floor(rate_d * hits_t / (N K)) (= alpha R_d * pi_t * F_{t,d}(L_t) with the sampled mix, R10). */
+ * G_{t,d} = floor(rate_d * hits_t / (N K)) (= alpha R_d * pi_t * F_{t,d}(L_t) with the sampled mix, R10).
+ * With routes (R26) the path is the drawn route's; with fork-join (R25) the latency is the critical
+ * path: a stage starts when its predecessor stages have finished (+ the delay of that edge). */
 int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* rate_mrps,
                        const orc_slo* slo, uint64_t seed, uint32_t variant, uint32_t* out_counts,
                        uint32_t* out_goodput_mrps) {
   if (int32_t rc = orc_validate(g, pl)) return rc;
   if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return ORC_ERR_ARG;
-  if (g->join_mode) return ORC_ERR_ARG; /* fork-join latency is a critical path, not a sum: not offered (R25) */
-  if (pl->max_routes) return ORC_ERR_ARG; /* routed plans: not offered (R26) */
   const uint32_t C = g->n_comp, T = g->n_types, N = g->n_req, K = g->n_trials;
   const uint32_t key[2] = {(uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32)};
   for (uint32_t p = 0; p < pl->n_plans; ++p) {
+    const uint8_t* smask = pl->stage_mask + (size_t)p * pl->max_stages;
     std::vector<uint64_t> pooled_hits(T, 0);
     for (uint32_t k = 0; k < K; ++k) {
       std::vector<uint32_t> cnt(T, 0), hits(T, 0);
@@ -165,6 +166,14 @@ int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* 
         for (uint32_t tt = 0; tt < T; ++tt)
           if (b0[1] < g->type_thresh[tt]) { t = tt; break; }
         const uint8_t tm = g->type_mask[t];
+        uint8_t route = 0xff; /* R26: the stages of the route this request drew */
+        if (pl->max_routes > 0) {
+          const uint32_t MR = pl->max_routes;
+          uint32_t r = MR - 1;
+          for (uint32_t rr = 0; rr < MR; ++rr)
+            if (b0[2] < pl->route_cum[((size_t)p * T + t) * MR + rr]) { r = rr; break; }
+          route = pl->route_mask[((size_t)p * T + t) * MR + r];
+        }
         int64_t svc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         for (uint32_t i = 0; i < C; ++i)
           if ((tm >> i) & 1) {
@@ -177,15 +186,32 @@ int32_t orc_mc_latency(const orc_graph* g, const orc_plans* pl, const uint32_t* 
               svc[i] += orc_qtab_sample(&g->tabs[g->cpu_tab[i * T + t]], b[i % 4]);
             }
           }
-        int64_t lat = 0; /* accumulated latency along the path, no waiting */
+        int64_t lat = 0; /* accumulated latency since the request's arrival, no waiting */
         bool first = true;
+        int64_t done[8];
+        bool visited[8] = {false, false, false, false, false, false, false, false};
         for (uint32_t s = 0; s < pl->n_stages[p]; ++s) {
-          const uint8_t m = pl->stage_mask[p * pl->max_stages + s] & tm;
-          if (m == 0) continue;
-          if (!first) lat += g->edge_delay_us;
+          const uint8_t m = smask[s] & tm;
+          if (m == 0 || !((route >> s) & 1)) continue;
+          int64_t x; /* when the request reaches stage s */
+          if (g->join_mode) { /* R25: after its last predecessor stage, plus that edge's delay */
+            x = 0;
+            for (uint32_t sp = 0; sp < s; ++sp) {
+              if (!visited[sp]) continue;
+              bool feeds = false;
+              for (uint32_t e = 0; e < g->n_edges; ++e)
+                if ((((smask[sp] & tm) >> g->edges[2 * e]) & 1) && ((m >> g->edges[2 * e + 1]) & 1)) feeds = true;
+              if (feeds) x = std::max(x, done[sp] + g->edge_delay_us);
+            }
+          } else {
+            x = lat + (first ? 0 : g->edge_delay_us);
+          }
           first = false;
           for (uint32_t i = 0; i < C; ++i)
-            if ((m >> i) & 1) lat += svc[i];
+            if ((m >> i) & 1) x += svc[i];
+          done[s] = x;
+          visited[s] = true;
+          lat = g->join_mode ? std::max(lat, x) : x; /* R25: done when the last branch is */
         }
         cnt[t]++;
         if (lat <= slo->L_us[t]) hits[t]++;

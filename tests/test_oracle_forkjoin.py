@@ -153,4 +153,30 @@ def test_chain_graphs_are_unaffected(orc):
     b = orc.eval_plans(w.graph, w.plans, w.rate_mrps, w.slo, w.seed, n_threads=4)
     for key in ("counts", "dep_sum", "makespan"):
         np.testing.assert_array_equal(a[key], b[key])
-    assert orc.mc_latency(w.graph, w.plans, w.rate_mrps[:, 0], w.slo, w.seed)["rc"] == orc.ORC_ERR_ARG
+    # ... and so is the Monte-Carlo latency (a critical path with one branch is the sum)
+    m1 = orc.mc_latency(w.graph, w.plans, w.rate_mrps[:, 0], w.slo, w.seed)
+    w.graph.join_mode = 0
+    m0 = orc.mc_latency(w.graph, w.plans, w.rate_mrps[:, 0], w.slo, w.seed)
+    assert m1["rc"] == m0["rc"] == 0
+    np.testing.assert_array_equal(m1["counts"], m0["counts"])
+
+
+def test_monte_carlo_latency_is_the_critical_path(orc):
+    # phase 2 under fork-join (R25): "queuing not modeled" -- the simulation with unlimited replicas at any
+    # rate; the simulation's fork-join rule is pinned above by path enumeration and two event simulators
+    w = W.config4_sweep(n_req=600, n_trials=2, vectors_per_pattern=1, n_variants=1)   # up to 3 parallel encoders
+    g, pl = w.graph, w.plans
+    g.join_mode = 1
+    g.edge_delay_us = 9_000
+    slo = W.Slo([150_000, 200_000, 180_000, 260_000, 3_600_000, 3_700_000, 3_650_000, 3_800_000], [9] * 8, [10] * 8)
+    big = W.Plans(pl.n_stages, pl.stage_mask, np.full_like(pl.stage_c, 600))
+    rate = np.full(pl.n_plans, 50_000, np.uint32)
+    sim = orc.eval_plans(g, big, rate[:, None], slo, w.seed, 2, n_threads=8)
+    mc = orc.mc_latency(g, pl, rate, slo, w.seed, 2)
+    assert mc["rc"] == 0
+    np.testing.assert_array_equal(mc["counts"], sim["counts"][:, 0])
+    h = mc["counts"][..., 1].sum()
+    assert 0 < h < mc["counts"][..., 0].sum()
+    g.join_mode = 0                      # the path mode queues the encoders one after another: later
+    seq = orc.mc_latency(g, pl, rate, slo, w.seed, 2)
+    assert (seq["counts"][..., 1] <= mc["counts"][..., 1]).all() and seq["counts"][..., 1].sum() < h

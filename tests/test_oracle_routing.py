@@ -115,7 +115,35 @@ def test_flow_bound_with_routing_hand_worked(orc):
     assert f["redundant"].tolist() == [1, 1, 1]  # plan 0: s1 sustains 9 815 with 3 executors (15 000); plan 2: with 2 (10 000)
     pl = two_path_plans([(1, 2, 2)], 0.5, 0.5)   # s1 with one executor fewer: 5 000 < 9 815; s2: 4 907 < 9 815
     assert orc.flow_bound(g, pl)["redundant"].tolist() == [0]
-    assert orc.mc_latency(g, pl, [1000], W.Slo([1, 1], [9, 9], [10, 10]), 0)["rc"] == orc.ORC_ERR_ARG
+
+
+def test_monte_carlo_latency_with_routes(orc):
+    # constant services (E 30 ms, LLM 400 ms) and a 1 s hop: a text request always takes 400 ms, an image
+    # request 430 ms on the colocated node and 1 430 ms on the disaggregated path; with L = 1 s the image
+    # hits are exactly the requests that drew the colocated route
+    g = mllm(4000, 2, delay=1_000_000, constant=True)
+    pl = two_path_plans([(1, 1, 1), (5, 5, 5)], 0.5, 0.3)
+    slo = W.Slo([1_000_000, 1_000_000], [9, 9], [10, 10])
+    mc = orc.mc_latency(g, pl, [1000, 2000], slo, 3)
+    assert mc["rc"] == 0
+    for k in range(2):
+        t = orc.trace_sim(g, two_path_plans([(4000, 4000, 4000)], 0.5, 0.3), 0, 1000, k, seed=3)
+        img = t["type"] == 1
+        colocated = (t["departure"] - t["arrival"])[img] == 430_000
+        for p in range(2):   # replica counts do not matter to phase 2
+            assert mc["counts"][p, k, :, 0].tolist() == [int((~img).sum()), int(img.sum())]
+            assert mc["counts"][p, k, :, 1].tolist() == [int((~img).sum()), int(colocated.sum())]
+    # random tables: phase 2 == the simulation with unlimited replicas, route draws included
+    g = mllm(900, 2, delay=30_000)
+    pl = two_path_plans([(2, 3, 2), (1, 1, 4)], 0.6, 0.4)
+    slo = W.Slo([450_000, 520_000], [9, 9], [10, 10])
+    big = W.Plans(pl.n_stages, pl.stage_mask, np.full_like(pl.stage_c, 900), pl.max_routes, pl.route_mask, pl.route_cum)
+    sim = orc.eval_plans(g, big, np.array([[7_000], [9_000]], np.uint32), slo, 5, 1, n_threads=4)
+    mc = orc.mc_latency(g, pl, [7_000, 9_000], slo, 5, 1)
+    np.testing.assert_array_equal(mc["counts"], sim["counts"][:, 0])
+    h = mc["counts"][..., 1].astype(np.int64).sum(1)
+    np.testing.assert_array_equal(mc["goodput_mrps"], np.array([[7_000], [9_000]]) * h // 1800)
+    assert 0 < h.sum() < 2 * 1800
 
 
 def test_validation(orc):

@@ -88,7 +88,8 @@ typedef struct {
                                   one holding a component u of the request with an edge (u, v) into a
                                   component v of the request on that stage -- has finished, plus
                                   edge_delay_us; with no predecessor at its system arrival; it is done when
-                                  its last stage is. 64-bit kernel only; no stream; cf_mc_latency refuses.  */
+                                  its last stage is. 64-bit kernel only; no stream; cf_mc_latency then returns
+                                  the critical path of every request (per-plan kernel).                     */
   uint32_t order_mode;         /* 0: every stage serves its visitors in request-index order (R2).
                                   1: in the order in which they REACH the stage, ties by request index --
                                   textbook FCFS at every node (R27). Runs on
@@ -114,7 +115,8 @@ typedef struct {
    * word 2) and visits the stages of bitmask route_mask (bit s = stage s) that hold one of its
    * components. Stage masks may then overlap across stages; along every route they must serve
    * each component of the type exactly once, in an order the DAG allows. Routed plans cannot be
-   * evaluated on a materialised stream, and cf_mc_latency refuses them (CF_ERR_ARG). */
+   * evaluated on a materialised stream; cf_mc_latency follows each request's drawn route (per-plan
+   * kernel over shared request records instead of the plan-independent histogram). */
   uint32_t max_routes;
   const uint8_t* route_mask;    /* [P*T*max_routes] */
   const uint32_t* route_cum;    /* [P*T*max_routes] */

@@ -1628,6 +1628,7 @@ namespace {
 
 struct AuxSetup {
   AuxParams ap;
+  KParams kp;  // graph part (tables, thresholds, seed): the request-record kernels of the generic Monte-Carlo path
   Blob blob;
   size_t mean_off = 0, demand_off = 0, hist_off = 0, need = 0;
 };
@@ -1639,8 +1640,10 @@ int32_t aux_setup(const cf_graph* g, const cf_plans* pl, const cf_slo* slo, uint
   AuxParams& ap = a.ap;
   std::memset(&ap, 0, sizeof(ap));
   a.blob.reserve(kAlign);  // status block
-  KParams kp;
+  KParams& kp = a.kp;
   const size_t pool_off = fill_graph_params(g, slo, seed, &a.blob, &kp);
+  ap.join = g->join_mode ? 1u : 0u;
+  for (uint32_t e = 0; e < g->n_edges; ++e) ap.edge_to[g->edges[2 * e]] |= (uint8_t)(1u << g->edges[2 * e + 1]);
   ap.C = kp.C; ap.T = kp.T; ap.N = kp.N; ap.K = kp.K;
   std::memcpy(ap.type_thresh, kp.type_thresh, sizeof(ap.type_thresh));
   std::memcpy(ap.type_mask, kp.type_mask, sizeof(ap.type_mask));
@@ -1681,6 +1684,8 @@ int32_t aux_setup(const cf_graph* g, const cf_plans* pl, const cf_slo* slo, uint
   if (int32_t rc = cuda_rc(cudaMemcpyAsync(w, a.blob.bytes.data(), a.blob.bytes.size(), cudaMemcpyHostToDevice, st)))
     return rc;
   ap.qpool = reinterpret_cast<const int32_t*>(w + pool_off);
+  kp.qpool = ap.qpool;
+  kp.status = reinterpret_cast<int32_t*>(w);
   ap.tabs = reinterpret_cast<const DevTab*>(w + tabs_off);
   if (pl) {
     ap.n_stages = w + ns_off;
@@ -1713,6 +1718,8 @@ size_t cf_aux_workspace_bytes(const cf_graph* g, const cf_plans* pl) {
   if (pl) n += 5 * kAlign + align_up((size_t)pl->n_plans) + align_up((size_t)pl->n_plans * pl->max_stages * 3) +
                align_up((size_t)pl->n_plans * g->n_types * pl->max_routes * 5);
   n += align_up((size_t)g->n_tabs * 8) + align_up(256 * 8) + align_up((size_t)g->n_trials * 72 * 4);
+  if (pl && (g->join_mode || pl->max_routes))  // generic Monte-Carlo path: request records + pooled hits
+    n += 2 * kAlign + fcfs_record_bytes(g, g->n_trials, nullptr, nullptr) + align_up((size_t)pl->n_plans * g->n_types * 8);
   return n + 4 * kAlign;
 }
 
@@ -1743,11 +1750,43 @@ int32_t cf_mc_latency(const cf_graph* g, const cf_plans* pl, const uint32_t* rat
   if (int32_t rc = check_graph(g)) return rc;
   if (int32_t rc = check_plans(g, pl)) return rc;
   if (!rate_mrps || !slo || !slo->L_us || !out_goodput_mrps) return CF_ERR_ARG;
-  if (g->join_mode) return CF_ERR_ARG;  // fork-join latency is a critical path, not a sum (R25)
-  if (pl->max_routes) return CF_ERR_ARG;  // routed plans: not offered (R26)
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   AuxSetup a;
   if (int32_t rc = aux_setup(g, pl, slo, seed, variant, workspace, workspace_bytes, st, &a)) return rc;
+  if (g->join_mode || pl->max_routes) {
+    // Routed plans (R26) and fork-join graphs (R25): the latency of a request depends on the plan through
+    // more than its hop count, so every (plan, trial) block walks the trial's request records
+    const uint32_t K = g->n_trials, P = pl->n_plans, T = g->n_types;
+    FcfsParams fp;
+    std::memset(&fp, 0, sizeof(fp));
+    const size_t rec_bytes = fcfs_record_bytes(g, K, &fp.n_seg, &fp.chunks_per_seg);
+    const size_t rec_off = align_up(a.need), pooled_off = align_up(rec_off + rec_bytes);
+    if (pooled_off + (size_t)P * T * 8 > workspace_bytes) return CF_ERR_WORKSPACE;
+    uint8_t* w = static_cast<uint8_t*>(workspace);
+    fp.records = reinterpret_cast<uint4*>(w + rec_off);
+    fp.seg_tot = reinterpret_cast<unsigned long long*>(w + rec_off + align_up((size_t)K * g->n_req * 5 * 16));
+    unsigned long long* pooled = reinterpret_cast<unsigned long long*>(w + pooled_off);
+    KParams kp = a.kp;
+    kp.variant_lo = variant;
+    kp.trial_base = 0;
+    kp.k_launch = K;
+    const int cmax = (g->n_comp <= 6 && !pl->max_routes) ? 6 : 8;
+    const bool has_cpu = kp.has_cpu != 0;
+    if (int32_t rc = cuda_rc(launch_fcfs_records_k(cmax, has_cpu, kp, fp, st))) return rc;
+    if (int32_t rc = cuda_rc(cudaMemsetAsync(pooled, 0, (size_t)P * T * 8, st))) return rc;
+    const dim3 grid(P, K);
+    if (K > 65535u) return CF_ERR_ARG;
+    if (cmax == 8) {
+      if (has_cpu) mc_generic_kernel<8, true><<<grid, 256, 0, st>>>(a.ap, fp.records, pooled, out_counts);
+      else mc_generic_kernel<8, false><<<grid, 256, 0, st>>>(a.ap, fp.records, pooled, out_counts);
+    } else {
+      if (has_cpu) mc_generic_kernel<6, true><<<grid, 256, 0, st>>>(a.ap, fp.records, pooled, out_counts);
+      else mc_generic_kernel<6, false><<<grid, 256, 0, st>>>(a.ap, fp.records, pooled, out_counts);
+    }
+    mc_generic_final_kernel<<<(P * T + 127) / 128, 128, 0, st>>>(a.ap, rate_mrps, pooled, out_goodput_mrps);
+    g_launch_count += 4;
+    return cuda_rc(cudaGetLastError());
+  }
   if (int32_t rc = cuda_rc(cudaMemsetAsync(a.ap.hist, 0, (size_t)g->n_trials * 72 * 4, st))) return rc;
   mc_hist_kernel<<<dim3((g->n_req + 255) / 256, g->n_trials), 256, 0, st>>>(a.ap);
   mc_plan_kernel<<<(pl->n_plans + 127) / 128, 128, 0, st>>>(a.ap, rate_mrps, out_counts, out_goodput_mrps);

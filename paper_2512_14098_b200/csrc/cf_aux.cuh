@@ -67,6 +67,8 @@ struct AuxParams {
   uint64_t* mean_q16;         // [n_tabs]
   uint64_t* demand_q16;       // [256] demand of the node with component mask m
   uint32_t* hist;             // [K][8][9]: hits for h = 0..7 hops, [8] = requests of the type
+  uint32_t join;              // R25: fork-join along the DAG edges (generic Monte-Carlo kernel)
+  uint8_t edge_to[8];         // edge_to[u] = bitmask of the components v with a DAG edge (u, v)
 };
 
 // ---- phase 1 -----------------------------------------------------------------------------------
@@ -261,6 +263,119 @@ mc_plan_kernel(const __grid_constant__ AuxParams prm, const uint32_t* rate_mrps,
     }
     out_goodput[(size_t)p * prm.T + t] = (uint32_t)u128_div(__umul64hi(rate, hits), rate * hits, nk);
   }
+}
+
+// Phase 2 for plans whose latency is not "services + hops x delay of the type": routed plans (R26: the
+// path depends on the request's route draw against the PLAN's probabilities) and fork-join graphs
+// (R25: the latency is the critical path over the request's stages). One block per (plan, trial)
+// walks the trial's request records (drawn once per call by the kernels of cf_fcfs.cuh, shared by
+// all plans: common random numbers) and accumulates every request's latency without queueing.
+template <int CMAX, bool HAS_CPU>
+__global__ void __launch_bounds__(256)
+mc_generic_kernel(const __grid_constant__ AuxParams prm, const uint4* __restrict__ records,
+                  unsigned long long* pooled_hits, uint32_t* out_counts) {
+  constexpr int kW = CompRec<CMAX, HAS_CPU>::kWords;
+  constexpr int kB = CompRec<CMAX, HAS_CPU>::kBase;
+  __shared__ uint32_t cnt_s[8][2];
+  __shared__ uint8_t smask_s[8], feeds_s[8][8], rmask_s[8][4];
+  __shared__ uint32_t rcum_s[8][4];
+  const uint32_t p = blockIdx.x, k = blockIdx.y, tid = threadIdx.x, lane = tid & 31u;
+  const uint32_t V = prm.n_stages[p], MR = prm.max_routes;
+  if (tid < 16) cnt_s[tid >> 1][tid & 1] = 0;
+  if (tid < 8) smask_s[tid] = tid < V ? prm.stage_mask[(size_t)p * prm.MS + tid] : 0;
+  if (tid < 32 && MR) {
+    const uint32_t t = tid >> 2, r = tid & 3u;
+    const bool has = t < prm.T && r < MR;
+    rcum_s[t][r] = has ? prm.route_cum[((size_t)p * prm.T + t) * MR + r] : 0xffffffffu;
+    rmask_s[t][r] = has ? prm.route_mask[((size_t)p * prm.T + t) * MR + r] : 0;
+  }
+  __syncthreads();
+  if (tid < 64) {  // feeds[t][s]: the stages before s holding a component of type t with an edge into one on s
+    const uint32_t t = tid >> 3, s = tid & 7u, tm = prm.type_mask[t];
+    uint32_t pm = 0;
+    const uint32_t ms = smask_s[s] & tm;
+    for (uint32_t sp = 0; sp < s; ++sp) {
+      const uint32_t mp = smask_s[sp] & tm;
+      for (uint32_t u = 0; u < prm.C; ++u)
+        if (((mp >> u) & 1u) && (prm.edge_to[u] & ms)) pm |= 1u << sp;
+    }
+    feeds_s[t][s] = (uint8_t)pm;
+  }
+  __syncthreads();
+  const int64_t delay = prm.edge_delay;
+  const uint4* recs = records + (size_t)k * prm.N * kW;
+  for (uint32_t base = 0; base < prm.N; base += 256) {
+    const uint32_t n = base + tid;
+    const bool valid = n < prm.N;
+    const uint4* src = recs + (size_t)min(n, prm.N - 1u) * kW;
+    const uint4 w0 = __ldg(src), w1 = __ldg(src + 1);
+    uint4 w2 = make_uint4(0, 0, 0, 0);
+    if (CMAX > 6) w2 = __ldg(src + 2);
+    const uint32_t t = w0.y >> 24, tm = prm.type_mask[t];
+    int64_t svc[8];
+    svc[0] = (int32_t)w0.z; svc[1] = (int32_t)w0.w; svc[2] = (int32_t)w1.x; svc[3] = (int32_t)w1.y;
+    svc[4] = (int32_t)w1.z; svc[5] = (int32_t)w1.w; svc[6] = (int32_t)w2.x; svc[7] = (int32_t)w2.y;
+    if (HAS_CPU) {  // R24: nobody queues, so every executor is idle at every arrival
+      const uint4 c0 = __ldg(src + kB), c1 = __ldg(src + kB + 1);
+      svc[0] += (int32_t)c0.x; svc[1] += (int32_t)c0.y; svc[2] += (int32_t)c0.z; svc[3] += (int32_t)c0.w;
+      svc[4] += (int32_t)c1.x; svc[5] += (int32_t)c1.y; svc[6] += (int32_t)c1.z; svc[7] += (int32_t)c1.w;
+    }
+    uint32_t rmask = 0xffu;
+    if (MR) {  // R26: first route with u < cum, the last one takes the rest
+      uint32_t r = MR - 1u;
+      for (int rr = (int)MR - 2; rr >= 0; --rr)
+        if (w2.z < rcum_s[t][rr]) r = (uint32_t)rr;
+      rmask = rmask_s[t][r];
+    }
+    int64_t lat = 0, fin[8];
+    uint32_t vm = 0;
+#pragma unroll
+    for (int s = 0; s < 8; ++s) {
+      fin[s] = 0;
+      const uint32_t m = smask_s[s] & tm;
+      if (m != 0u && ((rmask >> s) & 1u)) {
+        int64_t x;
+        if (prm.join) {  // R25: after the last predecessor stage, plus that edge's delay
+          x = 0;
+          const uint32_t pm = feeds_s[t][s] & vm;
+#pragma unroll
+          for (int sp = 0; sp < s; ++sp)
+            if ((pm >> sp) & 1u) x = max(x, fin[sp] + delay);
+        } else {
+          x = lat + (vm ? delay : 0);
+        }
+#pragma unroll
+        for (int i = 0; i < CMAX; ++i)
+          if ((m >> i) & 1u) x += svc[i];
+        fin[s] = x;
+        vm |= 1u << s;
+        lat = prm.join ? max(lat, x) : x;
+      }
+    }
+    const bool hit = valid && lat <= prm.L_us[t];
+    for (uint32_t tt = 0; tt < prm.T; ++tt) {
+      const uint32_t mc = __ballot_sync(0xffffffffu, valid && t == tt);
+      const uint32_t mh = __ballot_sync(0xffffffffu, hit && t == tt);
+      if (lane == 0 && mc) { atomicAdd(&cnt_s[tt][0], __popc(mc)); if (mh) atomicAdd(&cnt_s[tt][1], __popc(mh)); }
+    }
+  }
+  __syncthreads();
+  if (tid < prm.T) {
+    if (out_counts) {
+      out_counts[(((size_t)p * prm.K + k) * prm.T + tid) * 2 + 0] = cnt_s[tid][0];
+      out_counts[(((size_t)p * prm.K + k) * prm.T + tid) * 2 + 1] = cnt_s[tid][1];
+    }
+    atomicAdd(&pooled_hits[(size_t)p * prm.T + tid], (unsigned long long)cnt_s[tid][1]);
+  }
+}
+
+__global__ void __launch_bounds__(128)
+mc_generic_final_kernel(const __grid_constant__ AuxParams prm, const uint32_t* rate_mrps,
+                        const unsigned long long* pooled_hits, uint32_t* out_goodput) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= prm.P * prm.T) return;
+  const uint64_t rate = rate_mrps[i / prm.T], hits = pooled_hits[i], nk = (uint64_t)prm.N * prm.K;
+  out_goodput[i] = (uint32_t)u128_div(__umul64hi(rate, hits), rate * hits, nk);
 }
 
 // ---- pruning and selection -----------------------------------------------------------------------

@@ -66,6 +66,48 @@ def test_forkjoin_parity(cf, orc):
     check(cf, orc, g, pl, rates, w.slo, w.seed, 1)
 
 
+def test_forkjoin_monte_carlo_latency(cf, orc):
+    """Phase 2 under fork-join (R25): the critical path of every sampled request, per plan."""
+    w = W.config4_sweep(n_req=4000, n_trials=3, vectors_per_pattern=2, n_variants=1)
+    g, pl = w.graph, w.plans
+    g.join_mode = 1
+    g.edge_delay_us = 9_000
+    slo = W.Slo([150_000, 200_000, 180_000, 260_000, 3_600_000, 3_700_000, 3_650_000, 3_800_000], [9] * 8, [10] * 8)
+    rate = orc.flow_bound(g, pl, 4, 5)["rate_mrps"]
+    o = orc.mc_latency(g, pl, rate, slo, w.seed, 2)
+    m = cf.cf_mc_latency(g, pl, rate, slo, w.seed, 2)
+    assert o["rc"] == 0
+    np.testing.assert_array_equal(cf.to_numpy_u32(m["counts"]), o["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u32(m["goodput_mrps"]), o["goodput_mrps"])
+    g.join_mode = 0
+    seq = orc.mc_latency(g, pl, rate, slo, w.seed, 2)
+    assert (seq["counts"][..., 1] <= o["counts"][..., 1]).all() and seq["counts"][..., 1].sum() < o["counts"][..., 1].sum()
+    g.join_mode = 1
+    # an 8-component DAG with two fan-ins, 8 types, CPU times on three components
+    rng = np.random.default_rng(5)
+    C = T = 8
+    tabs = [W.lognormal_qtab(float(rng.integers(5_000, 60_000)), 0.5) for _ in range(C)] + [W.exponential_qtab(9_000.0)]
+    masks = [int(mm) | 1 << int(rng.integers(0, C)) for mm in rng.integers(0, 256, T)]
+    edges = [[0, 3], [1, 3], [2, 3], [3, 4], [3, 5], [4, 6], [5, 6], [6, 7]]
+    cpu = np.full(C * T, 0xFFFF, np.uint16)
+    cpu[:3 * T] = C
+    g = W.Graph(C, T, 2500, 2, masks, W.mix_thresholds(rng.dirichlet(np.ones(T))), np.repeat(np.arange(C, dtype=np.uint16), T),
+                tabs, W.gamma_qtab(0.5, 65536.0), edges, edge_delay_us=2_000, join_mode=1, cpu_tab=cpu)
+    plan_list = []
+    for _ in range(30):
+        cuts = sorted(rng.choice(np.arange(1, C), size=int(rng.integers(0, C)), replace=False).tolist())
+        bounds = [0] + cuts + [C]
+        plan_list.append([(sum(1 << i for i in range(a, b)), int(rng.integers(1, 9))) for a, b in zip(bounds, bounds[1:])])
+    pl = W.make_plans(plan_list, max_stages=8)
+    slo = W.Slo(rng.integers(50_000, 300_000, T), [9] * T, [10] * T)
+    rate = rng.integers(1, 2**31, 30).astype(np.uint32)
+    o = orc.mc_latency(g, pl, rate, slo, 77, 1)
+    m = cf.cf_mc_latency(g, pl, rate, slo, 77, 1)
+    np.testing.assert_array_equal(cf.to_numpy_u32(m["counts"]), o["counts"])
+    np.testing.assert_array_equal(cf.to_numpy_u32(m["goodput_mrps"]), o["goodput_mrps"])
+    assert 0 < o["counts"][..., 1].sum() < o["counts"][..., 0].sum()
+
+
 def test_forkjoin_wide_graph_and_refusals(cf, orc):
     import torch
     rng = np.random.default_rng(4)
@@ -90,6 +132,5 @@ def test_forkjoin_wide_graph_and_refusals(cf, orc):
     w.graph.join_mode = 1
     rec = torch.zeros((1, 1, 100, 32), dtype=torch.uint8, device="cuda")
     assert cf.cf_eval_plans(w.graph, w.plans, [[1000]] * 2, w.slo, 0, stream_records=rec, check=False)["rc"] == cf.CF_ERR_ARG
-    assert cf.cf_mc_latency(w.graph, w.plans, [1000, 1000], w.slo, 0, check=False)["rc"] == cf.CF_ERR_ARG
     w.graph.join_mode = 2
     assert cf.cf_eval_plans(w.graph, w.plans, [[1000]] * 2, w.slo, 0, check=False)["rc"] == cf.CF_ERR_ARG

@@ -111,6 +111,42 @@ def test_routed_plans_parity(cf, orc):
     both_modes(cf, orc, g, pl, rates, slo, 11, 3)
 
 
+def test_monte_carlo_latency_with_routes(cf, orc):
+    """Phase 2 on routed plans (R26): the per-plan kernel over shared request records, against the oracle."""
+    from test_oracle_routing import mllm, two_path_plans
+    g = mllm(5000, 3, delay=30_000)
+    rng = np.random.default_rng(8)
+    cs = [tuple(int(x) for x in rng.integers(1, 9, 3)) for _ in range(40)]
+    pl = two_path_plans(cs, 0.6, 0.4)
+    pl.route_cum[:, :, 0] = rng.integers(0, 2**32, (40, 2), dtype=np.uint64).astype(np.uint32)   # a different split per plan
+    slo = W.Slo([430_000, 520_000], [9, 9], [10, 10])
+    rate = rng.integers(1, 2**32, 40, dtype=np.uint64).astype(np.uint32)
+    for variant in (0, 6):
+        o = orc.mc_latency(g, pl, rate, slo, 21, variant)
+        m = cf.cf_mc_latency(g, pl, rate, slo, 21, variant)
+        assert o["rc"] == 0
+        np.testing.assert_array_equal(cf.to_numpy_u32(m["counts"]), o["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(m["goodput_mrps"]), o["goodput_mrps"])
+    assert len({tuple(c) for c in o["counts"][..., 1].reshape(40, -1)}) > 10     # the plans' splits matter
+    # the 8-stage Omni plan set with two routed choices, fork-join on top, CPU-GPU overlap on top of that
+    g2, pl2, slo2 = omni_routed(3000, 2, np.random.default_rng(8))
+    g2.edge_delay_us = 7_000
+    r1 = orc.flow_bound(g2, pl2, 4, 5)["rate_mrps"]
+    for join in (0, 1):
+        g2.join_mode = join
+        o = orc.mc_latency(g2, pl2, r1, slo2, 11, 2)
+        m = cf.cf_mc_latency(g2, pl2, r1, slo2, 11, 2)
+        np.testing.assert_array_equal(cf.to_numpy_u32(m["counts"]), o["counts"])
+        np.testing.assert_array_equal(cf.to_numpy_u32(m["goodput_mrps"]), o["goodput_mrps"])
+    g2.tabs = g2.tabs + [W.exponential_qtab(12_000.0)]
+    cpu = np.full(g2.n_comp * g2.n_types, 0xFFFF, np.uint16)
+    cpu[:2 * g2.n_types] = len(g2.tabs) - 1
+    g2.cpu_tab = cpu
+    o = orc.mc_latency(g2, pl2, r1, slo2, 11, 2)
+    m = cf.cf_mc_latency(g2, pl2, r1, slo2, 11, 2, want_counts=False)
+    np.testing.assert_array_equal(cf.to_numpy_u32(m["goodput_mrps"]), o["goodput_mrps"])
+
+
 def test_routing_refusals(cf, orc):
     import torch
     from test_oracle_routing import mllm, two_path_plans
@@ -119,7 +155,6 @@ def test_routing_refusals(cf, orc):
     slo = W.Slo([1, 1], [9, 9], [10, 10])
     rec = torch.zeros((1, 1, 64, 32), dtype=torch.uint8, device="cuda")
     assert cf.cf_eval_plans(g, pl, [[1000]], slo, 0, stream_records=rec, check=False)["rc"] == cf.CF_ERR_ARG
-    assert cf.cf_mc_latency(g, pl, [1000], slo, 0, check=False)["rc"] == cf.CF_ERR_ARG
     bad = two_path_plans([(1, 1, 1)], 0.5, 0.5)
     bad.route_mask[0, 1, 0] = 0b010
     assert cf.cf_eval_plans(g, bad, [[1000]], slo, 0, check=False)["rc"] == cf.CF_ERR_PLAN == orc.validate(g, bad)

@@ -96,7 +96,8 @@ typedef struct {
                                   the arrival-order kernel: one warp per simulation, stage by stage, over
                                   36 N bytes of workspace per simulation in flight (40 N with cpu_tab) plus
                                   80 N K bytes of request records; cf_workspace_bytes asks for 2368
-                                  simulations in flight, a larger workspace runs up to 2960 at once.
+                                  simulations in flight (fewer if that exceeds 16 GiB), a larger workspace
+                                  runs up to 2960 at once.
                                   Replicas per stage <= 256; path routing only (join_mode = 0); no stream.  */
 } cf_graph;
 

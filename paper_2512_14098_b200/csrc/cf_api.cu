@@ -1338,7 +1338,9 @@ size_t cf_workspace_bytes(const cf_graph* g, const cf_plans* pl, uint32_t R) {
   if (g->order_mode) {  // arrival-order kernel: scratch of the simulations in flight
     const FcfsParams fp = fcfs_slot_layout(g);
     n += 2 * kAlign + fcfs_record_bytes(g, (uint32_t)K, nullptr, nullptr);
-    n += (size_t)fp.slot_bytes * std::min<uint64_t>((uint64_t)P * R * K, kFcfsAskSlots);
+    // ... of up to 2368 simulations in flight, capped at 16 GiB of scratch (never below one)
+    const uint64_t by_bytes = std::max<uint64_t>(1, (16ull << 30) / fp.slot_bytes);
+    n += (size_t)fp.slot_bytes * std::min<uint64_t>({(uint64_t)P * R * K, (uint64_t)kFcfsAskSlots, by_bytes});
   }
   return n + 4 * kAlign;
 }

@@ -82,7 +82,7 @@ int32_t validate(const orc_graph* g, const orc_plans* pl) {
   if (!g->type_mask || !g->type_thresh || !g->svc_tab || !g->tabs || g->n_tabs < 1)
     return ORC_ERR_ARG;
   if (g->n_edges > 0 && !g->edges) return ORC_ERR_ARG;
-  if (g->order_mode > 1 || (g->order_mode && g->join_mode)) return ORC_ERR_ARG; /* R27: path routing only */
+  if (g->order_mode > 1) return ORC_ERR_ARG;
   for (uint32_t t = 0; t < T; ++t) {
     if (g->type_mask[t] >> C) return ORC_ERR_ARG;
     if (t > 0 && g->type_thresh[t] < g->type_thresh[t - 1]) return ORC_ERR_ARG;
@@ -193,7 +193,8 @@ struct SimOut {
  * forward, so the arrivals at stage s are known once stages 0..s-1 are done: the stages are
  * processed one after another, each over all its visitors sorted by (arrival at the stage, index).
  * Same draws, same arrival times, same per-visit rule (Kiefer-Wolfowitz, idle/busy R24, hop delay
- * R9, routes R26) as simulate(); only the order of service differs. */
+ * R9, routes R26, fork-join R25: a request reaches a stage when its predecessor stages are done) as
+ * simulate(); only the order of service differs. */
 void simulate_fcfs(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t rate_mrps, uint32_t k,
                    const orc_slo* slo, uint64_t seed, uint32_t variant, SimOut* out,
                    int64_t* trace_arr, int64_t* trace_dep, uint8_t* trace_type) {
@@ -210,7 +211,8 @@ void simulate_fcfs(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t
   const uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
   /* the requests of the trial: the draws of simulate(), kept per request */
   std::vector<int64_t> A(N), x(N), svc((size_t)N * 8, 0), cpu((size_t)N * 8, 0);
-  std::vector<uint8_t> type(N), route(N, 0xff), hops(N, 0);
+  std::vector<uint8_t> type(N), route(N, 0xff), hops(N, 0), visited(N, 0);
+  std::vector<int64_t> done(g->join_mode ? (size_t)N * 8 : 0, 0); /* R25: departure of request n from stage s */
   uint64_t CU = 0;
   for (uint32_t n = 0; n < N; ++n) {
     uint32_t b0[4];
@@ -250,6 +252,18 @@ void simulate_fcfs(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t
     for (uint32_t n = 0; n < N; ++n) {
       const uint8_t m = smask[s] & g->type_mask[type[n]];
       if (m == 0 || !((route[n] >> s) & 1)) continue;
+      if (g->join_mode) { /* R25: after every predecessor stage, plus that edge's delay; else at A_n */
+        int64_t a = A[n];
+        for (uint32_t sp = 0; sp < s; ++sp) {
+          if (!((visited[n] >> sp) & 1)) continue;
+          bool feeds = false;
+          for (uint32_t e = 0; e < g->n_edges; ++e)
+            if ((((smask[sp] & g->type_mask[type[n]]) >> g->edges[2 * e]) & 1) && ((m >> g->edges[2 * e + 1]) & 1)) feeds = true;
+          if (feeds) a = std::max(a, done[(size_t)n * 8 + sp] + g->edge_delay_us);
+        }
+        order.emplace_back(a, n);
+        continue;
+      }
       order.emplace_back(x[n] + (hops[n] ? g->edge_delay_us : 0), n); /* R9: a hop delay after the first visit */
     }
     std::sort(order.begin(), order.end()); /* first come, first served; ties: lower index */
@@ -265,7 +279,13 @@ void simulate_fcfs(const orc_graph* g, const orc_plans* pl, uint32_t p, uint32_t
       int64_t d;
       if (f <= a) d = a + S_cpu + S; /* idle executor: CPU + GPU time */
       else d = f + S;                /* busy: GPU time alone */
-      x[n] = d;
+      if (g->join_mode) { /* done when the last branch is */
+        done[(size_t)n * 8 + s] = d;
+        visited[n] |= (uint8_t)(1u << s);
+        x[n] = std::max(x[n], d);
+      } else {
+        x[n] = d;
+      }
       hops[n]++;
       F[0] = d;
       std::sort(F.begin(), F.end());

@@ -63,7 +63,7 @@ typedef struct {
                                   stages on the request's subgraph have finished */
   uint32_t order_mode;         /* 0: every stage serves its visitors in request-index order (R2);
                                   1: in the order in which they reach the stage, ties by index -- textbook
-                                  FCFS (R27); not with join_mode = 1 */
+                                  FCFS (R27) */
 } orc_graph;
 
 /* P physical plans, each an ordered list of stages = (component bitmask, replica count). */

@@ -169,11 +169,85 @@ def test_invariants_and_bisection(orc):
             assert all(c[t, 1] * 10 >= 9 * c[t, 0] for t in range(4)) == want
 
 
+def forkjoin_fcfs_event_sim(A, tasks, stage_c, delay):
+    """Event-driven fork-join with ARRIVAL-order service: tasks[n] = {stage: (S, [pred stages])}; a task
+    becomes ready when all its predecessors are done (+ delay each) and joins its stage's waiting queue;
+    an idle server takes the waiting task that became ready first (ties: lower request index)."""
+    import heapq
+    V = len(stage_c)
+    idle = list(stage_c)
+    queue = [[] for _ in range(V)]
+    done = [dict() for _ in range(len(A))]
+    ev = []                                   # (time, kind, n, s): 0 = task ready, 1 = service completion
+    for n in range(len(A)):
+        for s, (_, pr) in tasks[n].items():
+            if not pr:
+                heapq.heappush(ev, (A[n], 0, n, s))
+
+    def dispatch(s, now):
+        while queue[s] and idle[s] > 0:
+            _, n = heapq.heappop(queue[s])
+            idle[s] -= 1
+            heapq.heappush(ev, (now + tasks[n][s][0], 1, n, s))
+
+    while ev:
+        now, kind, n, s = heapq.heappop(ev)
+        if kind == 0:
+            heapq.heappush(queue[s], (now, n))
+        else:
+            idle[s] += 1
+            done[n][s] = now
+            for s2, (_, pr) in tasks[n].items():
+                if s in pr and all(q in done[n] for q in pr):
+                    heapq.heappush(ev, (max(done[n][q] + delay for q in pr), 0, n, s2))
+        dispatch(s, now)
+    return [max(done[n].values(), default=A[n]) for n in range(len(A))]
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_forkjoin_under_arrival_order(orc, seed):
+    """R25 + R27: a stage starts a request when its predecessor stages are done, and serves in the order in
+    which requests become ready -- against an event simulator with task dependencies and waiting queues."""
+    from test_oracle_forkjoin import omni, stage_preds
+    rng = np.random.default_rng(300 + seed)
+    w = omni(n_req=int(rng.integers(30, 160)), delay=int(rng.choice([0, 9_000])))
+    g = w.graph
+    g.order_mode = 1
+    for p in rng.choice(w.plans.n_plans, 3, replace=False):
+        p = int(p)
+        V = int(w.plans.n_stages[p])
+        cs = [int(c) for c in rng.integers(1, 4, V)]
+        pl = W.make_plans([[(int(w.plans.stage_mask[p, s]), cs[s]) for s in range(V)]])
+        rate = int(rng.uniform(0.6, 1.4) * float(W.flow_bound_mrps(g, pl)[0]))
+        A, types, svc = refsim.gen_requests(g, 40 + seed, 1, 0, rate)
+        tasks = []
+        for n, t in enumerate(types):
+            masks, pred = stage_preds(g, pl, 0, t)
+            tasks.append({s: (sum(svc[n][i] for i in range(6) if (masks[s] >> i) & 1), pr) for s, pr in pred.items()})
+        got = orc.trace_sim(g, pl, 0, rate, 0, seed=40 + seed, variant=1)
+        assert got["departure"].tolist() == forkjoin_fcfs_event_sim(A, tasks, cs, g.edge_delay_us)
+    # unlimited replicas: nobody waits, the service order is immaterial -- the critical path of the index-order run
+    big = W.Plans(w.plans.n_stages, w.plans.stage_mask, np.full_like(w.plans.stage_c, g.n_req))
+    a = orc.trace_sim(g, big, 5, 3000, 0, seed=1)
+    g.order_mode = 0
+    b = orc.trace_sim(g, big, 5, 3000, 0, seed=1)
+    np.testing.assert_array_equal(a["departure"], b["departure"])
+    # on a chain graph fork-join is the path mode, in arrival order too
+    w1 = W.config1_mllm(n_req=700, n_trials=1, n_rates=2, llm_max=4, e_steps=3)
+    w1.graph.edge_delay_us = 5_000
+    w1.graph.order_mode = 1
+    a = orc.eval_plans(w1.graph, w1.plans, w1.rate_mrps, w1.slo, w1.seed, n_threads=4)
+    w1.graph.join_mode = 1
+    b = orc.eval_plans(w1.graph, w1.plans, w1.rate_mrps, w1.slo, w1.seed, n_threads=4)
+    for key in ("counts", "dep_sum", "makespan"):
+        np.testing.assert_array_equal(a[key], b[key])
+
+
 def test_validation(orc):
     g = omni_like(16)
     pl = W.make_plans([[(0b0011, 1), (0b0100, 1), (0b1000, 1)]])
     assert orc.validate(g, pl) == 0
     g.order_mode = 2
     assert orc.validate(g, pl) == orc.ORC_ERR_ARG
-    g.order_mode, g.join_mode = 1, 1     # arrival order is offered on path routing only
-    assert orc.validate(g, pl) == orc.ORC_ERR_ARG
+    g.order_mode, g.join_mode = 1, 1     # arrival order composes with fork-join
+    assert orc.validate(g, pl) == 0

@@ -98,7 +98,8 @@ typedef struct {
                                   80 N K bytes of request records; cf_workspace_bytes asks for 2368
                                   simulations in flight (fewer if that exceeds 16 GiB), a larger workspace
                                   runs up to 2960 at once.
-                                  Replicas per stage <= 256; path routing only (join_mode = 0); no stream.  */
+                                  Replicas per stage <= 256; no stream. With join_mode = 1 a slot holds 64 N
+                                  bytes more (the departure of every request from every stage).            */
 } cf_graph;
 
 /* P physical plans; plan p is an ORDERED list of n_stages[p] stages, stage s = (bitmask of the

@@ -73,7 +73,7 @@ int32_t check_graph(const cf_graph* g) {
     if (int32_t rc = check_tab(g->tabs[j])) return rc;
   if (int32_t rc = check_tab(g->arr_tab)) return rc;
   if (g->join_mode > 1) return CF_ERR_ARG;
-  if (g->order_mode > 1 || (g->order_mode && g->join_mode)) return CF_ERR_ARG;  // R27: arrival order on path routing only
+  if (g->order_mode > 1) return CF_ERR_ARG;
   if (g->edge_delay_us < 0 || g->edge_delay_us >= (1ll << 31)) return CF_ERR_RANGE;
   // DESIGN.md R17: a request's total service over all its components must fit int32
   int64_t worst = 0;
@@ -703,6 +703,11 @@ FcfsParams fcfs_slot_layout(const cf_graph* g) {
   fp.off_sv = (uint32_t)off;  off += align_up(N * 4);
   fp.off_scpu = (uint32_t)off;
   if (graph_has_cpu(g)) off += align_up(N * 4);
+  if (g->join_mode) {  // R25 under arrival order: the departure of every request from every stage
+    fp.off_done = (uint32_t)off;
+    fp.done_stride = (uint32_t)align_up(N * 8);
+    off += 8 * align_up(N * 8);
+  }
   fp.slot_bytes = off;
   fp.only_plan = 0xffffffffu;
   return fp;

@@ -225,6 +225,8 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
   uint32_t* const idx[2] = {reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[0]), reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[1])};
   int32_t* sv = reinterpret_cast<int32_t*>(slot_mem + fp.off_sv);
   int32_t* scpu = reinterpret_cast<int32_t*>(slot_mem + fp.off_scpu);
+  auto done_of = [&](uint32_t s) { return reinterpret_cast<int64_t*>(slot_mem + fp.off_done + (size_t)s * fp.done_stride); };
+  const bool join = prm.join != 0;  // R25: a request reaches a stage when its predecessor stages are done
   const int64_t delay = prm.edge_delay;
   const uint32_t lt_mask = (1u << lane) - 1u;
 
@@ -323,6 +325,16 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
             const uint32_t n = n0 + lane, pos = M + __popc(b & lt_mask);
             const bool first = (r.vm & ((1u << s) - 1u)) == 0u;
             a = x_cur + (first ? 0 : delay);  // R9: a hop delay after the first visit
+            if (join) {  // R25: after every predecessor stage of the request, plus that edge's delay; else at A_n
+              a = (int64_t)((r.cu * (uint64_t)period + 32768ull) >> 16);
+              uint32_t pm = prm.topo_pred[topo_id * 64u + r.t * 8u + s] & r.vm;
+              while (pm) {
+                const uint32_t sp = (uint32_t)__ffs((int)pm) - 1u;
+                pm &= pm - 1u;
+                const int64_t dsp = done_of(sp)[n] + delay;
+                a = dsp > a ? dsp : a;
+              }
+            }
             key[0][pos] = a;
             idx[0][pos] = n;
             sv[n] = S;
@@ -410,7 +422,15 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
               if (lane == j) d = D;
             }
           }
-          if (e < M) xs[n] = d;
+          if (e < M) {
+            if (join) {  // the request is done when its last branch is
+              done_of(s)[n] = d;
+              const int64_t xo = xs[n];
+              xs[n] = d > xo ? d : xo;
+            } else {
+              xs[n] = d;
+            }
+          }
         }
         __syncwarp();
       }

@@ -141,6 +141,53 @@ def test_routes_overlap_and_wide_graph(cf, orc):
     check(cf, orc, g, pl, rates, W.Slo(rng.integers(50_000, 400_000, T), [9] * T, [10] * T), 77)
 
 
+def test_forkjoin_under_arrival_order(cf, orc):
+    """R25 + R27: predecessor stages gate a request's arrival at a stage; service in order of readiness."""
+    w = W.config4_sweep(n_req=1700, n_trials=2, vectors_per_pattern=3, n_variants=1)   # 8 types, up to 3 parallel encoders
+    g, pl = w.graph, w.plans
+    g.join_mode, g.order_mode = 1, 1
+    rates = np.maximum(W.rate_grid(W.flow_bound_mrps(g, pl), [0.05, 0.8, 1.3]), 1)
+    for delay in (0, 9_000):
+        g.edge_delay_us = delay
+        a = check(cf, orc, g, pl, rates, w.slo, w.seed, 2)
+    g.order_mode = 0
+    b = orc.eval_plans(g, pl, rates, w.slo, w.seed, 2, n_threads=NT)
+    g.order_mode = 1
+    assert (a["dep_sum"] != b["dep_sum"]).any()
+    for p in (0, 40, 95):
+        t = cf.cf_trace_sim(g, pl, p, int(rates[p, 1]), 1, w.seed, variant=2)
+        o = orc.trace_sim(g, pl, p, int(rates[p, 1]), 1, w.seed, variant=2)
+        np.testing.assert_array_equal(t["departure"].cpu().numpy(), o["departure"])
+    hi = orc.flow_bound(g, pl, 3, 2)["rate_mrps"]
+    bb = cf.cf_goodput_bisect(g, pl, hi, 9, w.slo, w.seed)
+    bo = orc.goodput_bisect(g, pl, hi, 9, w.slo, w.seed, n_threads=NT)
+    np.testing.assert_array_equal(cf.to_numpy_u32(bb["rate_mrps"]), bo["rate_mrps"])
+    np.testing.assert_array_equal(cf.to_numpy_u32(bb["counts"]), bo["counts"])
+    # with CPU-GPU overlap on the encoders on top (R24 + R25 + R27)
+    g.tabs = g.tabs + [W.lognormal_qtab(25_000.0, 0.5), W.lognormal_qtab(220_000.0, 0.6), W.exponential_qtab(8_000.0)]
+    cpu = np.full(6 * 8, 0xFFFF, np.uint16)
+    for i in range(3):
+        cpu[i * 8:(i + 1) * 8] = 6 + i
+    g.cpu_tab = cpu
+    check(cf, orc, g, pl, rates, w.slo, w.seed, 1)
+    # an 8-component DAG with two fan-ins, 8 stages
+    rng = np.random.default_rng(4)
+    C = T = 8
+    tabs = [W.lognormal_qtab(float(rng.integers(5_000, 60_000)), 0.5) for _ in range(C)]
+    masks = [int(m) | 1 << int(rng.integers(0, C)) for m in rng.integers(0, 256, T)]
+    edges = [[0, 3], [1, 3], [2, 3], [3, 4], [3, 5], [4, 6], [5, 6], [6, 7]]
+    g = W.Graph(C, T, 1000, 2, masks, W.mix_thresholds(rng.dirichlet(np.ones(T))), np.repeat(np.arange(C, dtype=np.uint16), T),
+                tabs, W.gamma_qtab(0.5, 65536.0), edges, edge_delay_us=2_000, join_mode=1, order_mode=1)
+    plan_list = []
+    for _ in range(30):
+        cuts = sorted(rng.choice(np.arange(1, C), size=int(rng.integers(0, C)), replace=False).tolist())
+        bounds = [0] + cuts + [C]
+        plan_list.append([(sum(1 << i for i in range(a, b)), int(rng.integers(1, 9))) for a, b in zip(bounds, bounds[1:])])
+    pl = W.make_plans(plan_list, max_stages=8)
+    rates = np.maximum(W.rate_grid(W.flow_bound_mrps(g, pl), [0.5, 0.9, 1.3]), 1)
+    check(cf, orc, g, pl, rates, W.Slo(rng.integers(50_000, 400_000, T), [9] * T, [10] * T), 77)
+
+
 def test_more_simulations_than_warps_in_flight_and_edge_cases(cf, orc):
     import torch
     g = omni_like(300, n_trials=8)
@@ -158,10 +205,7 @@ def test_more_simulations_than_warps_in_flight_and_edge_cases(cf, orc):
     c = cf.to_numpy_u32(got["counts"])
     assert (c[1, 2] == 0).all()
     np.testing.assert_array_equal(c[0], want["counts"][0])
-    # refusals: fork-join, materialised stream, forced index-order kernels, too many replicas
-    g.join_mode = 1
-    assert cf.cf_eval_plans(g, pl, rates, slo, 9, check=False)["rc"] == cf.CF_ERR_ARG
-    g.join_mode = 0
+    # refusals: materialised stream, too many replicas, unknown mode
     w = W.config4_sweep(n_req=100, n_trials=1, vectors_per_pattern=1, n_patterns=2, n_variants=1)
     w.graph.order_mode = 1
     rec = torch.zeros((1, 1, 100, 32), dtype=torch.uint8, device="cuda")

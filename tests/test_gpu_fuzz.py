@@ -189,7 +189,8 @@ FCFS_SEEDS = list(range(500, 564)) + list(range(18000, 18000 + EXTRA // 4))
 def test_random_arrival_order(cf, orc, seed):
     """Arrival-order service (R27, cf_fcfs.cuh) on the random graphs: radix sorts of 0..5 passes, both
     bodies of the recursion (rates of 1 milli-request/s span more than 2^32 us per batch), replica
-    counts up to 40 (two free-time elements per lane); a third with CPU-GPU overlap, a fourth bisected."""
+    counts up to 40 (two free-time elements per lane); a third with CPU-GPU overlap, a fifth with
+    fork-join, a fourth bisected."""
     w, R_p = random_case(seed)
     g, pl = w.graph, w.plans
     g.order_mode = 1
@@ -202,6 +203,11 @@ def test_random_arrival_order(cf, orc, seed):
             if rng.random() < 0.5:
                 cpu[i * T:(i + 1) * T] = C + int(rng.integers(0, 2))
         g.cpu_tab = cpu
+    if seed % 5 == 1:  # fork-join on top (R25): skip-edges turn the chain into a DAG with parallel branches
+        C = g.n_comp
+        edges = [[i, i + 2] for i in range(C - 2)] + ([[0, 1]] if C > 1 and rng.random() < 0.5 else [])
+        g.edges = np.asarray(edges, dtype=np.uint8).reshape(-1, 2)
+        g.join_mode = 1
     if orc.validate(g, pl) != 0:
         assert seed >= 564  # none of the committed seeds
         pytest.skip("the generator drew services whose worst-case sum exceeds int32 (R17)")

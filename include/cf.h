@@ -261,6 +261,21 @@ int32_t cf_pareto_select(const uint32_t* goodput_mrps, uint32_t n_plans, uint32_
                          const uint8_t* alive, uint8_t* out_pruned, uint32_t* out_best,
                          uint32_t* out_n_survivors, void* workspace, size_t workspace_bytes, void* stream);
 
+/* cf_pareto_select for callers that cannot provide scratch because they cannot allocate device memory
+ * (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): same arguments
+ * without the workspace, same results. Its scratch is a fixed array inside the library,
+ * (32 + CF_PARETO_STATIC_MAX_PLANS) x 8 bytes = 512.25 KiB that every GPU which loads the library holds
+ * until the process exits; n_plans > CF_PARETO_STATIC_MAX_PLANS returns CF_ERR_RANGE (and says so on
+ * stderr) before anything is enqueued. The call allocates nothing (no cudaMalloc / cudaFree): three
+ * kernel launches on `stream`, which must belong to the current device. All calls on a device share
+ * the array: calls that may overlap on the GPU (different streams, concurrent graph branches) race on
+ * it -- keep them on one stream or order them with events. */
+#define CF_PARETO_STATIC_MAX_PLANS 65536u
+uint32_t cf_pareto_static_max_plans(void);
+int32_t cf_pareto_select_static(const uint32_t* goodput_mrps, uint32_t n_plans, uint32_t n_types,
+                                const uint8_t* alive, uint8_t* out_pruned, uint32_t* out_best,
+                                uint32_t* out_n_survivors, void* stream);
+
 /* Releases the host-side cache of prepared calls (waits for uploads still in flight). */
 void cf_cache_clear(void);
 

@@ -25,7 +25,8 @@ EXPORTS = ["cf_workspace_bytes", "cf_eval_plans", "cf_goodput_bisect", "cf_strea
            "cf_materialize_workspace_bytes", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_strerror",
            "cf_workspace_wide_count", "cf_bisect_probes", "cf_aux_workspace_bytes",
-           "cf_pareto_workspace_bytes", "cf_flow_bound", "cf_mc_latency", "cf_pareto_select", "cf_cache_clear"]
+           "cf_pareto_workspace_bytes", "cf_flow_bound", "cf_mc_latency", "cf_pareto_select", "cf_cache_clear",
+           "cf_pareto_select_static", "cf_pareto_static_max_plans"]
 DEBUG_EXPORTS = ["cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
                  "cf_goodput_bisect_stream_opt", "cf_trace_sim_opt", "cf_last_launch_count",
                  "cf_bench_int32_peak"]
@@ -82,8 +83,9 @@ _lib.cf_workspace_wide_count.restype = C.c_int64
 _lib.cf_bisect_probes.restype = C.c_int32
 _lib.cf_aux_workspace_bytes.restype = C.c_size_t
 _lib.cf_pareto_workspace_bytes.restype = C.c_size_t
-for _n in ("cf_flow_bound", "cf_mc_latency", "cf_pareto_select"):
+for _n in ("cf_flow_bound", "cf_mc_latency", "cf_pareto_select", "cf_pareto_select_static"):
     getattr(_lib, _n).restype = C.c_int32
+_lib.cf_pareto_static_max_plans.restype = C.c_uint32
 for _n in ("cf_eval_plans", "cf_goodput_bisect", "cf_materialize_stream", "cf_eval_plans_stream",
            "cf_goodput_bisect_stream", "cf_trace_sim", "cf_workspace_status", "cf_bench_int32_peak",
            "cf_eval_plans_opt", "cf_eval_plans_stream_opt", "cf_goodput_bisect_opt",
@@ -458,3 +460,22 @@ def to_numpy_u32(t: torch.Tensor) -> np.ndarray:
 
 def to_numpy_u64(t: torch.Tensor) -> np.ndarray:
     return t.detach().cpu().numpy().view(np.uint64)
+
+
+def cf_pareto_static_max_plans() -> int:
+    return int(_lib.cf_pareto_static_max_plans())
+
+
+@_on_stream
+def cf_pareto_select_static(goodput_mrps, alive, pruned, best, n_survivors, *, stream=None, check=True):
+    """cf_pareto_select without a workspace (scratch = a fixed array inside the library; at most
+    cf_pareto_static_max_plans() plans). Allocates nothing: every argument is a CUDA tensor the caller
+    made beforehand (goodput_mrps int32 [P,T] contiguous, alive uint8 [P] or None, outputs pruned uint8
+    [P], best int32 [1] or None, n_survivors int32 [1] or None). Returns the status code."""
+    _require_cuda()
+    P, T = goodput_mrps.shape
+    rc = int(_lib.cf_pareto_select_static(_dp(goodput_mrps), C.c_uint32(P), C.c_uint32(T), _dp(alive), _dp(pruned),
+                                          _dp(best), _dp(n_survivors), _stream_ptr(stream)))
+    if check and rc != CF_OK:
+        raise CfError(rc, "cf_pareto_select_static")
+    return rc

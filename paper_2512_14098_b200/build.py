@@ -20,7 +20,8 @@ HEADERS = ["cf_device.cuh", "cf_rel32.cuh", "cf_scan.cuh", "cf_launch.h", "cf_au
 UNITS = [("cf_api", "cf_api.cu", []),
          ("cf_k64", "cf_k64.cu", []),
          ("cf_scan", "cf_scan.cu", []),
-         ("cf_fcfs", "cf_fcfs.cu", [])] + \
+         ("cf_fcfs", "cf_fcfs.cu", []),
+         ("cf_noalloc", "cf_noalloc.cu", [])] + \
         [(f"cf_k32_v{v}c{c}", "cf_k32.cu", [f"-DCF_VMAX={v}", f"-DCF_CMAX={c}"])
          for v, c in ((2, 6), (4, 6), (6, 6), (8, 6), (8, 8))]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -502,10 +502,12 @@ def measure_phases(torch, cf, stream, n_plans=1_000_000):
 
 
 def measure_fidelity(torch, cf, stream):
-    """Sub-record: arrival-order service (cf_graph.order_mode = 1, R27) on configs[1] at
-    full size next to the index-order run of the same call: milliseconds through the C ABI (best of
-    3) and the largest per-type attainment difference between the two disciplines over all (plan,
-    rate). Parity of this variant with the oracle: tests/test_gpu_fcfs.py."""
+    """Sub-record: the simulator fidelity variants, milliseconds through the C
+    ABI (best of 3) and updates/s. Arrival-order service (cf_graph.order_mode = 1, R27) on
+    configs[1] at full size next to the index-order run of the same call, with the largest per-type
+    attainment difference between the two disciplines over all (plan, rate); CPU-GPU overlap (R24),
+    fork-join (R25) and routed plans (R26). Parity of the variants with the oracle:
+    tests/test_gpu_{fcfs,overlap,forkjoin,routing}.py."""
     w = W.config1_mllm()
     g, pl = w.graph, w.plans
     out = {"workload": workload_name(1)}
@@ -531,6 +533,47 @@ def measure_fidelity(torch, cf, stream):
             out["_att0"] = counts[..., 1].sum(axis=2) / np.maximum(counts[..., 0].sum(axis=2), 1)
         del ws
     g.order_mode = 0
+
+    def timed(graph, plans, rates, slo, seed):
+        ws2 = cf.alloc_workspace(graph, plans, rates.shape[1])
+        best2, res2 = None, None
+        for _ in range(3):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            res2 = cf.cf_eval_plans(graph, plans, rates, slo, seed, workspace=ws2, stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            best2 = e0.elapsed_time(e1) if best2 is None else min(best2, e0.elapsed_time(e1))
+        upd2 = int(W.count_updates(graph, plans, cf.to_numpy_u32(res2["counts"])))
+        return {"ms": best2, "updates_per_s": upd2 / (best2 * 1e-3)}
+
+    # CPU-GPU overlap (R24): configs[1] with a CPU pre-processing table (exponential, 10 ms) on the encoder
+    w = W.config1_mllm()
+    w.graph.tabs = list(w.graph.tabs) + [W.exponential_qtab(10_000.0)]
+    cpu = np.full(w.graph.n_comp * w.graph.n_types, 0xFFFF, np.uint16)
+    cpu[0:w.graph.n_types] = len(w.graph.tabs) - 1
+    w.graph.cpu_tab = cpu
+    out["cpu_gpu_overlap"] = dict(timed(w.graph, w.plans, w.rate_mrps, w.slo, w.seed), workload=workload_name(1), kernel="64-bit, HAS_CPU")
+    # fork-join (R25): configs[4]'s graph (up to three encoders in parallel), 512 plans x 4 rates x 8 trials x 2^15
+    w = W.config4_sweep(n_req=1 << 15, vectors_per_pattern=16, n_variants=1)
+    rates = W.rate_grid(W.flow_bound_mrps(w.graph, w.plans), [0.5, 0.7, 0.9, 1.1])
+    base = timed(w.graph, w.plans, rates, w.slo, w.seed)
+    w.graph.join_mode = 1
+    out["fork_join"] = dict(timed(w.graph, w.plans, rates, w.slo, w.seed), path_mode_ms=base["ms"], kernel="64-bit, JOIN",
+                            workload="configs[4] graph, 512 plans x 4 rates x 8 trials x 2^15 requests")
+    # routing (R26): configs[1]'s graph, per plan the disaggregated path AND a colocated node, split 50/50 per type
+    w = W.config1_mllm()
+    P = 256
+    c = w.plans.stage_c[256:512, :2].astype(np.int64)   # the disaggregated plans' (e, l)
+    pl = W.make_plans([[(0b01, int(e)), (0b10, max(1, int(l) // 2)), (0b11, max(1, (int(l) + 1) // 2))] for e, l in c], max_stages=3)
+    rm = np.tile(np.array([[0b011, 0b100], [0b011, 0b100]], np.uint8), (P, 1, 1))
+    rc = np.tile(np.array([[1 << 31, 0xFFFFFFFF], [1 << 31, 0xFFFFFFFF]], np.uint32), (P, 1, 1))
+    routed = W.Plans(pl.n_stages, pl.stage_mask, pl.stage_c, 2, rm, rc)
+    fb = cf.cf_flow_bound(w.graph, routed)
+    rr = W.rate_grid(cf.to_numpy_u32(fb["bound_mrps"]).astype(np.float64), np.arange(0.40, 1.16, 0.05))
+    out["routing"] = dict(timed(w.graph, routed, rr, w.slo, w.seed), kernel="fast kernel, route draw in the 3-word record",
+                          workload="configs[1] graph, 256 plans with two routes per type x 16 rates x 8 trials x 100k requests")
     return out
 
 

@@ -94,7 +94,7 @@ typedef struct {
                                   1: in the order in which they REACH the stage, ties by request index --
                                   textbook FCFS at every node (R27). Runs on
                                   the arrival-order kernel: one warp per simulation, stage by stage, over
-                                  36 N bytes of workspace per simulation in flight (40 N with cpu_tab) plus
+                                  48 N bytes of workspace per simulation in flight (52 N with cpu_tab) plus
                                   80 N K bytes of request records; cf_workspace_bytes asks for 2368
                                   simulations in flight (fewer if that exceeds 16 GiB), a larger workspace
                                   runs up to 2960 at once.

@@ -698,8 +698,8 @@ FcfsParams fcfs_slot_layout(const cf_graph* g) {
   std::memset(&fp, 0, sizeof(fp));
   const size_t N = g->n_req;
   size_t off = align_up(N * 8);
-  for (int b = 0; b < 2; ++b) { fp.off_key[b] = (uint32_t)off; off += align_up(N * 8); }
-  for (int b = 0; b < 2; ++b) { fp.off_idx[b] = (uint32_t)off; off += align_up(N * 4); }
+  for (int b = 0; b < 3; ++b) { fp.off_key[b] = (uint32_t)off; off += align_up(N * 8); }
+  for (int b = 0; b < 3; ++b) { fp.off_idx[b] = (uint32_t)off; off += align_up(N * 4); }
   fp.off_sv = (uint32_t)off;  off += align_up(N * 4);
   fp.off_scpu = (uint32_t)off;
   if (graph_has_cpu(g)) off += align_up(N * 4);

@@ -117,7 +117,8 @@ struct KParams {
 // Request records of the call's trials (drawn once, shared by every simulation of a trial):
 //   records[(trial - trial_base) * N + n] = CompRec<CMAX, HAS_CPU> words with the ABSOLUTE cumulative gap.
 // Scratch of one simulation in flight (byte offsets inside its slot; x at 0):
-//   x int64[N] | key int64[N] x 2 | idx u32[N] x 2 (the radix sort ping-pongs) | sv i32[N] | scpu i32[N]
+//   x int64[N] | key int64[N] x 3 | idx u32[N] x 3 (two for the radix sort to ping-pong, one for the visitors
+//   that are in order by construction) | sv i32[N] | scpu i32[N]
 //   | fork-join (R25): done int64[8][N], the departure of request n from stage s
 struct FcfsParams {
   uint8_t* scratch;
@@ -129,7 +130,7 @@ struct FcfsParams {
   uint32_t R;          // rates per plan
   uint32_t n_sims;     // P * R * k_launch, or 1 with only_plan
   uint32_t only_plan;  // cf_trace_sim: the one plan to run (R = 1); 0xffffffff = all
-  uint32_t off_key[2], off_idx[2], off_sv, off_scpu;
+  uint32_t off_key[3], off_idx[3], off_sv, off_scpu;
   uint32_t off_done, done_stride;  // fork-join: byte offset of done[0], bytes between done[s] and done[s+1]
 };
 

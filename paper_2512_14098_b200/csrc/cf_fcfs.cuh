@@ -11,9 +11,11 @@
 //   phase 0   x[n] = A_n;
 //   per stage gather   the visitors of the stage, compacted with ballots: (arrival = x[n] + hop
 //                      delay, n) and, by request, the summed service (and CPU time, R24) at the stage;
-//             sort     by arrival, stable in the request index: LSD radix sort of the warp's segment,
-//                      8 bits a pass over the bits in which the keys differ (match.any ranks a chunk
-//                      of 32 keys); skipped when the arrivals are already in order (every first stage);
+//             sort     by (arrival, request index). Visitors whose first stage this is arrive at A_n:
+//                      they are in order as they come and form a run of their own; the others get an LSD
+//                      radix sort, 8 bits a pass over the bits in which their keys differ (match.any
+//                      ranks a chunk of 32 keys), skipped when they too are in order; a warp-level merge
+//                      (each lane ranks its pair in the other run's 32-pair window) joins the two runs;
 //             serve    the Kiefer-Wolfowitz recursion in that order with the LANES AS REPLICAS: the
 //                      sorted free-time vector of the stage lives one element per lane (CPL per lane
 //                      for c > 32); replace-min is F'[e] = min(F[e+1], max(F[e], D)) -- one shuffle, one
@@ -188,6 +190,45 @@ __device__ __forceinline__ int warp_radix_sort(int64_t* const (&key)[2], uint32_
   return cur;
 }
 
+// ---- merge of two sorted runs of (key, idx) pairs, ordered by (key, idx): one warp ------------------------
+// Each step holds the next 32 pairs of either run, one per lane; a lane ranks its pair against the other
+// run's window with a binary search over lanes (shuffles); the 32 smallest pairs of the two windows are
+// the next 32 of the merged order (a pair that all 32 of the other window precede is not among them).
+__device__ __forceinline__ bool pair_less(int64_t ka, uint32_t ia, int64_t kb, uint32_t ib) {
+  return ka < kb || (ka == kb && ia < ib);
+}
+__device__ __forceinline__ uint32_t rank_in_window(int64_t wk, uint32_t wi, int64_t k, uint32_t i) {
+  uint32_t lo = 0, hi = 32;  // number of window pairs (sorted across the lanes) that precede (k, i)
+#pragma unroll
+  for (int it = 0; it < 6; ++it) {
+    const uint32_t mid = (lo + hi) >> 1;
+    const int64_t mk = __shfl_sync(kAll, wk, (int)(mid & 31u));
+    const uint32_t mi = __shfl_sync(kAll, wi, (int)(mid & 31u));
+    if (lo < hi) {
+      if (pair_less(mk, mi, k, i)) lo = mid + 1u; else hi = mid;
+    }
+  }
+  return lo;
+}
+__device__ __forceinline__ void warp_merge(const int64_t* Ak, const uint32_t* Ai, uint32_t MA, const int64_t* Bk,
+                                           const uint32_t* Bi, uint32_t MB, int64_t* Ok, uint32_t* Oi, int lane) {
+  uint32_t i = 0, j = 0, o = 0;
+  const uint32_t M = MA + MB;
+  while (o < M) {
+    const bool av = i + lane < MA, bv = j + lane < MB;
+    const int64_t ak = av ? Ak[i + lane] : kInf, bk = bv ? Bk[j + lane] : kInf;
+    const uint32_t ai = av ? Ai[i + lane] : 0xffffffffu, bi = bv ? Bi[j + lane] : 0xffffffffu;
+    const uint32_t pa = (uint32_t)lane + rank_in_window(bk, bi, ak, ai);
+    const uint32_t pb = (uint32_t)lane + rank_in_window(ak, ai, bk, bi);
+    const bool ea = av && pa < 32u, eb = bv && pb < 32u;
+    if (ea) { Ok[o + pa] = ak; Oi[o + pa] = ai; }
+    if (eb) { Ok[o + pb] = bk; Oi[o + pb] = bi; }
+    const uint32_t na = __popc(__ballot_sync(kAll, ea)), nb = __popc(__ballot_sync(kAll, eb));
+    i += na; j += nb; o += na + nb;
+  }
+  __syncwarp();
+}
+
 // ---- Kiefer-Wolfowitz on a sorted free-time vector spread over the warp ----------------------------------
 // Element e = j * 32 + lane lives in F[j] of that lane; elements >= c hold +inf. One visit with arrival
 // a, service S, CPU time Sc (R24: paid when the earliest-free replica is idle at a): departure D, then
@@ -221,8 +262,12 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
   if (wid >= fp.n_slots) return;  // nothing below synchronises the block
   uint8_t* slot_mem = fp.scratch + (size_t)wid * fp.slot_bytes;
   int64_t* xs = reinterpret_cast<int64_t*>(slot_mem);
+  // key / idx [0], [1]: the visitors that come from an earlier stage (the radix sort ping-pongs between them, the
+  // merge writes into the free one); [2]: the visitors whose first stage this is (their arrival is A_n: in order)
   int64_t* const key[2] = {reinterpret_cast<int64_t*>(slot_mem + fp.off_key[0]), reinterpret_cast<int64_t*>(slot_mem + fp.off_key[1])};
   uint32_t* const idx[2] = {reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[0]), reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[1])};
+  int64_t* const keyF = reinterpret_cast<int64_t*>(slot_mem + fp.off_key[2]);
+  uint32_t* const idxF = reinterpret_cast<uint32_t*>(slot_mem + fp.off_idx[2]);
   int32_t* sv = reinterpret_cast<int32_t*>(slot_mem + fp.off_sv);
   int32_t* scpu = reinterpret_cast<int32_t*>(slot_mem + fp.off_scpu);
   auto done_of = [&](uint32_t s) { return reinterpret_cast<int64_t*>(slot_mem + fp.off_done + (size_t)s * fp.done_stride); };
@@ -300,7 +345,7 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
       for (uint32_t s = 0; s < topo.n_stages; ++s) {
         // ---- gather the visitors of stage s ------------------------------------------------------
         const uint32_t sm = topo.mask[s];
-        uint32_t M = 0;
+        uint32_t M = 0, MF = 0;  // visitors from an earlier stage / visitors that start here
         bool unsorted = false;
         int64_t kmin = kInf, kmax = 0, prev_last = 0;
         Req r_nx = load(0, true);
@@ -319,15 +364,22 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
             S += ((sm >> i) & 1u) ? r.svc[i] : 0;
             if (HAS_CPU) Sc += ((sm >> i) & 1u) ? r.cpu[i] : 0;
           }
-          const uint32_t b = __ballot_sync(kAll, vis);
+          // a visitor with no earlier stage (fork-join: no predecessor stage) arrives at A_n: those are in
+          // order as they come and go to their own run; only the others may need sorting
+          bool first = (r.vm & ((1u << s) - 1u)) == 0u;
+          uint32_t pm = 0;
+          if (join && vis) {
+            pm = prm.topo_pred[topo_id * 64u + r.t * 8u + s] & r.vm;
+            first = pm == 0u;
+          }
+          const uint32_t bf = __ballot_sync(kAll, vis && first);
+          const uint32_t b = __ballot_sync(kAll, vis && !first);
           int64_t a = 0;
           if (vis) {
-            const uint32_t n = n0 + lane, pos = M + __popc(b & lt_mask);
-            const bool first = (r.vm & ((1u << s) - 1u)) == 0u;
+            const uint32_t n = n0 + lane;
             a = x_cur + (first ? 0 : delay);  // R9: a hop delay after the first visit
             if (join) {  // R25: after every predecessor stage of the request, plus that edge's delay; else at A_n
               a = (int64_t)((r.cu * (uint64_t)period + 32768ull) >> 16);
-              uint32_t pm = prm.topo_pred[topo_id * 64u + r.t * 8u + s] & r.vm;
               while (pm) {
                 const uint32_t sp = (uint32_t)__ffs((int)pm) - 1u;
                 pm &= pm - 1u;
@@ -335,24 +387,32 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
                 a = dsp > a ? dsp : a;
               }
             }
-            key[0][pos] = a;
-            idx[0][pos] = n;
+            if (first) {
+              const uint32_t pos = MF + __popc(bf & lt_mask);
+              keyF[pos] = a;
+              idxF[pos] = n;
+            } else {
+              const uint32_t pos = M + __popc(b & lt_mask);
+              key[0][pos] = a;
+              idx[0][pos] = n;
+              kmin = a < kmin ? a : kmin;
+              kmax = a > kmax ? a : kmax;
+            }
             sv[n] = S;
             if (HAS_CPU) scpu[n] = Sc;
-            kmin = a < kmin ? a : kmin;
-            kmax = a > kmax ? a : kmax;
           }
-          if (b) {  // in order? every visitor against the visitor before it (the previous chunk's last for the first)
+          if (b) {  // in order? every such visitor against the one before it (the previous chunk's last for the first)
             const uint32_t below = b & lt_mask;
             const int src = below ? 31 - __clz((int)below) : 0;
             const int64_t pa = __shfl_sync(kAll, a, src);
-            if (vis && (below ? pa : prev_last) > a && (below || M > 0)) unsorted = true;
+            if (vis && !first && (below ? pa : prev_last) > a && (below || M > 0)) unsorted = true;
             prev_last = __shfl_sync(kAll, a, 31 - __clz((int)b));
           }
           M += __popc(b);
+          MF += __popc(bf);
         }
         __syncwarp();
-        if (M == 0) continue;
+        if (M + MF == 0) continue;
         // ---- order of service: by arrival, ties by index -----------------------------------------------
         int cur = 0;
         if (__any_sync(kAll, unsorted)) {
@@ -367,6 +427,13 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
         }
         const int64_t* ks = key[cur];
         const uint32_t* is = idx[cur];
+        if (M == 0) {
+          ks = keyF; is = idxF;
+        } else if (MF != 0) {  // two sorted runs -> one
+          warp_merge(keyF, idxF, MF, key[cur], idx[cur], M, key[cur ^ 1], idx[cur ^ 1], lane);
+          ks = key[cur ^ 1]; is = idx[cur ^ 1];
+        }
+        M += MF;
         // ---- serve in that order, lanes as replicas -------------------------------------------------
         const uint32_t c = prm.plan_c[plan * 8 + s];
         int64_t F[CPL];

@@ -210,14 +210,39 @@ __device__ __forceinline__ uint32_t rank_in_window(int64_t wk, uint32_t wi, int6
   }
   return lo;
 }
+// The runs stream from HBM through a ring of kRing pairs per run in shared memory: a chunk of 32 is loaded
+// into registers as soon as the ring has room for it and stored two steps later, so no step waits for a
+// load it has just issued (a run gives at most 32 pairs a step: the ring is always 3 chunks ahead).
+constexpr uint32_t kRing = 256;
+struct MergePend { int64_t k; uint32_t i, pos; bool v; };
 __device__ __forceinline__ void warp_merge(const int64_t* Ak, const uint32_t* Ai, uint32_t MA, const int64_t* Bk,
-                                           const uint32_t* Bi, uint32_t MB, int64_t* Ok, uint32_t* Oi, int lane) {
+                                           const uint32_t* Bi, uint32_t MB, int64_t* Ok, uint32_t* Oi,
+                                           int64_t* ringk, uint32_t* ringi, int lane) {  // rings: [2][kRing]
+  int64_t* rak = ringk; int64_t* rbk = ringk + kRing;
+  uint32_t* rai = ringi; uint32_t* rbi = ringi + kRing;
+  for (uint32_t t = lane; t < min(MA, kRing); t += 32) { rak[t] = Ak[t]; rai[t] = Ai[t]; }
+  for (uint32_t t = lane; t < min(MB, kRing); t += 32) { rbk[t] = Bk[t]; rbi[t] = Bi[t]; }
+  uint32_t ta = min(MA, kRing), tb = min(MB, kRing);  // pairs of the run issued so far
+  MergePend pa0{0, 0, 0, false}, pa1 = pa0, pb0 = pa0, pb1 = pa0;
+  __syncwarp();
   uint32_t i = 0, j = 0, o = 0;
   const uint32_t M = MA + MB;
   while (o < M) {
+    MergePend na_{0, 0, 0, false}, nb_ = na_;
+    if (ta < MA && ta - i <= kRing - 32u) {  // room for [ta, ta + 32): its slots hold pairs already consumed
+      na_.v = true; na_.pos = ta;
+      if (ta + lane < MA) { na_.k = Ak[ta + lane]; na_.i = Ai[ta + lane]; }
+      ta += 32u;
+    }
+    if (tb < MB && tb - j <= kRing - 32u) {
+      nb_.v = true; nb_.pos = tb;
+      if (tb + lane < MB) { nb_.k = Bk[tb + lane]; nb_.i = Bi[tb + lane]; }
+      tb += 32u;
+    }
     const bool av = i + lane < MA, bv = j + lane < MB;
-    const int64_t ak = av ? Ak[i + lane] : kInf, bk = bv ? Bk[j + lane] : kInf;
-    const uint32_t ai = av ? Ai[i + lane] : 0xffffffffu, bi = bv ? Bi[j + lane] : 0xffffffffu;
+    const uint32_t sa = (i + lane) & (kRing - 1u), sb = (j + lane) & (kRing - 1u);
+    const int64_t ak = av ? rak[sa] : kInf, bk = bv ? rbk[sb] : kInf;
+    const uint32_t ai = av ? rai[sa] : 0xffffffffu, bi = bv ? rbi[sb] : 0xffffffffu;
     const uint32_t pa = (uint32_t)lane + rank_in_window(bk, bi, ak, ai);
     const uint32_t pb = (uint32_t)lane + rank_in_window(ak, ai, bk, bi);
     const bool ea = av && pa < 32u, eb = bv && pb < 32u;
@@ -225,6 +250,11 @@ __device__ __forceinline__ void warp_merge(const int64_t* Ak, const uint32_t* Ai
     if (eb) { Ok[o + pb] = bk; Oi[o + pb] = bi; }
     const uint32_t na = __popc(__ballot_sync(kAll, ea)), nb = __popc(__ballot_sync(kAll, eb));
     i += na; j += nb; o += na + nb;
+    __syncwarp();  // every lane has read its window: slots of consumed pairs may be overwritten
+    if (pa0.v) { const uint32_t t = (pa0.pos + lane) & (kRing - 1u); rak[t] = pa0.k; rai[t] = pa0.i; }
+    if (pb0.v) { const uint32_t t = (pb0.pos + lane) & (kRing - 1u); rbk[t] = pb0.k; rbi[t] = pb0.i; }
+    pa0 = pa1; pa1 = na_; pb0 = pb1; pb1 = nb_;
+    __syncwarp();
   }
   __syncwarp();
 }
@@ -257,6 +287,8 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
   constexpr int kW = CompRec<CMAX, HAS_CPU>::kWords;
   constexpr int kB = CompRec<CMAX, HAS_CPU>::kBase;
   __shared__ uint32_t cnt_s[kFcfsWarps][256];
+  __shared__ int64_t ringk_s[kFcfsWarps][2 * kRing];
+  __shared__ uint32_t ringi_s[kFcfsWarps][2 * kRing];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t wid = blockIdx.x * kFcfsWarps + warp;
   if (wid >= fp.n_slots) return;  // nothing below synchronises the block
@@ -430,7 +462,7 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
         if (M == 0) {
           ks = keyF; is = idxF;
         } else if (MF != 0) {  // two sorted runs -> one
-          warp_merge(keyF, idxF, MF, key[cur], idx[cur], M, key[cur ^ 1], idx[cur ^ 1], lane);
+          warp_merge(keyF, idxF, MF, key[cur], idx[cur], M, key[cur ^ 1], idx[cur ^ 1], ringk_s[warp], ringi_s[warp], lane);
           ks = key[cur ^ 1]; is = idx[cur ^ 1];
         }
         M += MF;

@@ -17,8 +17,8 @@
 //                      ranks a chunk of 32 keys), skipped when they too are in order; a warp-level merge
 //                      (each lane ranks its pair in the other run's 32-pair window) joins the two runs;
 //             serve    the Kiefer-Wolfowitz recursion in that order with the LANES AS REPLICAS: the
-//                      sorted free-time vector of the stage lives one element per lane (CPL per lane
-//                      for c > 32); replace-min is F'[e] = min(F[e+1], max(F[e], D)) -- one shuffle, one
+//                      sorted free-time vector of the stage lives one element per lane (CPL consecutive
+//                      elements per lane for c > 32); replace-min is F'[e] = min(F[e+1], max(F[e], D)) -- one shuffle, one
 //                      max, one min, no search for the insertion point. A batch of 32 visits whose
 //                      times span less than 2^32 us runs on 32-bit offsets from the batch's first
 //                      arrival (free times before it are clamped to it: exact, they are "idle");
@@ -260,23 +260,23 @@ __device__ __forceinline__ void warp_merge(const int64_t* Ak, const uint32_t* Ai
 }
 
 // ---- Kiefer-Wolfowitz on a sorted free-time vector spread over the warp ----------------------------------
-// Element e = j * 32 + lane lives in F[j] of that lane; elements >= c hold +inf. One visit with arrival
-// a, service S, CPU time Sc (R24: paid when the earliest-free replica is idle at a): departure D, then
-// the minimum leaves and D enters: F'[e] = min(F[e+1], max(F[e], D)) (F sorted, F[0] <= D).
+// Lane l holds elements l * CPL .. l * CPL + CPL - 1 in F[0..CPL); elements >= c hold +inf. One visit with
+// arrival a, service S, CPU time Sc (R24: paid when the earliest-free replica is idle at a): departure D, then
+// the minimum leaves and D enters: F'[e] = min(F[e+1], max(F[e], D)) (F sorted, F[0] <= D). The serve loop
+// costs two shuffles on the vector whatever CPL is: the minimum from lane 0 and the neighbour's first element.
 template <int CPL, bool HAS_CPU, typename TT>
 __device__ __forceinline__ TT kw_visit(TT (&F)[CPL], TT a, uint32_t S, uint32_t Sc, TT inf, int lane) {
   const TT f0 = __shfl_sync(kAll, F[0], 0);
+  TT next = __shfl_sync(kAll, F[0], (lane + 1) & 31);
+  if (lane == 31) next = inf;
   TT D;
   if (HAS_CPU) D = (f0 <= a) ? a + (TT)Sc + (TT)S : f0 + (TT)S;
   else D = (f0 > a ? f0 : a) + (TT)S;
 #pragma unroll
   for (int j = 0; j < CPL; ++j) {
-    TT next = __shfl_sync(kAll, F[j], (lane + 1) & 31);
-    TT wrap = inf;
-    if (j + 1 < CPL) wrap = __shfl_sync(kAll, F[j + 1 < CPL ? j + 1 : j], 0);
-    if (lane == 31) next = wrap;
+    const TT nx = j + 1 < CPL ? F[j + 1 < CPL ? j + 1 : j] : next;
     const TT up = F[j] > D ? F[j] : D;
-    F[j] = next < up ? next : up;
+    F[j] = nx < up ? nx : up;
   }
   return D;
 }
@@ -470,7 +470,7 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
         const uint32_t c = prm.plan_c[plan * 8 + s];
         int64_t F[CPL];
 #pragma unroll
-        for (int j = 0; j < CPL; ++j) F[j] = (uint32_t)(j * 32 + lane) < c ? 0 : kInf;
+        for (int j = 0; j < CPL; ++j) F[j] = (uint32_t)(lane * CPL + j) < c ? 0 : kInf;
         // the sorted pairs are loaded two batches ahead, the services they point to one batch ahead
         int64_t a_n1 = 0, a_n2 = 0;
         uint32_t n_n1 = 0, n_n2 = 0, S_n1 = 0, Sc_n1 = 0;
@@ -490,8 +490,8 @@ cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ Fcfs
           int64_t fm = 0;  // the largest free time: element c - 1 of the sorted vector
 #pragma unroll
           for (int j = 0; j < CPL; ++j) {
-            const int64_t v = __shfl_sync(kAll, F[j], (c - 1u) & 31u);
-            if ((uint32_t)j == ((c - 1u) >> 5)) fm = v;
+            const int64_t v = __shfl_sync(kAll, F[j], (int)((c - 1u) / CPL));
+            if ((uint32_t)j == (c - 1u) % CPL) fm = v;
           }
           const uint32_t work = (e < M) ? S + Sc : 0u;
           const bool big = __any_sync(kAll, work >= (1u << 26));

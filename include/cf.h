@@ -95,9 +95,9 @@ typedef struct {
                                   textbook FCFS at every node (R27). Runs on
                                   the arrival-order kernel: one warp per simulation, stage by stage, over
                                   48 N bytes of workspace per simulation in flight (52 N with cpu_tab) plus
-                                  80 N K bytes of request records; cf_workspace_bytes asks for 2368
-                                  simulations in flight (fewer if that exceeds 16 GiB), a larger workspace
-                                  runs up to 2960 at once.
+                                  80 N K bytes of request records; cf_workspace_bytes asks for 3552
+                                  simulations in flight (fewer if that exceeds 16 GiB): the warps a B200 holds
+                                  at once.
                                   Replicas per stage <= 256; no stream. With join_mode = 1 a slot holds 64 N
                                   bytes more (the departure of every request from every stage).            */
 } cf_graph;

@@ -691,7 +691,7 @@ cudaError_t launch_scan(KParams kp, const Schedule& sc, uint32_t n_trials, cudaS
 }
 
 // ---- arrival-order kernel (cf_fcfs.cuh): scratch of the simulations in flight, after `used` bytes of workspace
-constexpr uint32_t kFcfsAskSlots = 148 * 16, kFcfsMaxSlots = 148 * 20;  // measured best: 20 warps per SM (more thrash L2)
+constexpr uint32_t kFcfsAskSlots = 148 * 24, kFcfsMaxSlots = 148 * 24;  // 24 warps per SM measured best of 16 / 20 / 24 / 28 (the launch clamps to what the device holds at once)
 
 FcfsParams fcfs_slot_layout(const cf_graph* g) {
   FcfsParams fp;

@@ -1,4 +1,6 @@
 // cf_fcfs.cu -- instantiations and launches of the arrival-order kernels (cf_fcfs.cuh).
+#include <algorithm>
+
 #include "cf_launch.h"
 #include "cf_fcfs.cuh"
 
@@ -7,15 +9,25 @@ namespace cfk {
 namespace {
 template <int CMAX, bool HAS_CPU>
 cudaError_t launch_cpl(int cpl, const KParams& kp, const FcfsParams& fp, cudaStream_t st) {
-  const uint32_t blocks = (fp.n_slots + kFcfsWarps - 1) / kFcfsWarps;
-  const dim3 b(kFcfsWarps * 32);
+  // one wave: no more warps than the device holds at once (a simulation in flight is a warp with a
+  // scratch slot; the call's simulations take turns on them, so a second, thin wave would only add a tail)
+  void (*kern)(KParams, FcfsParams) = nullptr;
   switch (cpl) {
-    case 1: cf_fcfs_kernel<CMAX, HAS_CPU, 1><<<blocks, b, 0, st>>>(kp, fp); break;
-    case 2: cf_fcfs_kernel<CMAX, HAS_CPU, 2><<<blocks, b, 0, st>>>(kp, fp); break;
-    case 4: cf_fcfs_kernel<CMAX, HAS_CPU, 4><<<blocks, b, 0, st>>>(kp, fp); break;
-    case 8: cf_fcfs_kernel<CMAX, HAS_CPU, 8><<<blocks, b, 0, st>>>(kp, fp); break;
+    case 1: kern = cf_fcfs_kernel<CMAX, HAS_CPU, 1>; break;
+    case 2: kern = cf_fcfs_kernel<CMAX, HAS_CPU, 2>; break;
+    case 4: kern = cf_fcfs_kernel<CMAX, HAS_CPU, 4>; break;
+    case 8: kern = cf_fcfs_kernel<CMAX, HAS_CPU, 8>; break;
     default: return cudaErrorInvalidValue;
   }
+  int dev = 0, sms = 0, per_sm = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kFcfsWarps * 32, 0);
+  if (e != cudaSuccess) return e;
+  FcfsParams f = fp;
+  f.n_slots = std::min<uint32_t>(fp.n_slots, (uint32_t)std::max(1, sms * per_sm) * kFcfsWarps);
+  const uint32_t blocks = (f.n_slots + kFcfsWarps - 1) / kFcfsWarps;
+  kern<<<blocks, kFcfsWarps * 32, 0, st>>>(kp, f);
   return cudaGetLastError();
 }
 }  // namespace

@@ -282,7 +282,7 @@ __device__ __forceinline__ TT kw_visit(TT (&F)[CPL], TT a, uint32_t S, uint32_t 
 }
 
 template <int CMAX, bool HAS_CPU, int CPL>
-__global__ void __launch_bounds__(kFcfsWarps * 32)
+__global__ void __launch_bounds__(kFcfsWarps * 32, 6)
 cf_fcfs_kernel(const __grid_constant__ KParams prm, const __grid_constant__ FcfsParams fp) {
   constexpr int kW = CompRec<CMAX, HAS_CPU>::kWords;
   constexpr int kB = CompRec<CMAX, HAS_CPU>::kBase;

@@ -18,8 +18,9 @@
 //                      (each lane ranks its pair in the other run's 32-pair window) joins the two runs;
 //             serve    the Kiefer-Wolfowitz recursion in that order with the LANES AS REPLICAS: the
 //                      sorted free-time vector of the stage lives one element per lane (CPL consecutive
-//                      elements per lane for c > 32); replace-min is F'[e] = min(F[e+1], max(F[e], D)) -- one shuffle, one
-//                      max, one min, no search for the insertion point. A batch of 32 visits whose
+//                      elements per lane for c > 32); replace-min is F'[e] = min(F[e+1], max(F[e], D)):
+//                      two shuffles a visit, one max and one min per element, no search for the
+//                      insertion point. A batch of 32 visits whose
 //                      times span less than 2^32 us runs on 32-bit offsets from the batch's first
 //                      arrival (free times before it are clamped to it: exact, they are "idle");
 //   last      per-type counts and hits, checksum, makespan from x[n] - A_n.
